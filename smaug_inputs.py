@@ -1,0 +1,115 @@
+"""Seeded / analytic input generators shared by the tests, bench.py and smoke() for BOTH the oracle and
+the CUDA path.  numpy only.  Holds none of the method's arithmetic: it only tabulates initial conditions
+(BASELINE.json "configs"; PAPER.md:99-112 Orszag-Tang, PAPER.md:130 Brio-Wu) on the cell-centred grid
+x_i = (i + 1/2) Lx / nx and converts primitive (rho, v, p, B) to the stored variables
+w = (rho, mx, my, e, bx, by), e = p/(gamma-1) + rho v^2/2 + B^2/2 (PAPER.md:39-43 solved for e).
+
+The workloads are analytic, so they stand in for no external dataset (the paper uses none).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2
+FIELDS = ("rho", "mx", "my", "e", "bx", "by")
+
+
+def centres(n: int, length: float = 1.0) -> np.ndarray:
+    return (np.arange(n, dtype=np.float64) + 0.5) * (length / n)
+
+
+def prim_to_cons(rho, vx, vy, p, bx, by, gamma: float) -> np.ndarray:
+    rho, vx, vy, p, bx, by = np.broadcast_arrays(rho, vx, vy, p, bx, by)
+    e = p / (gamma - 1.0) + 0.5 * rho * (vx * vx + vy * vy) + 0.5 * (bx * bx + by * by)
+    return np.ascontiguousarray(np.stack([rho, rho * vx, rho * vy, e, bx, by]).astype(np.float64))
+
+
+def orszag_tang(nx: int, ny: int | None = None, gamma: float = 5.0 / 3.0, symmetrise: bool = False):
+    """BASELINE.json configs 2-5: rho=25/(36 pi), p=5/(12 pi), vx=-sin 2 pi y, vy=sin 2 pi x,
+    Bx=-sin(2 pi y)/sqrt(4 pi), By=sin(4 pi x)/sqrt(4 pi) on [0,1]^2, periodic.
+    Returns (w[6,ny,nx], bc, gamma).  symmetrise=True makes the 180-degree point symmetry exact in fp."""
+    ny = nx if ny is None else ny
+    x = centres(nx)[None, :]
+    y = centres(ny)[:, None]
+    rho = 25.0 / (36.0 * np.pi)
+    p = 5.0 / (12.0 * np.pi)
+    b0 = 1.0 / np.sqrt(4.0 * np.pi)
+    one = np.ones((ny, nx))
+    w = prim_to_cons(rho * one, -np.sin(2 * np.pi * y) * one, np.sin(2 * np.pi * x) * one, p * one,
+                     -b0 * np.sin(2 * np.pi * y) * one, b0 * np.sin(4 * np.pi * x) * one, gamma)
+    if symmetrise:
+        sign = np.array([1, -1, -1, 1, -1, -1], dtype=np.float64)[:, None, None]
+        w = 0.5 * (w + sign * w[:, ::-1, ::-1])
+    return np.ascontiguousarray(w), (BC_PERIODIC,) * 4, gamma
+
+
+def brio_wu(nx: int = 800, ny: int = 1, gamma: float = 2.0, transpose: bool = False):
+    """BASELINE.json config 1: left (x<0.5) rho=1,p=1,By=1; right rho=0.125,p=0.1,By=-1; Bx=0.75, v=0;
+    open in x, periodic in y (y-invariant).  transpose=True swaps the roles of x and y.
+    Returns (w, bc, gamma)."""
+    x = centres(nx)[None, :] * np.ones((ny, 1))
+    left = x < 0.5
+    rho = np.where(left, 1.0, 0.125)
+    p = np.where(left, 1.0, 0.1)
+    by = np.where(left, 1.0, -1.0)
+    bx = 0.75 * np.ones_like(x)
+    zero = np.zeros_like(x)
+    w = prim_to_cons(rho, zero, zero, p, bx, by, gamma)
+    bc = (BC_OPEN, BC_OPEN, BC_PERIODIC, BC_PERIODIC)
+    if transpose:
+        w = transpose_state(w)
+        bc = (BC_PERIODIC, BC_PERIODIC, BC_OPEN, BC_OPEN)
+    return w, bc, gamma
+
+
+def transpose_state(w: np.ndarray) -> np.ndarray:
+    """The x<->y mirrored problem: swap axes and swap the x/y components."""
+    wt = np.transpose(w, (0, 2, 1))
+    return np.ascontiguousarray(wt[[0, 2, 1, 3, 5, 4]])
+
+
+def smooth_random(nx: int, ny: int, seed: int = 1710, kmax: int = 4, amp: float = 1e-3,
+                  gamma: float = 5.0 / 3.0, mean=None):
+    """Periodic random smooth state: Orszag-Tang mean state (rho, p) with v=0, B=mean B, plus a sum of
+    Fourier modes |k| <= kmax of relative amplitude `amp` on each primitive variable (SURVEY P2 recipe).
+    Returns (w, bc, gamma)."""
+    rng = np.random.default_rng(seed)
+    x = centres(nx)[None, :]
+    y = centres(ny)[:, None]
+    if mean is None:
+        mean = dict(rho=25.0 / (36.0 * np.pi), p=5.0 / (12.0 * np.pi), vx=0.0, vy=0.0, bx=0.2, by=0.1)
+
+    def field(scale):
+        f = np.zeros((ny, nx))
+        norm = 0.0
+        for kx in range(-kmax, kmax + 1):
+            for ky in range(0, kmax + 1):
+                if kx * kx + ky * ky > kmax * kmax or (kx == 0 and ky == 0):
+                    continue
+                a, ph = rng.normal(), rng.uniform(0, 2 * np.pi)
+                f += a * np.cos(2 * np.pi * (kx * x + ky * y) + ph)
+                norm += abs(a)
+        return scale * amp * f / norm          # grid-independent normalisation: |field| <= scale*amp
+
+    rho = mean["rho"] + field(mean["rho"])
+    p = mean["p"] + field(mean["p"])
+    vx = mean["vx"] + field(1.0)
+    vy = mean["vy"] + field(1.0)
+    bx = mean["bx"] + field(1.0)
+    by = mean["by"] + field(1.0)
+    return prim_to_cons(rho, vx, vy, p, bx, by, gamma), (BC_PERIODIC,) * 4, gamma
+
+
+def uniform_background(nx: int, ny: int, rho_b: float, e_b: float, bx_b: float, by_b: float) -> np.ndarray:
+    bg = np.empty((4, ny, nx))
+    bg[0], bg[1], bg[2], bg[3] = rho_b, e_b, bx_b, by_b
+    return bg
+
+
+def rel_l2(a: np.ndarray, ref: np.ndarray) -> np.ndarray:
+    """c-9 error metric per field: ||a_f - ref_f||_2 / ||ref_f||_2; where the denominator is 0 the
+    numerator is divided by max_f ||ref_f||_2 instead."""
+    num = np.sqrt(((a - ref) ** 2).reshape(a.shape[0], -1).sum(1))
+    den = np.sqrt((ref ** 2).reshape(ref.shape[0], -1).sum(1))
+    fallback = den.max() if den.max() > 0 else 1.0
+    return num / np.where(den > 0, den, fallback)
