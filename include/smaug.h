@@ -1,0 +1,125 @@
+/* smaug.h -- C ABI of the B200-native SMAUG+ hot path: one full 2-D MHD time step on one GPU.
+ *
+ * What the library computes (citations: /root/reference/PAPER.md = "PAPER.md"; DESIGN.md section 3 lists
+ * every reading "c-1".."c-9" taken where the paper is silent):
+ *   - the SAC/VAC-style split ideal-MHD right-hand side for the perturbed variables
+ *     w = (rho~, mx, my, e~, bx~, by~) on a static background (rho_b, e_b, Bbx, Bby)   PAPER.md:35-43, c-2
+ *   - 4th-order central differences of the flux components                                PAPER.md:45,    c-3
+ *   - hyperdiffusion / hyper-resistivity with the coefficient "ratio of the forward
+ *     difference ... to third order and first order" times the max wave speed             PAPER.md:45-49, c-5
+ *   - the Runge-Kutta stage updates (classical RK4; 2 = midpoint, 1 = Euler)              PAPER.md:45,    c-6
+ *   - ghost-cell (halo) fill, periodic / open / fixed, in device memory                   PAPER.md:59,101, c-8
+ *   - the max-wavespeed reduction and the CFL time step                                   PAPER.md:45,    c-4, c-7
+ * Every step of that path runs in hand-written fp64 CUDA kernels for sm_100a; there is no CPU fallback
+ * (every entry point fails with SMAUG_ECUDA when no CUDA device is usable).
+ *
+ * Conventions
+ *   - Arrays are fp64, SoA, field-major, row-major with x fastest, INTERIOR CELLS ONLY:
+ *       state      w  [6][ny][nx]  order rho~, mx, my, e~, bx~, by~
+ *       background bg [4][ny][nx]  order rho_b, e_b, Bbx, Bby          (NULL = zero background)
+ *     Pointers may be HOST or DEVICE memory (detected with cudaPointerGetAttributes); the caller owns
+ *     them and the library copies; nothing is retained after the call returns.
+ *   - Grid: cell centres x_i = (i+1/2) Lx/nx, y_j = (j+1/2) Ly/ny; Lx = Ly = 1 by default.  Ghost width 3.
+ *   - Return value: 0 = SMAUG_OK, negative = error; smaug_last_error() gives a thread-local message.
+ *     No exception crosses the ABI.  No global state except that message.
+ *   - A context is not thread-safe; use one context per host thread (or lock).
+ *   - All work is enqueued on the context's stream (default: the legacy default stream 0; pass torch's
+ *     current stream with smaug_set_stream).  smaug_step / smaug_get_state / smaug_get_time synchronise
+ *     that stream before returning; smaug_step_async does not.
+ */
+#ifndef SMAUG_H_
+#define SMAUG_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct smaug_ctx smaug_ctx; /* opaque, library-owned */
+
+enum { SMAUG_BC_PERIODIC = 0, SMAUG_BC_OPEN = 1, SMAUG_BC_FIXED = 2 };
+
+enum {
+  SMAUG_OK = 0,
+  SMAUG_EINVAL = -1,    /* bad argument: nx<1, ny<1, gamma<=1, unknown bc, periodic on one side only, NULL */
+  SMAUG_ENOMEM = -2,    /* device allocation failed / workspace too small */
+  SMAUG_ECUDA = -3,     /* CUDA runtime error (message in smaug_last_error), incl. "no device" */
+  SMAUG_ENONFINITE = -4 /* a time step was non-finite or <= 0; the state is then unspecified */
+};
+
+enum { /* keys of smaug_set_param */
+  SMAUG_PARAM_LX = 0,       /* domain length in x, > 0 (default 1) */
+  SMAUG_PARAM_LY = 1,       /* domain length in y, > 0 (default 1) */
+  SMAUG_PARAM_HD_ON = 2,    /* 0 = no hyperdiffusion ("Without HD" column of PAPER.md Table 1), else on (default) */
+  SMAUG_PARAM_C_RHO = 3,    /* hyperdiffusion coefficients c_u of c-5, >= 0; defaults 0.02, */
+  SMAUG_PARAM_C_MOM = 4,    /*   0.4, */
+  SMAUG_PARAM_C_E = 5,      /*   0.02, */
+  SMAUG_PARAM_C_B = 6,      /*   0.02 */
+  SMAUG_PARAM_RK_ORDER = 7, /* 4 (default), 2 (midpoint) or 1 (forward Euler) */
+  SMAUG_PARAM_FIXED_DT = 8  /* > 0: use this dt instead of the CFL step; 0 (default): CFL */
+};
+
+/* Bytes of device memory a context for an nx-by-ny grid needs (has_bg != 0: a background is given).
+ * Returns 0 if nx or ny is < 1. */
+size_t smaug_workspace_bytes(int nx, int ny, int has_bg);
+
+/* Create a context.  bc = {x_lo, x_hi, y_lo, y_hi}; periodic must be set on both sides of an axis.
+ * bg: background [4][ny][nx] (host or device) or NULL.  Its ghosts are filled once (periodic -> wrap,
+ * else nearest interior cell).  The library allocates device memory with cudaMalloc. */
+int smaug_create(int nx, int ny, double gamma, const int bc[4], const double* bg, smaug_ctx** out);
+
+/* Same, but all device memory is carved out of `workspace` (DEVICE pointer, 256-byte aligned, at least
+ * smaug_workspace_bytes(nx, ny, bg != NULL) bytes, e.g. a torch uint8 tensor) which the caller keeps
+ * alive until smaug_destroy.  `stream` is a cudaStream_t (NULL = default stream). */
+int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], const double* bg,
+                              void* workspace, size_t workspace_bytes, void* stream, smaug_ctx** out);
+
+/* cudaStream_t on which all later work of this context is enqueued. */
+int smaug_set_stream(smaug_ctx* ctx, void* stream);
+
+int smaug_set_param(smaug_ctx* ctx, int key, double value);
+
+/* Load the perturbed state w [6][ny][nx] (host or device), fill its ghosts (fixed sides are frozen at
+ * the nearest-interior value from now on), reduce its wave-speed maxima, reset t = 0. */
+int smaug_set_state(smaug_ctx* ctx, const double* w);
+
+/* Advance n_steps time steps: per step  dt = cfl * min_d(Delta_d / cmax_d)  (c-7; an axis with n = 1 is
+ * excluded; or SMAUG_PARAM_FIXED_DT), then the RK stages, each = ghost fill + fused RHS/hyperdiffusion/
+ * RK-combine/wavespeed-reduction kernel.  dt and the maxima stay on the device; the host synchronises
+ * once, at the end, to read the status.  Returns SMAUG_ENONFINITE if any dt was non-finite or <= 0. */
+int smaug_step(smaug_ctx* ctx, int n_steps, double cfl);
+
+/* Same, but only enqueues the work; the status is picked up by the next synchronising call. */
+int smaug_step_async(smaug_ctx* ctx, int n_steps, double cfl);
+
+/* Copy the perturbed state out, [6][ny][nx] (host or device). */
+int smaug_get_state(smaug_ctx* ctx, double* w);
+
+/* Simulated time and the last dt used (either pointer may be NULL). */
+int smaug_get_time(smaug_ctx* ctx, double* t, double* last_dt);
+
+/* out = { max(|vx|+c_fx), max(|vy|+c_fy), max a^2, max b^2 } of the current state (c-4). */
+int smaug_get_wavespeeds(smaug_ctx* ctx, double out[4]);
+
+/* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
+int smaug_get_launch_count(smaug_ctx* ctx, long long* n);
+
+/* Algorithmic / launch facts of the fused stage kernel, for the roofline report:
+ * out = { tile_w, tile_h, threads, dynamic_smem_bytes, ctas_last_launch }. */
+int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
+
+/* Device time, in milliseconds, spent in the fused stage kernels (summed over launches) and the number of
+ * those launches, measured with CUDA events on the context's stream when enabled with
+ * smaug_set_kernel_timing(ctx, 1).  Reading synchronises the stream.  */
+int smaug_set_kernel_timing(smaug_ctx* ctx, int on);
+int smaug_get_kernel_timing(smaug_ctx* ctx, double* stage_ms, long long* stage_launches);
+
+void smaug_destroy(smaug_ctx* ctx); /* NULL is a no-op */
+
+const char* smaug_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SMAUG_H_ */

@@ -1,0 +1,191 @@
+"""paper_1710_06423_b200 -- B200-native SMAUG+ hot path (one full 2-D MHD time step), Python binding.
+
+Thin ctypes layer over ``libsmaug.so`` (C ABI in include/smaug.h, CUDA sources in csrc/).  Argument
+marshalling only: every step of the path runs in the library's kernels.  PyTorch supplies device memory
+(the workspace tensor, state tensors) and the stream; nothing here computes.  There is no CPU fallback:
+``lib()`` raises if the extension is missing, and every call fails loudly without a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "csrc")
+LIB_PATH = os.path.join(_HERE, "libsmaug.so")
+INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
+
+BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2
+OK, EINVAL, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
+PARAMS = dict(lx=0, ly=1, hd_on=2, c_rho=3, c_mom=4, c_e=5, c_b=6, rk_order=7, fixed_dt=8)
+
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+_lib = None
+
+
+def _sources():
+    return sorted(os.path.join(_CSRC, f) for f in os.listdir(_CSRC))
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/smaug.cu for sm_100a into libsmaug.so (in-tree) if missing or stale."""
+    newest = max(os.path.getmtime(p) for p in _sources() + [os.path.join(INCLUDE, "smaug.h")])
+    if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+              ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu")]
+        subprocess.run(cmd, check=True)
+    return LIB_PATH
+
+
+def lib() -> C.CDLL:
+    """Load libsmaug.so (never builds implicitly on a box without nvcc: fails loudly instead)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            try:
+                build()
+            except Exception as e:  # noqa: BLE001
+                raise RuntimeError(f"libsmaug.so is missing and could not be built ({e}); "
+                                   "there is no CPU fallback") from e
+        L = C.CDLL(LIB_PATH)
+        dp, vp = C.POINTER(C.c_double), C.c_void_p
+        L.smaug_last_error.restype = C.c_char_p
+        L.smaug_workspace_bytes.restype = C.c_size_t
+        L.smaug_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.smaug_create.argtypes = [C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), vp, C.POINTER(vp)]
+        L.smaug_create_in_workspace.argtypes = [C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), vp, vp,
+                                                C.c_size_t, vp, C.POINTER(vp)]
+        L.smaug_set_stream.argtypes = [vp, vp]
+        L.smaug_set_param.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug_set_state.argtypes = [vp, vp]
+        L.smaug_step.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug_step_async.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug_get_state.argtypes = [vp, vp]
+        L.smaug_get_time.argtypes = [vp, dp, dp]
+        L.smaug_get_wavespeeds.argtypes = [vp, dp]
+        L.smaug_get_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.smaug_get_kernel_info.argtypes = [vp, C.POINTER(C.c_int)]
+        L.smaug_set_kernel_timing.argtypes = [vp, C.c_int]
+        L.smaug_get_kernel_timing.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+        L.smaug_destroy.argtypes = [vp]
+        L.smaug_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+class SmaugError(RuntimeError):
+    def __init__(self, code: int):
+        self.code = code
+        super().__init__(f"smaug error {code}: {lib().smaug_last_error().decode()}")
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise SmaugError(rc)
+
+
+def _ptr(x):
+    """Raw address of a torch tensor or numpy array (must be contiguous float64), or None."""
+    if x is None:
+        return None
+    if hasattr(x, "data_ptr"):
+        assert x.is_contiguous() and str(x.dtype) == "torch.float64"
+        return C.c_void_p(x.data_ptr())
+    assert x.flags["C_CONTIGUOUS"] and x.dtype.name == "float64"
+    return C.c_void_p(x.ctypes.data)
+
+
+class Smaug:
+    """One simulation context: smaug_create / set_state / step / get_state / destroy (include/smaug.h).
+
+    State and background are float64, ``[6, ny, nx]`` / ``[4, ny, nx]``, torch (cuda or cpu) tensors or
+    numpy arrays.  Device memory is a torch uint8 workspace tensor; work is enqueued on torch's current
+    stream of ``device`` at construction time.
+    """
+
+    def __init__(self, nx, ny, gamma, bc, bg=None, device="cuda:0", **params):
+        import torch
+        L = lib()
+        self.nx, self.ny = int(nx), int(ny)
+        self.device = torch.device(device)
+        nbytes = L.smaug_workspace_bytes(self.nx, self.ny, int(bg is not None))
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+            h = C.c_void_p()
+            bc_arr = (C.c_int * 4)(*[int(b) for b in bc])
+            if bg is not None:
+                assert tuple(bg.shape) == (4, ny, nx)
+            _check(L.smaug_create_in_workspace(self.nx, self.ny, float(gamma), bc_arr, _ptr(bg),
+                                               C.c_void_p(base), nbytes, C.c_void_p(stream), C.byref(h)))
+        self._h = h
+        for k, v in params.items():
+            self.set_param(k, v)
+
+    def set_param(self, key, value):
+        k = PARAMS[key] if isinstance(key, str) else int(key)
+        _check(lib().smaug_set_param(self._h, k, float(value)))
+
+    def set_state(self, w):
+        assert tuple(w.shape) == (6, self.ny, self.nx)
+        _check(lib().smaug_set_state(self._h, _ptr(w)))
+
+    def step(self, n_steps, cfl=0.3):
+        _check(lib().smaug_step(self._h, int(n_steps), float(cfl)))
+
+    def step_async(self, n_steps, cfl=0.3):
+        _check(lib().smaug_step_async(self._h, int(n_steps), float(cfl)))
+
+    def get_state(self, out=None):
+        """Copy the state into `out` (torch tensor on any device / numpy array); default: new cuda tensor."""
+        import torch
+        if out is None:
+            out = torch.empty((6, self.ny, self.nx), dtype=torch.float64, device=self.device)
+        assert tuple(out.shape) == (6, self.ny, self.nx)
+        _check(lib().smaug_get_state(self._h, _ptr(out)))
+        return out
+
+    def time(self):
+        t, dt = C.c_double(), C.c_double()
+        _check(lib().smaug_get_time(self._h, C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def wavespeeds(self):
+        o = (C.c_double * 4)()
+        _check(lib().smaug_get_wavespeeds(self._h, o))
+        return list(o)
+
+    def launch_count(self):
+        n = C.c_longlong()
+        _check(lib().smaug_get_launch_count(self._h, C.byref(n)))
+        return n.value
+
+    def kernel_info(self):
+        o = (C.c_int * 5)()
+        _check(lib().smaug_get_kernel_info(self._h, o))
+        return dict(tile_w=o[0], tile_h=o[1], threads=o[2], smem_bytes=o[3], ctas=o[4])
+
+    def set_kernel_timing(self, on=True):
+        _check(lib().smaug_set_kernel_timing(self._h, int(on)))
+
+    def kernel_timing(self):
+        ms, n = C.c_double(), C.c_longlong()
+        _check(lib().smaug_get_kernel_timing(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().smaug_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # noqa: BLE001
+            pass

@@ -1,0 +1,472 @@
+// smaug.cu -- host side of libsmaug.so: the C ABI of include/smaug.h, device memory layout, and the
+// launch sequence of one time step.  No torch types, no CPU fallback: every numerical step is a kernel
+// from smaug_aux_kernels.cuh / smaug_stage_kernel.cuh.
+#include "../../include/smaug.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "smaug_stage_kernel.cuh"
+
+using namespace smaug;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(SMAUG_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));                \
+  } while (0)
+
+// Tile / launch configuration of the fused stage kernel.
+constexpr int TW = 32, TH = 16, NT = 256;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  int pitch;
+  long long plane;          // doubles
+  size_t state_bytes;       // one buffer of 6 planes
+  size_t bg_bytes;
+  size_t scalars_off, bufs_off[4], bg_off, total;
+};
+
+Layout make_layout(int nx, int ny, bool has_bg) {
+  Layout L;
+  L.pitch = (int)align_up((size_t)XOFF + nx + NG, 16);
+  L.plane = (long long)L.pitch * (ny + 2 * NG);
+  const size_t plane_bytes = align_up((size_t)L.plane * sizeof(double), 256);
+  L.state_bytes = NF * plane_bytes;
+  L.bg_bytes = has_bg ? NBG * plane_bytes : 0;
+  size_t off = 0;
+  L.scalars_off = off; off += align_up(sizeof(DeviceScalars), 256);
+  for (int b = 0; b < 4; ++b) { L.bufs_off[b] = off; off += L.state_bytes; }
+  L.bg_off = off; off += L.bg_bytes;
+  L.total = off;
+  return L;
+}
+
+}  // namespace
+
+struct smaug_ctx {
+  Grid g;
+  double gamma = 0;
+  double Lx = 1, Ly = 1;
+  int hd_on = 1;
+  double c_rho = 0.02, c_mom = 0.4, c_e = 0.02, c_b = 0.02;
+  int rk_order = 4;
+  double fixed_dt = 0;
+  bool has_bg = false;
+  Layout L;
+  char* base = nullptr;     // device workspace
+  bool owns = false;
+  cudaStream_t stream = nullptr;
+  DeviceScalars* sc = nullptr;
+  Planes6 buf[4];           // buf[0] holds the state between steps; 1, 2: stage buffers; 3: accumulator
+  CPlanes4 bg;
+  int state_set = 0;        // reduction set holding the maxima of the state (0 or 4)
+  long long launches = 0;
+  int last_ctas = 0;
+  // stage-kernel timing (CUDA events on the stream)
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;   // pairs
+  size_t ev_used = 0;
+  double stage_ms = 0;
+  long long stage_launches = 0;
+  bool pending_status = false;
+};
+
+namespace {
+
+CPlanes6 cview(const Planes6& p) {
+  CPlanes6 c;
+  for (int f = 0; f < NF; ++f) c.p[f] = p.p[f];
+  return c;
+}
+
+Params make_params(const smaug_ctx* c) {
+  Params p;
+  p.gamma = c->gamma;
+  p.inv_dx = c->g.nx / c->Lx;
+  p.inv_dy = c->g.ny / c->Ly;
+  p.c_rho = c->c_rho; p.c_mom = c->c_mom; p.c_e = c->c_e; p.c_b = c->c_b;
+  p.hd_on = c->hd_on;
+  return p;
+}
+
+int launch_ghost(smaug_ctx* c, const Planes6& pl, int nplanes, int freeze) {
+  const long long total = 2LL * NG * (c->g.nx + 2 * NG) + 2LL * NG * c->g.ny;
+  const int blocks = (int)std::min<long long>((total + 255) / 256, 1024);
+  ghost_fill_kernel<<<dim3(blocks, nplanes), 256, 0, c->stream>>>(c->g, pl, freeze);
+  c->launches++;
+  CU(cudaGetLastError());
+  return SMAUG_OK;
+}
+
+int launch_wavespeeds(smaug_ctx* c, const Planes6& w, int set) {
+  const long long n = (long long)c->g.nx * c->g.ny;
+  const int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 8);
+  unsigned long long* slots = c->sc->red[set];
+  if (c->has_bg)
+    wavespeed_kernel<true><<<blocks, 256, 0, c->stream>>>(c->g, cview(w), c->bg, c->gamma, slots);
+  else
+    wavespeed_kernel<false><<<blocks, 256, 0, c->stream>>>(c->g, cview(w), c->bg, c->gamma, slots);
+  c->launches++;
+  CU(cudaGetLastError());
+  return SMAUG_OK;
+}
+
+template <bool BG, bool HD>
+int launch_stage_t(smaug_ctx* c, const StageArgs& a) {
+  static bool configured = false;
+  constexpr size_t smem = stage_smem_bytes<TW, TH, BG>();
+  auto kern = stage_kernel<TW, TH, NT, BG, HD>;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  dim3 grid((c->g.nx + TW - 1) / TW, (c->g.ny + TH - 1) / TH);
+  c->last_ctas = (int)(grid.x * grid.y);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing && c->ev_used + 2 <= c->ev.size()) {
+    e0 = c->ev[c->ev_used++];
+    e1 = c->ev[c->ev_used++];
+    CU(cudaEventRecord(e0, c->stream));
+  }
+  kern<<<grid, NT, smem, c->stream>>>(a);
+  if (e1) CU(cudaEventRecord(e1, c->stream));
+  c->launches++;
+  CU(cudaGetLastError());
+  return SMAUG_OK;
+}
+
+int launch_stage(smaug_ctx* c, const StageArgs& a) {
+  if (c->has_bg) return c->hd_on ? launch_stage_t<true, true>(c, a) : launch_stage_t<true, false>(c, a);
+  return c->hd_on ? launch_stage_t<false, true>(c, a) : launch_stage_t<false, false>(c, a);
+}
+
+// One stage: ghost fill of the input buffer, then the fused kernel.
+int run_stage(smaug_ctx* c, int in, int base, int acc_in, int out, int acc_out, double coef, int combine,
+              int red_in, int red_out, int ws_mode) {
+  int rc = launch_ghost(c, c->buf[in], NF, 0);
+  if (rc) return rc;
+  StageArgs a;
+  a.g = c->g;
+  a.prm = make_params(c);
+  a.in = cview(c->buf[in]);
+  a.base = cview(c->buf[base]);
+  a.acc_in = cview(c->buf[acc_in]);
+  a.out = c->buf[out];
+  a.acc_out = c->buf[acc_out];
+  a.bg = c->bg;
+  a.sc = c->sc;
+  a.red_in = red_in;
+  a.red_out = red_out;
+  a.c = coef;
+  a.combine = combine;
+  a.ws_mode = ws_mode;
+  return launch_stage(c, a);
+}
+
+// One full time step (c-6, c-7).  The state lives in buf[0] before and after.
+int enqueue_step(smaug_ctx* c, double cfl) {
+  const int A = c->state_set, B = A == 0 ? 4 : 0;
+  const int vt_mode = c->hd_on ? WS_VT : WS_NONE;
+  dt_kernel<<<1, 32, 0, c->stream>>>(c->sc, A, (1u << 1) | (1u << 2) | (1u << 3) | (1u << B), cfl,
+                                     c->fixed_dt, c->Lx / c->g.nx, c->Ly / c->g.ny, c->g.nx, c->g.ny);
+  c->launches++;
+  CU(cudaGetLastError());
+  int rc = SMAUG_OK;
+  if (c->rk_order == 4) {
+    //            in base acc_in out acc_out  c     combine        red_in red_out ws
+    rc = run_stage(c, 0, 0, 3, 1, 3, 0.5, COMBINE_BASE, A, 1, vt_mode);            // w1 = wn + dt/2 R(wn)
+    if (!rc) rc = run_stage(c, 1, 0, 3, 2, 3, 0.5, COMBINE_ACC, 1, 2, vt_mode);    // w2; acc = (w1+2w2-wn)/3
+    if (!rc) rc = run_stage(c, 2, 0, 3, 1, 3, 1.0, COMBINE_BASE, 2, 3, vt_mode);   // w3 = wn + dt R(w2)
+    if (!rc) rc = run_stage(c, 1, 0, 3, 0, 3, 1.0 / 6.0, COMBINE_FINAL, 3, B, WS_FULL);  // w^{n+1}
+  } else if (c->rk_order == 2) {
+    rc = run_stage(c, 0, 0, 3, 1, 3, 0.5, COMBINE_BASE, A, 1, vt_mode);
+    // in-place on buf[0] is safe: base is read and out written by the same thread at the same cell only
+    if (!rc) rc = run_stage(c, 1, 0, 3, 0, 3, 1.0, COMBINE_BASE, 1, B, WS_FULL);
+  } else {
+    rc = run_stage(c, 0, 0, 3, 1, 3, 1.0, COMBINE_BASE, A, B, WS_FULL);
+    if (!rc) std::swap(c->buf[0], c->buf[1]);
+  }
+  c->state_set = B;
+  return rc;
+}
+
+int check_ctx(smaug_ctx* c) {
+  if (!c) return fail(SMAUG_EINVAL, "NULL context");
+  return SMAUG_OK;
+}
+
+// copy interior [6][ny][nx] (host or device) <-> padded planes
+int copy_in(smaug_ctx* c, const double* src, double* const* planes, int nplanes) {
+  const Grid& g = c->g;
+  for (int f = 0; f < nplanes; ++f)
+    CU(cudaMemcpy2DAsync(planes[f] + cell_addr(g, 0, 0), (size_t)g.pitch * sizeof(double),
+                         src + (size_t)f * g.nx * g.ny, (size_t)g.nx * sizeof(double),
+                         (size_t)g.nx * sizeof(double), g.ny, cudaMemcpyDefault, c->stream));
+  return SMAUG_OK;
+}
+
+int collect_timing(smaug_ctx* c) {
+  for (size_t k = 0; k + 1 < c->ev_used; k += 2) {
+    float ms = 0;
+    CU(cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]));
+    c->stage_ms += ms;
+    c->stage_launches++;
+  }
+  c->ev_used = 0;
+  return SMAUG_OK;
+}
+
+int sync_and_status(smaug_ctx* c) {
+  CU(cudaStreamSynchronize(c->stream));
+  if (c->timing) {
+    int rc = collect_timing(c);
+    if (rc) return rc;
+  }
+  if (c->pending_status) {
+    int status = 0;
+    CU(cudaMemcpy(&status, &c->sc->status, sizeof(int), cudaMemcpyDeviceToHost));
+    c->pending_status = false;
+    if (status) return fail(SMAUG_ENONFINITE, "a time step was non-finite or <= 0");
+  }
+  return SMAUG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* smaug_last_error(void) { return g_err.c_str(); }
+
+size_t smaug_workspace_bytes(int nx, int ny, int has_bg) {
+  if (nx < 1 || ny < 1) return 0;
+  return make_layout(nx, ny, has_bg != 0).total;
+}
+
+int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], const double* bg,
+                              void* workspace, size_t workspace_bytes, void* stream, smaug_ctx** out) {
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!bc) return fail(SMAUG_EINVAL, "bc is NULL");
+  if (nx < 1 || ny < 1) return fail(SMAUG_EINVAL, "nx and ny must be >= 1");
+  if (!(gamma > 1.0)) return fail(SMAUG_EINVAL, "gamma must be > 1");
+  for (int s = 0; s < 4; ++s)
+    if (bc[s] < 0 || bc[s] > 2) return fail(SMAUG_EINVAL, "unknown boundary kind");
+  for (int ax = 0; ax < 2; ++ax)
+    if ((bc[2 * ax] == SMAUG_BC_PERIODIC) != (bc[2 * ax + 1] == SMAUG_BC_PERIODIC))
+      return fail(SMAUG_EINVAL, "periodic must be set on both sides of an axis");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(SMAUG_ECUDA, "no CUDA device: libsmaug has no CPU fallback");
+  }
+  smaug_ctx* c = new (std::nothrow) smaug_ctx();
+  if (!c) return fail(SMAUG_ENOMEM, "host allocation failed");
+  c->has_bg = bg != nullptr;
+  c->L = make_layout(nx, ny, c->has_bg);
+  c->g.nx = nx; c->g.ny = ny; c->g.pitch = c->L.pitch; c->g.plane = c->L.plane;
+  for (int s = 0; s < 4; ++s) c->g.bc[s] = bc[s];
+  c->gamma = gamma;
+  c->stream = (cudaStream_t)stream;
+  if (workspace) {
+    if (workspace_bytes < c->L.total || ((uintptr_t)workspace & 255)) {
+      delete c;
+      return fail(SMAUG_ENOMEM, "workspace too small or not 256-byte aligned");
+    }
+    c->base = (char*)workspace;
+  } else {
+    if (cudaMalloc((void**)&c->base, c->L.total) != cudaSuccess) {
+      cudaGetLastError();
+      delete c;
+      return fail(SMAUG_ENOMEM, "cudaMalloc of the workspace failed");
+    }
+    c->owns = true;
+  }
+  auto cleanup = [&](int rc) { smaug_destroy(c); return rc; };
+  if (cudaMemsetAsync(c->base, 0, c->L.total, c->stream) != cudaSuccess)
+    return cleanup(fail(SMAUG_ECUDA, "cudaMemsetAsync failed"));
+  c->sc = (DeviceScalars*)(c->base + c->L.scalars_off);
+  const size_t plane_bytes = c->L.state_bytes / NF;
+  for (int b = 0; b < 4; ++b)
+    for (int f = 0; f < NF; ++f) c->buf[b].p[f] = (double*)(c->base + c->L.bufs_off[b] + f * plane_bytes);
+  for (int k = 0; k < NBG; ++k)
+    c->bg.p[k] = c->has_bg ? (const double*)(c->base + c->L.bg_off + k * plane_bytes) : nullptr;
+  if (c->has_bg) {
+    Planes6 bgp;
+    for (int k = 0; k < NF; ++k) bgp.p[k] = k < NBG ? (double*)c->bg.p[k] : nullptr;
+    int rc = copy_in(c, bg, bgp.p, NBG);
+    if (!rc) rc = launch_ghost(c, bgp, NBG, 1);   // c-8: periodic -> wrap, else nearest interior, once
+    if (rc) return cleanup(rc);
+  }
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess)
+    return cleanup(fail(SMAUG_ECUDA, "stream synchronise failed in create"));
+  *out = c;
+  return SMAUG_OK;
+}
+
+int smaug_create(int nx, int ny, double gamma, const int bc[4], const double* bg, smaug_ctx** out) {
+  return smaug_create_in_workspace(nx, ny, gamma, bc, bg, nullptr, 0, nullptr, out);
+}
+
+void smaug_destroy(smaug_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->owns && c->base) cudaFree(c->base);
+  cudaGetLastError();
+  delete c;
+}
+
+int smaug_set_stream(smaug_ctx* c, void* stream) {
+  if (int rc = check_ctx(c)) return rc;
+  CU(cudaStreamSynchronize(c->stream));
+  c->stream = (cudaStream_t)stream;
+  return SMAUG_OK;
+}
+
+int smaug_set_param(smaug_ctx* c, int key, double v) {
+  if (int rc = check_ctx(c)) return rc;
+  switch (key) {
+    case SMAUG_PARAM_LX: if (!(v > 0)) break; c->Lx = v; return SMAUG_OK;
+    case SMAUG_PARAM_LY: if (!(v > 0)) break; c->Ly = v; return SMAUG_OK;
+    case SMAUG_PARAM_HD_ON: c->hd_on = v != 0.0; return SMAUG_OK;
+    case SMAUG_PARAM_C_RHO: if (!(v >= 0)) break; c->c_rho = v; return SMAUG_OK;
+    case SMAUG_PARAM_C_MOM: if (!(v >= 0)) break; c->c_mom = v; return SMAUG_OK;
+    case SMAUG_PARAM_C_E: if (!(v >= 0)) break; c->c_e = v; return SMAUG_OK;
+    case SMAUG_PARAM_C_B: if (!(v >= 0)) break; c->c_b = v; return SMAUG_OK;
+    case SMAUG_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c->rk_order = (int)v; return SMAUG_OK;
+    case SMAUG_PARAM_FIXED_DT: if (!(v >= 0)) break; c->fixed_dt = v; return SMAUG_OK;
+    default: return fail(SMAUG_EINVAL, "unknown parameter key");
+  }
+  return fail(SMAUG_EINVAL, "parameter value out of range");
+}
+
+int smaug_set_state(smaug_ctx* c, const double* w) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!w) return fail(SMAUG_EINVAL, "w is NULL");
+  int rc = copy_in(c, w, c->buf[0].p, NF);
+  if (rc) return rc;
+  // ghosts: fixed sides are frozen here, in every buffer that is ever read with its halo (0, 1, 2)
+  if ((rc = launch_ghost(c, c->buf[0], NF, 1))) return rc;
+  for (int b = 1; b <= 2; ++b)
+    for (int f = 0; f < NF; ++f)
+      CU(cudaMemcpyAsync(c->buf[b].p[f], c->buf[0].p[f], (size_t)c->g.plane * sizeof(double),
+                         cudaMemcpyDeviceToDevice, c->stream));
+  CU(cudaMemsetAsync(c->sc, 0, sizeof(DeviceScalars), c->stream));
+  c->state_set = 0;
+  if ((rc = launch_wavespeeds(c, c->buf[0], 0))) return rc;
+  c->pending_status = false;
+  CU(cudaStreamSynchronize(c->stream));
+  return SMAUG_OK;
+}
+
+int smaug_step_async(smaug_ctx* c, int n_steps, double cfl) {
+  if (int rc = check_ctx(c)) return rc;
+  if (n_steps < 0) return fail(SMAUG_EINVAL, "n_steps must be >= 0");
+  if (!(c->fixed_dt > 0.0) && !(cfl > 0.0)) return fail(SMAUG_EINVAL, "cfl must be > 0");
+  for (int s = 0; s < n_steps; ++s) {
+    int rc = enqueue_step(c, cfl);
+    if (rc) return rc;
+    // keep the event pool bounded: drain it when full (only when timing is on)
+    if (c->timing && c->ev_used + 8 > c->ev.size()) {
+      CU(cudaStreamSynchronize(c->stream));
+      if ((rc = collect_timing(c))) return rc;
+    }
+  }
+  if (n_steps > 0) c->pending_status = true;
+  return SMAUG_OK;
+}
+
+int smaug_step(smaug_ctx* c, int n_steps, double cfl) {
+  int rc = smaug_step_async(c, n_steps, cfl);
+  if (rc) return rc;
+  return sync_and_status(c);
+}
+
+int smaug_get_state(smaug_ctx* c, double* w) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!w) return fail(SMAUG_EINVAL, "w is NULL");
+  const Grid& g = c->g;
+  for (int f = 0; f < NF; ++f)
+    CU(cudaMemcpy2DAsync(w + (size_t)f * g.nx * g.ny, (size_t)g.nx * sizeof(double),
+                         c->buf[0].p[f] + cell_addr(g, 0, 0), (size_t)g.pitch * sizeof(double),
+                         (size_t)g.nx * sizeof(double), g.ny, cudaMemcpyDefault, c->stream));
+  return sync_and_status(c);
+}
+
+int smaug_get_time(smaug_ctx* c, double* t, double* last_dt) {
+  if (int rc = check_ctx(c)) return rc;
+  int rc = sync_and_status(c);
+  double v[2];
+  CU(cudaMemcpy(v, &c->sc->dt, 2 * sizeof(double), cudaMemcpyDeviceToHost));
+  if (last_dt) *last_dt = v[0];
+  if (t) *t = v[1];
+  return rc;
+}
+
+int smaug_get_wavespeeds(smaug_ctx* c, double out[4]) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  int rc = sync_and_status(c);
+  CU(cudaMemcpy(out, c->sc->red[c->state_set], 4 * sizeof(double), cudaMemcpyDeviceToHost));
+  return rc;
+}
+
+int smaug_get_launch_count(smaug_ctx* c, long long* n) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!n) return fail(SMAUG_EINVAL, "n is NULL");
+  *n = c->launches;
+  return SMAUG_OK;
+}
+
+int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
+  if (int rc = check_ctx(c)) return rc;
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  out[0] = TW; out[1] = TH; out[2] = NT;
+  out[3] = (int)(c->has_bg ? stage_smem_bytes<TW, TH, true>() : stage_smem_bytes<TW, TH, false>());
+  out[4] = c->last_ctas;
+  return SMAUG_OK;
+}
+
+int smaug_set_kernel_timing(smaug_ctx* c, int on) {
+  if (int rc = check_ctx(c)) return rc;
+  CU(cudaStreamSynchronize(c->stream));
+  c->timing = on != 0;
+  c->ev_used = 0;
+  c->stage_ms = 0;
+  c->stage_launches = 0;
+  if (c->timing && c->ev.empty()) {
+    c->ev.resize(2048);
+    for (auto& e : c->ev) CU(cudaEventCreate(&e));
+  }
+  return SMAUG_OK;
+}
+
+int smaug_get_kernel_timing(smaug_ctx* c, double* stage_ms, long long* stage_launches) {
+  if (int rc = check_ctx(c)) return rc;
+  CU(cudaStreamSynchronize(c->stream));
+  if (int rc = collect_timing(c)) return rc;
+  if (stage_ms) *stage_ms = c->stage_ms;
+  if (stage_launches) *stage_launches = c->stage_launches;
+  return SMAUG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,176 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle, element by
+element on the same seeded/analytic inputs.  Bar (north_star, SURVEY c-9): relative L2 <= 1e-10 per field.
+Where the oracle field is identically zero the error is measured against the largest field norm."""
+import numpy as np
+import pytest
+
+import smaug_inputs as si
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests need a B200")
+    import paper_1710_06423_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def gpu_run(pkg, w, bc, gamma, steps, cfl=0.3, bg=None, host=True, chunks=1, **params):
+    import torch
+    ny, nx = w.shape[1:]
+    wt = torch.from_numpy(w) if host else torch.from_numpy(w).cuda()
+    bgt = None if bg is None else (torch.from_numpy(np.ascontiguousarray(bg)) if host
+                                   else torch.from_numpy(np.ascontiguousarray(bg)).cuda())
+    s = pkg.Smaug(nx, ny, gamma, bc, bg=bgt, **params)
+    s.set_state(wt)
+    for _ in range(chunks):
+        s.step(steps // chunks, cfl)
+    out = torch.empty((6, ny, nx), dtype=torch.float64) if host else None
+    out = s.get_state(out)
+    t = s.time()
+    ws = s.wavespeeds()
+    s.close()
+    return out.cpu().numpy(), t, ws
+
+
+def cpu_run(oracle_mod, w, bc, gamma, steps, cfl=0.3, bg=None, threads=8, **params):
+    ny, nx = w.shape[1:]
+    o = oracle_mod.Oracle(nx, ny, gamma, bc, bg=bg, threads=threads, **params)
+    o.set_state(w)
+    o.step(steps, cfl)
+    out, t, ws = o.get_state(), o.time(), o.wavespeeds()
+    o.close()
+    return out, t, ws
+
+
+def check(a, ta, wsa, b, tb, wsb, tol=TOL):
+    err = si.rel_l2(a, b)
+    assert np.isfinite(a).all()
+    assert (err <= tol).all(), err
+    assert abs(ta[0] - tb[0]) <= 1e-12 * abs(tb[0]) and abs(ta[1] - tb[1]) <= 1e-12 * abs(tb[1])
+    assert np.allclose(wsa, wsb, rtol=1e-11, atol=0)
+    return err
+
+
+# sizes span several 32x16 tiles plus ragged tails in both directions
+@pytest.mark.parametrize("nx,ny,steps", [(70, 45, 20), (32, 16, 10), (33, 17, 10), (200, 200, 40)])
+def test_orszag_tang_parity(gpu, oracle_mod, nx, ny, steps):
+    w, bc, gamma = si.orszag_tang(nx, ny)
+    a = gpu_run(gpu, w, bc, gamma, steps)
+    b = cpu_run(oracle_mod, w, bc, gamma, steps)
+    check(*a, *b)
+
+
+def test_orszag_tang_parity_device_pointers(gpu, oracle_mod):
+    w, bc, gamma = si.orszag_tang(96, 64)
+    a = gpu_run(gpu, w, bc, gamma, 12, host=False)
+    b = cpu_run(oracle_mod, w, bc, gamma, 12)
+    check(*a, *b)
+
+
+def test_brio_wu_config_parity(gpu, oracle_mod):
+    """BASELINE.json config 1 in full: 800 x 1, open in x, gamma = 2, CFL 0.3, 1000 steps."""
+    w, bc, gamma = si.brio_wu(800, 1)
+    a = gpu_run(gpu, w, bc, gamma, 1000)
+    b = cpu_run(oracle_mod, w, bc, gamma, 1000, threads=1)
+    check(*a, *b)
+    assert np.array_equal(a[0][4], np.full_like(a[0][4], 0.75))       # Bx stays 0.75 exactly (P13)
+
+
+def test_brio_wu_2d_and_transposed(gpu, oracle_mod):
+    w, bc, gamma = si.brio_wu(160, 24)
+    a = gpu_run(gpu, w, bc, gamma, 100)
+    b = cpu_run(oracle_mod, w, bc, gamma, 100)
+    check(*a, *b)
+    wt, bct, _ = si.brio_wu(160, 24, transpose=True)
+    at = gpu_run(gpu, wt, bct, gamma, 100)
+    bt = cpu_run(oracle_mod, wt, bct, gamma, 100)
+    check(*at, *bt)
+    assert np.abs(si.transpose_state(at[0]) - a[0]).max() < 1e-11     # P5 on the GPU
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0), (1, 1, 1, 1), (2, 2, 0, 0), (1, 1, 2, 2), (0, 0, 1, 2)])
+def test_boundary_kinds_with_background(gpu, oracle_mod, bc):
+    nx, ny = 50, 37
+    w, _, gamma = si.smooth_random(nx, ny, seed=3, amp=5e-2)
+    w[1] += 0.3 * w[0]
+    x = si.centres(nx)[None, :] * np.ones((ny, 1))
+    y = si.centres(ny)[:, None] * np.ones((1, nx))
+    bg = np.stack([0.5 + 0.1 * np.cos(2 * np.pi * x), 0.8 + 0.05 * np.sin(2 * np.pi * y),
+                   0.2 + 0.05 * np.sin(2 * np.pi * y), 0.1 + 0.05 * np.cos(2 * np.pi * x)])
+    a = gpu_run(gpu, w, bc, gamma, 15, bg=bg)
+    b = cpu_run(oracle_mod, w, bc, gamma, 15, bg=bg)
+    check(*a, *b)
+
+
+@pytest.mark.parametrize("params", [dict(hd_on=0), dict(rk_order=2), dict(rk_order=1, hd_on=1),
+                                    dict(fixed_dt=1e-4), dict(c_rho=0.1, c_mom=0.2, c_e=0.05, c_b=0.3),
+                                    dict(lx=2.0, ly=0.5)])
+def test_parameters(gpu, oracle_mod, params):
+    w, bc, gamma = si.orszag_tang(64, 48)
+    a = gpu_run(gpu, w, bc, gamma, 10, **params)
+    b = cpu_run(oracle_mod, w, bc, gamma, 10, **params)
+    check(*a, *b)
+
+
+def test_uniform_state_preserved_bitwise_on_gpu(gpu):
+    nx, ny, gamma = 40, 20, 5.0 / 3.0
+    w = si.prim_to_cons(0.3, 0.7, -0.4, 0.2, 0.5, -0.25, gamma)[:, None, None] * np.ones((1, ny, nx))
+    for bg in (None, si.uniform_background(nx, ny, 1.3, 2.1, 0.4, 0.3)):
+        out, _, _ = gpu_run(gpu, np.ascontiguousarray(w), (1, 1, 0, 0), gamma, 5, bg=bg)
+        assert np.array_equal(out, w)
+
+
+def test_restart_is_bitwise_on_gpu(gpu):
+    w, bc, gamma = si.orszag_tang(80, 40)
+    a, _, _ = gpu_run(gpu, w, bc, gamma, 10)
+    half, _, _ = gpu_run(gpu, w, bc, gamma, 5)
+    b, _, _ = gpu_run(gpu, half, bc, gamma, 5)
+    assert np.array_equal(a, b)
+    c, _, _ = gpu_run(gpu, w, bc, gamma, 10, chunks=2)      # two smaug_step calls == one
+    assert np.array_equal(a, c)
+
+
+def test_edge_cases(gpu, oracle_mod):
+    # degenerate grids: a single cell, a single column, n < ghost width
+    for nx, ny in [(1, 1), (1, 9), (2, 2), (5, 1)]:
+        w, bc, gamma = si.smooth_random(nx, ny, seed=4, amp=1e-2)
+        a = gpu_run(gpu, w, bc, gamma, 3, fixed_dt=1e-3)
+        b = cpu_run(oracle_mod, w, bc, gamma, 3, fixed_dt=1e-3, threads=1)
+        assert (si.rel_l2(a[0], b[0]) <= TOL).all()
+    # zero steps, and the non-finite status (rho = 0)
+    w, bc, gamma = si.orszag_tang(16, 16)
+    a = gpu_run(gpu, w, bc, gamma, 0)
+    assert np.array_equal(a[0], w)
+    s = gpu.Smaug(8, 8, 1.4, bc)
+    import torch
+    s.set_state(torch.zeros((6, 8, 8), dtype=torch.float64))
+    with pytest.raises(gpu.SmaugError) as ei:
+        s.step(1, 0.3)
+    assert ei.value.code == gpu.ENONFINITE
+    s.close()
+
+
+def test_full_size_config2_sampled_steps(gpu, oracle_mod):
+    """Orszag-Tang 1000 x 1000 (BASELINE.json config 2, the bench workload): 3 full steps against the
+    oracle on every cell, then properties that hold at any size for the full 200 steps (below)."""
+    w, bc, gamma = si.orszag_tang(1000)
+    a = gpu_run(gpu, w, bc, gamma, 3)
+    b = cpu_run(oracle_mod, w, bc, gamma, 3)
+    check(*a, *b)
+
+
+def test_full_config2_properties_after_200_steps(gpu):
+    """P2 (conservation) and P3 (180-degree point symmetry) on the GPU result of the full config 2 run."""
+    w, bc, gamma = si.orszag_tang(1000, symmetrise=True)
+    out, (t, dt), _ = gpu_run(gpu, w, bc, gamma, 200)
+    assert np.isfinite(out).all() and 0.02 < t < 0.03
+    sign = np.array([1, -1, -1, 1, -1, -1.0])[:, None, None]
+    assert np.abs(out - sign * out[:, ::-1, ::-1]).max() <= 1e-11 * np.abs(out).max()
+    drift = np.abs(out.reshape(6, -1).sum(1) - w.reshape(6, -1).sum(1)) / np.abs(w).reshape(6, -1).sum(1)
+    assert (drift < 1e-12).all(), drift
