@@ -11,7 +11,7 @@
 //   fill_ghosts            P5 (ny=1 == ny=8), P3 (periodic wrap keeps the OT point symmetry), brute force
 //   central differences    P4 (numerical phase speed k*), P6 (4th-order convergence), exact on cubics
 //   fluxes / split form    P1, P2 (conservation), P4 (sound/Alfven/fast/slow phase speeds), split==unsplit
-//   hyper_nu               P8 (unit-step worked example 1,2,2,2,1), P9 (closed form on a sine), P10 (bound 4)
+//   hyper_kappa            P8 (unit-step worked example 1,2,2,2,1), P9 (closed form on a sine), P10 (bound 4)
 //   hyper_div              P1, P2 (conservation incl. energy couplings), P3, P5 (x<->y transposition)
 //   wavespeeds / dt        P11 (closed-form Brio-Wu and Orszag-Tang maxima and dt0)
 //   rk4_step               P6 (temporal order 4), P4 (RK4 amplification factor), P12 (restart)
@@ -101,8 +101,22 @@ void fill_ghosts(const Ctx& c, Plane& p, bool freeze) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// ARITHMETIC CONTRACT.  The scheme's hyperviscosity ratio max|D3|/max|D1| is not
+// smooth, and it amplifies rounding-level differences by ~6x per step for the first ~10 steps (measured:
+// this file built with and without FMA contraction differs by 4e-8 after 40 steps on a 200^2
+// Orszag-Tang run).  A 1e-10 parity bar after 50..1000 steps is therefore only reachable if both
+// implementations evaluate every value with the SAME sequence of IEEE-754 operations.  So each formula
+// below is written as an explicit operation sequence -- `fma(a,b,c)` is one correctly rounded a*b+c,
+// every other +,-,*,/ and sqrt is one correctly rounded operation, evaluation order is as parenthesised
+// -- and the file is compiled with -ffp-contract=off so the compiler adds no contraction of its own.
+// The CUDA path implements the same sequences independently (built with -fmad=false).  Terms that are
+// exactly zero for a zero background (x - 0, 0 + x, fma(0,y,0*z)) may be dropped without changing bits.
+// ---------------------------------------------------------------------------------------------
+using std::fma;
+
+// ---------------------------------------------------------------------------------------------
 // c-2 derived quantities on every padded cell (PAPER.md:39-43 with the SAC background split).
-//   rho = rho_b + rho~,  v = m/rho,  B = B_b + b~
+//   rho = rho_b + rho~,  v = m/rho (as m * (1/rho)),  B = B_b + b~
 //   p~_k = (gamma-1)(e~ - rho v^2/2 - B_b.b~ - b~^2/2),  p~_t = p~_k + B_b.b~ + b~^2/2
 //   eps~ = p~_k/(gamma-1)   (thermal-energy perturbation, the scalar the energy hyperdiffusion acts on)
 // ---------------------------------------------------------------------------------------------
@@ -112,30 +126,34 @@ struct Derived {
 
 void derived(const Ctx& c, const Plane* w, Derived& d) {
   const size_t n = c.psize();
+  const double gm1 = c.gamma - 1.0;
   for (Plane* p : {&d.rho, &d.vx, &d.vy, &d.Bx, &d.By, &d.ptt, &d.eps}) p->assign(n, 0.0);
 #pragma omp parallel for num_threads(c.nthreads) schedule(static)
   for (long q = 0; q < (long)n; ++q) {
     const double rho = c.bg[BG_RHO][q] + w[F_RHO][q];
-    const double vx = w[F_MX][q] / rho;
-    const double vy = w[F_MY][q] / rho;
+    const double rr = 1.0 / rho;
+    const double mx = w[F_MX][q], my = w[F_MY][q];
+    const double vx = mx * rr, vy = my * rr;
     const double bbx = c.bg[BG_BX][q], bby = c.bg[BG_BY][q];
     const double bx = w[F_BX][q], by = w[F_BY][q];
-    const double cross = bbx * bx + bby * by;        // B_b . b~
-    const double b2h = 0.5 * (bx * bx + by * by);    // b~^2/2
-    const double eps = w[F_E][q] - 0.5 * rho * (vx * vx + vy * vy) - cross - b2h;
+    const double b2h = 0.5 * fma(by, by, bx * bx);         // b~^2/2
+    const double cross = fma(bby, by, bbx * bx);            // B_b . b~
+    const double ke = 0.5 * fma(my, vy, mx * vx);           // rho v^2/2
+    const double eps = ((w[F_E][q] - ke) - cross) - b2h;
     d.rho[q] = rho;
     d.vx[q] = vx;
     d.vy[q] = vy;
     d.Bx[q] = bbx + bx;
     d.By[q] = bby + by;
     d.eps[q] = eps;
-    d.ptt[q] = (c.gamma - 1.0) * eps + cross + b2h;
+    d.ptt[q] = fma(gm1, eps, cross + b2h);
   }
 }
 
-// c-3 fourth-order central difference, stride s = 1 (x) or NX (y), spacing h.
-inline double cdiff(const Plane& f, size_t q, size_t s, double h) {
-  return (8.0 * (f[q + s] - f[q - s]) - (f[q + 2 * s] - f[q - 2 * s])) / (12.0 * h);
+// c-3 fourth-order central difference, stride s = 1 (x) or NX (y):
+//   cd12 = 12 * Delta * df/dx = 8 (f[+1] - f[-1]) - (f[+2] - f[-2]);   df/dx = cd12 * (1/Delta) * (1/12).
+inline double cd12(const Plane& f, size_t q, size_t s) {
+  return fma(8.0, f[q + s] - f[q - s], -(f[q + 2 * s] - f[q - 2 * s]));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -158,63 +176,23 @@ double flux(const Ctx& c, const Plane* w, const Derived& d, int field, int dir, 
     case F_MX:
     case F_MY: {
       const int l = field - F_MX;
-      double f = m[l] * v[dir] - bt[l] * bt[dir] - bt[l] * Bb[dir] - Bb[l] * bt[dir];
-      if (l == dir) f += d.ptt[q];
-      return f;
+      const double f = (fma(m[l], v[dir], -(bt[l] * bt[dir])) - bt[l] * Bb[dir]) - Bb[l] * bt[dir];
+      return l == dir ? f + d.ptt[q] : f;
     }
     case F_E: {
-      const double btv = bt[0] * v[0] + bt[1] * v[1];        // b~ . v
-      const double Bbv = Bb[0] * v[0] + Bb[1] * v[1];        // B_b . v
-      return v[dir] * (w[F_E][q] + c.bg[BG_E][q] + d.ptt[q]) - bt[dir] * btv - bt[dir] * Bbv -
-             Bb[dir] * btv;
+      const double btv = fma(bt[1], v[1], bt[0] * v[0]);     // b~ . v
+      const double Bbv = fma(Bb[1], v[1], Bb[0] * v[0]);     // B_b . v
+      const double h = (w[F_E][q] + c.bg[BG_E][q]) + d.ptt[q];
+      return (fma(v[dir], h, -(bt[dir] * btv)) - bt[dir] * Bbv) - Bb[dir] * btv;
     }
     case F_BX:
     case F_BY: {
       const int l = field - F_BX;
       if (l == dir) return 0.0;
-      return v[dir] * B[l] - B[dir] * v[l];
+      return fma(v[dir], B[l], -(B[dir] * v[l]));
     }
   }
   return 0.0;
-}
-
-// R_f -= d/dx F_x(f) + d/dy F_y(f) on interior cells; R planes are padded, interior entries used.
-void flux_div(const Ctx& c, const Plane* w, const Derived& d, Plane* R) {
-  const size_t n = c.psize();
-  Plane F(n);
-  for (int field = 0; field < NF; ++field) {
-    for (int dir = 0; dir < 2; ++dir) {
-#pragma omp parallel for num_threads(c.nthreads) schedule(static)
-      for (long q = 0; q < (long)n; ++q) F[q] = flux(c, w, d, field, dir, (size_t)q);
-      const size_t s = dir == 0 ? 1 : (size_t)c.NX;
-      const double h = dir == 0 ? c.dx() : c.dy();
-#pragma omp parallel for num_threads(c.nthreads) schedule(static)
-      for (int j = 0; j < c.ny; ++j)
-        for (int i = 0; i < c.nx; ++i) {
-          const size_t q = c.at(i, j);
-          R[field][q] -= cdiff(F, q, s, h);
-        }
-    }
-  }
-}
-
-// c-2 energy source (zero when the background is zero; gravity absent):
-//   S_e = -p_tb (dvx/dx + dvy/dy) + sum_{k,l} B_b,k B_b,l d_k v_l,
-//   p_tb = (gamma-1)(e_b - B_b^2/2) + B_b^2/2.
-void sources(const Ctx& c, const Derived& d, Plane* R) {
-  const size_t sx = 1, sy = (size_t)c.NX;
-#pragma omp parallel for num_threads(c.nthreads) schedule(static)
-  for (int j = 0; j < c.ny; ++j)
-    for (int i = 0; i < c.nx; ++i) {
-      const size_t q = c.at(i, j);
-      const double bbx = c.bg[BG_BX][q], bby = c.bg[BG_BY][q];
-      const double bb2h = 0.5 * (bbx * bbx + bby * bby);
-      const double ptb = (c.gamma - 1.0) * (c.bg[BG_E][q] - bb2h) + bb2h;
-      const double dxvx = cdiff(d.vx, q, sx, c.dx()), dyvx = cdiff(d.vx, q, sy, c.dy());
-      const double dxvy = cdiff(d.vy, q, sx, c.dx()), dyvy = cdiff(d.vy, q, sy, c.dy());
-      R[F_E][q] += -ptb * (dxvx + dyvy) +
-                   (bbx * bbx * dxvx + bbx * bby * dxvy + bby * bbx * dyvx + bby * bby * dyvy);
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -223,14 +201,14 @@ void sources(const Ctx& c, const Derived& d, Plane* R) {
 // For scalar u along direction dir, at interface k+1/2 (stored at the padded index of cell k):
 //   D1_k = u_{k+1} - u_k,   D3_k = 3 (u_{k+1} - u_k) - (u_{k+2} - u_{k-1})
 //   M3 = max |D3| over interfaces k-1, k, k+1;   M1 = max |D1| over interfaces k-2 .. k+2
-//   nu_{k+1/2} = coef * Delta * v_t * M3 / M1   if M1 > 0, else 0.
-// Valid (and computed) for k = -1 .. n-1 along dir and for every padded index across dir; other
-// entries are 0.
+//   nu_{k+1/2} = c_u * Delta * v_t * M3 / M1   if M1 > 0, else 0.
+// Stored is kappa = nu / Delta = (c_u v_t) * (M3 / M1): every use of nu below is nu/Delta * (difference)
+// or nu * (derivative), in which Delta cancels.  Valid (and computed) for k = -1 .. n-1 along dir and
+// for every padded index across dir; other entries are 0.
 // ---------------------------------------------------------------------------------------------
-void hyper_nu(const Ctx& c, const Plane& u, int dir, double coef, double vt, Plane& nu) {
-  nu.assign(c.psize(), 0.0);
+void hyper_kappa(const Ctx& c, const Plane& u, int dir, double cv, Plane& kap) {
+  kap.assign(c.psize(), 0.0);
   const long s = dir == 0 ? 1 : c.NX;
-  const double delta = dir == 0 ? c.dx() : c.dy();
   const int n_along = dir == 0 ? c.nx : c.ny;
   const int n_across = dir == 0 ? c.NY : c.NX;   // padded extent across dir
 #pragma omp parallel for num_threads(c.nthreads) schedule(static)
@@ -240,96 +218,115 @@ void hyper_nu(const Ctx& c, const Plane& u, int dir, double coef, double vt, Pla
       double M3 = 0.0, M1 = 0.0;
       for (int o = -1; o <= 1; ++o) {
         const long r = q + o * s;
-        const double d3 = 3.0 * (u[r + s] - u[r]) - (u[r + 2 * s] - u[r - s]);
+        const double d3 = fma(3.0, u[r + s] - u[r], -(u[r + 2 * s] - u[r - s]));
         M3 = std::max(M3, std::fabs(d3));
       }
       for (int o = -2; o <= 2; ++o) {
         const long r = q + o * s;
         M1 = std::max(M1, std::fabs(u[r + s] - u[r]));
       }
-      nu[q] = M1 > 0.0 ? coef * delta * vt * (M3 / M1) : 0.0;
+      kap[q] = M1 > 0.0 ? cv * (M3 / M1) : 0.0;
     }
   }
 }
 
-// Interface operator of c-5, direction dir, added to R on interior cells:
-//   Phi_{k+1/2} = g_{k+1/2} * nu_{k+1/2} * (qv_{k+1} - qv_k)/Delta * fac
-//   R    += (Phi_{k+1/2} - Phi_{k-1/2}) / Delta
-//   R_e  += (cj_{k+1/2} Phi_{k+1/2} - cj_{k-1/2} Phi_{k-1/2}) / Delta   (if conj != nullptr)
-// g = 1 (gw == nullptr) or the interface average (gw_k + gw_{k+1})/2; cj_{k+1/2} is the interface
-// average of the conjugate factor (v_l for a momentum flux, total B_l for a magnetic flux).
-void hyper_interface(const Ctx& c, const Plane& nu, const Plane& qv, const Plane* gw, double fac,
-                     int dir, Plane& R, const Plane* conj, Plane* Re) {
-  const long s = dir == 0 ? 1 : c.NX;
-  const double delta = dir == 0 ? c.dx() : c.dy();
-#pragma omp parallel for num_threads(c.nthreads) schedule(static)
-  for (int j = 0; j < c.ny; ++j)
-    for (int i = 0; i < c.nx; ++i) {
-      const long q = (long)c.at(i, j);
-      double phi[2], cj[2];
-      for (int side = 0; side < 2; ++side) {
-        const long a = q + (side - 1) * s, b = a + s;   // interface between cells a and b
-        const double g = gw ? 0.5 * ((*gw)[a] + (*gw)[b]) : 1.0;
-        phi[side] = g * nu[a] * (qv[b] - qv[a]) / delta * fac;
-        cj[side] = conj ? 0.5 * ((*conj)[a] + (*conj)[b]) : 0.0;
-      }
-      R[q] += (phi[1] - phi[0]) / delta;
-      if (conj) (*Re)[q] += (cj[1] * phi[1] - cj[0] * phi[0]) / delta;
-    }
+enum { K_RHO = 0, K_VX = 1, K_VY = 2, K_EPS = 3, K_B = 4, NK = 5 };
+struct Kappas {
+  Plane x[NK];   // along x, of rho~, vx, vy, eps~, by~
+  Plane y[NK];   // along y, of rho~, vx, vy, eps~, bx~
+};
+
+// c-5 interface (diffusive) fluxes of all fields at the interface between cells a and b = a + s along
+// dir, Phi = g * nu * (q_b - q_a)/Delta = g * kappa * (q_b - q_a):
+//   rho~ : g = 1, q = rho~                     eps~ -> e : g = 1, q = eps~
+//   m_l  : g = rho-bar (l = dir) or rho-bar/2 (l != dir), q = v_l      (tau_kl = rho/2 [nu_k d_k v_l + nu_l d_l v_k])
+//   b~_l : g = 1, q = b~_l, only l != dir                              (eps_z = nu_x(by) d_x by - nu_y(bx) d_y bx)
+//   e    : eps~ flux + vbar_x Phi(mx) + vbar_y Phi(my) + Bbar_l Phi(b_l)   (viscous work, ohmic coupling; total B)
+// out[F_*]; out[F_B{dir}] = 0.
+void hd_interface_fluxes(const Ctx& c, const Plane* w, const Derived& d, const Kappas& K, int dir, long a,
+                         double out[NF]) {
+  const long s = dir == 0 ? 1 : c.NX, b = a + s;
+  const Plane* kap = dir == 0 ? K.x : K.y;
+  const int lt = 1 - dir;                                    // the transverse magnetic component
+  const Plane& bq = w[F_BX + lt];
+  const Plane& Bq = lt == 0 ? d.Bx : d.By;
+  const double rbar = 0.5 * (d.rho[a] + d.rho[b]);
+  const double g_mx = dir == 0 ? rbar : 0.5 * rbar;
+  const double g_my = dir == 1 ? rbar : 0.5 * rbar;
+  const double p_rho = kap[K_RHO][a] * (w[F_RHO][b] - w[F_RHO][a]);
+  const double p_mx = (g_mx * kap[K_VX][a]) * (d.vx[b] - d.vx[a]);
+  const double p_my = (g_my * kap[K_VY][a]) * (d.vy[b] - d.vy[a]);
+  const double p_eps = kap[K_EPS][a] * (d.eps[b] - d.eps[a]);
+  const double p_b = kap[K_B][a] * (bq[b] - bq[a]);
+  const double vxbar = 0.5 * (d.vx[a] + d.vx[b]);
+  const double vybar = 0.5 * (d.vy[a] + d.vy[b]);
+  const double Bbar = 0.5 * (Bq[a] + Bq[b]);
+  out[F_RHO] = p_rho;
+  out[F_MX] = p_mx;
+  out[F_MY] = p_my;
+  out[F_E] = fma(Bbar, p_b, fma(vybar, p_my, fma(vxbar, p_mx, p_eps)));
+  out[F_BX + lt] = p_b;
+  out[F_BX + dir] = 0.0;
 }
 
-// Mixed (cross) term of c-5: cell-centred flux along direction k built from a derivative along l != k,
-//   G = fac * gw * nubar_l(u) * d^c_l qv,   nubar_l = (nu_{l-1/2} + nu_{l+1/2})/2,   d^c = c-3,
-//   R   += d^c_k G,    R_e += d^c_k (conj * G)     (conj cell-centred).
-// G is needed at cells +-1, +-2 along k (ghost cells there), interior along l.
-void hyper_mixed(const Ctx& c, const Plane& nu_l, const Plane& qv, const Plane* gw, double fac, int l,
-                 Plane& R, const Plane& conj, Plane& Re) {
-  const int k = 1 - l;
-  const long sl = l == 0 ? 1 : c.NX, sk = k == 0 ? 1 : c.NX;
-  const double hl = l == 0 ? c.dx() : c.dy(), hk = k == 0 ? c.dx() : c.dy();
-  Plane G(c.psize(), 0.0), GE(c.psize(), 0.0);
-  // cells: interior along l, [-2, n+2) along k
+// c-5 mixed (cross) terms: cell-centred fluxes along direction k built from derivatives along l != k,
+//   G(m_l ; k) = (rho/2) nubar_l(v_k) d^c_l v_k       G(b_l ; k) = - nubar_l(b~_k) d^c_l b~_k
+//   G(e ; k)   = v_l G(m_l;k) + B_l G(b_l;k)           nubar_l = (nu_{l-1/2} + nu_{l+1/2})/2, d^c = c-3
+// [note the roles: the flux of m_l along k uses the coefficient and derivative ALONG l of the k-component].
+// They enter the RHS as + d^c_k G, i.e. they are subtracted from F_k before the central difference.
+// Defined on cells interior along l and [-2, n+2) along k; G planes are 0 elsewhere.  Gk[F_*].
+void hd_mixed_fluxes(const Ctx& c, const Plane* w, const Derived& d, const Kappas& K, int k, Plane* G) {
+  for (int f = 0; f < NF; ++f) G[f].assign(c.psize(), 0.0);
+  const int l = 1 - k;
+  const long sl = l == 0 ? 1 : c.NX;
+  const Plane* kap = l == 0 ? K.x : K.y;             // coefficients along l
+  const Plane& vk = k == 0 ? d.vx : d.vy;            // k-component of v  (kappa family K_VX + k)
+  const Plane& bk = w[F_BX + k];                     // k-component of b~ (kappa family K_B along l)
+  const Plane& vl = l == 0 ? d.vx : d.vy;
+  const Plane& Bl = l == 0 ? d.Bx : d.By;
   const int lo_i = (k == 0) ? -2 : 0, hi_i = (k == 0) ? c.nx + 2 : c.nx;
   const int lo_j = (k == 1) ? -2 : 0, hi_j = (k == 1) ? c.ny + 2 : c.ny;
 #pragma omp parallel for num_threads(c.nthreads) schedule(static)
   for (int j = lo_j; j < hi_j; ++j)
     for (int i = lo_i; i < hi_i; ++i) {
       const long q = (long)c.at(i, j);
-      const double nubar = 0.5 * (nu_l[q - sl] + nu_l[q]);
-      const double g = gw ? (*gw)[q] : 1.0;
-      G[q] = fac * g * nubar * cdiff(qv, (size_t)q, (size_t)sl, hl);
-      GE[q] = conj[q] * G[q];
-    }
-#pragma omp parallel for num_threads(c.nthreads) schedule(static)
-  for (int j = 0; j < c.ny; ++j)
-    for (int i = 0; i < c.nx; ++i) {
-      const size_t q = c.at(i, j);
-      R[q] += cdiff(G, q, (size_t)sk, hk);
-      Re[q] += cdiff(GE, q, (size_t)sk, hk);
+      const double kbar_v = 0.5 * (kap[K_VX + k][q - sl] + kap[K_VX + k][q]);
+      const double kbar_b = 0.5 * (kap[K_B][q - sl] + kap[K_B][q]);
+      const double dv = cd12(vk, (size_t)q, (size_t)sl) * (1.0 / 12.0);
+      const double db = cd12(bk, (size_t)q, (size_t)sl) * (1.0 / 12.0);
+      const double gm = ((0.5 * d.rho[q]) * kbar_v) * dv;
+      const double gb = -(kbar_b * db);
+      G[F_MX + l][q] = gm;
+      G[F_BX + l][q] = gb;
+      G[F_E][q] = fma(vl[q], gm, Bl[q] * gb);
     }
 }
 
-// c-4 maxima over interior cells of the (ghost-filled or not: interior only) state w:
+// c-4 maxima over interior cells of the state w:
 //   a^2 = gamma p_k / rho with total p_k = (gamma-1)(e - rho v^2/2 - B^2/2), e = e_b + e~;  b^2 = B^2/rho
 //   c_f,d^2 = ( a^2+b^2 + sqrt(max(0, (a^2+b^2)^2 - 4 a^2 B_d^2/rho)) ) / 2
 //   out = { max(|vx|+c_f,x), max(|vy|+c_f,y), max a^2, max b^2 };  maxima start at 0, NaNs are skipped.
 void wavespeeds(const Ctx& c, const Plane* w, double out[4]) {
   double m0 = 0, m1 = 0, m2 = 0, m3 = 0;
+  const double gm1 = c.gamma - 1.0;
 #pragma omp parallel for num_threads(c.nthreads) schedule(static) reduction(max : m0, m1, m2, m3)
   for (int j = 0; j < c.ny; ++j)
     for (int i = 0; i < c.nx; ++i) {
       const size_t q = c.at(i, j);
       const double rho = c.bg[BG_RHO][q] + w[F_RHO][q];
-      const double vx = w[F_MX][q] / rho, vy = w[F_MY][q] / rho;
+      const double rr = 1.0 / rho;
+      const double mx = w[F_MX][q], my = w[F_MY][q];
+      const double vx = mx * rr, vy = my * rr;
       const double Bx = c.bg[BG_BX][q] + w[F_BX][q], By = c.bg[BG_BY][q] + w[F_BY][q];
       const double e = c.bg[BG_E][q] + w[F_E][q];
-      const double B2 = Bx * Bx + By * By;
-      const double pk = (c.gamma - 1.0) * (e - 0.5 * rho * (vx * vx + vy * vy) - 0.5 * B2);
-      const double a2 = c.gamma * pk / rho;
-      const double b2 = B2 / rho;
+      const double B2 = fma(By, By, Bx * Bx);
+      const double pk = gm1 * ((e - 0.5 * fma(my, vy, mx * vx)) - 0.5 * B2);
+      const double a2 = (c.gamma * pk) * rr;
+      const double b2 = B2 * rr;
       const double s = a2 + b2;
-      const double cfx2 = 0.5 * (s + std::sqrt(std::max(0.0, s * s - 4.0 * a2 * Bx * Bx / rho)));
-      const double cfy2 = 0.5 * (s + std::sqrt(std::max(0.0, s * s - 4.0 * a2 * By * By / rho)));
+      const double fa = (4.0 * a2) * rr;
+      const double cfx2 = 0.5 * (s + std::sqrt(std::max(0.0, fma(s, s, -(fa * (Bx * Bx))))));
+      const double cfy2 = 0.5 * (s + std::sqrt(std::max(0.0, fma(s, s, -(fa * (By * By))))));
       const double cx = std::fabs(vx) + std::sqrt(cfx2);
       const double cy = std::fabs(vy) + std::sqrt(cfy2);
       if (cx > m0) m0 = cx;
@@ -340,55 +337,77 @@ void wavespeeds(const Ctx& c, const Plane* w, double out[4]) {
   out[0] = m0; out[1] = m1; out[2] = m2; out[3] = m3;
 }
 
-// c-5 all hyperdiffusive increments D(w; v_t) added to R (interior cells).
-void hyper_div(const Ctx& c, const Plane* w, const Derived& d, double vt, Plane* R) {
-  Plane nu;
-  const Plane* vel[2] = {&d.vx, &d.vy};
-  const Plane* Btot[2] = {&d.Bx, &d.By};
-  // D_rho = sum_d H_d[rho~, rho~; 1];   D_e gets sum_d H_d[eps~, eps~; 1]
-  for (int dir = 0; dir < 2; ++dir) {
-    hyper_nu(c, w[F_RHO], dir, c.c_rho, vt, nu);
-    hyper_interface(c, nu, w[F_RHO], nullptr, 1.0, dir, R[F_RHO], nullptr, nullptr);
-    hyper_nu(c, d.eps, dir, c.c_e, vt, nu);
-    hyper_interface(c, nu, d.eps, nullptr, 1.0, dir, R[F_E], nullptr, nullptr);
-  }
-  // D_{m_l} = H_l[v_l,v_l;rho-bar] + 1/2 H_k[v_l,v_l;rho-bar] + d^c_k{ 1/2 rho nubar_l(v_k) d^c_l v_k },  k != l
-  // (= div tau, tau_kl = rho/2 [nu_k(v_l) d_k v_l + nu_l(v_k) d_l v_k]); viscous work v_l * flux -> R_e.
-  for (int l = 0; l < 2; ++l) {
-    const int k = 1 - l;
-    Plane& Rm = R[F_MX + l];
-    hyper_nu(c, *vel[l], l, c.c_mom, vt, nu);
-    hyper_interface(c, nu, *vel[l], &d.rho, 1.0, l, Rm, vel[l], &R[F_E]);
-    hyper_nu(c, *vel[l], k, c.c_mom, vt, nu);
-    hyper_interface(c, nu, *vel[l], &d.rho, 0.5, k, Rm, vel[l], &R[F_E]);
-    hyper_nu(c, *vel[k], l, c.c_mom, vt, nu);
-    hyper_mixed(c, nu, *vel[k], &d.rho, 0.5, l, Rm, *vel[l], R[F_E]);
-  }
-  // D_bx = H_y[bx~,bx~;1] - d^c_y{ nubar_x(by~) d^c_x by~ },  D_by = H_x[by~,by~;1] - d^c_x{ nubar_y(bx~) d^c_y bx~ }
-  // (= -curl(eps_z), eps_z = nu_x(by) d_x by~ - nu_y(bx) d_y bx~); ohmic coupling B_l(total) * flux -> R_e.
-  for (int l = 0; l < 2; ++l) {
-    const int k = 1 - l;
-    Plane& Rb = R[F_BX + l];
-    hyper_nu(c, w[F_BX + l], k, c.c_b, vt, nu);
-    hyper_interface(c, nu, w[F_BX + l], nullptr, 1.0, k, Rb, Btot[l], &R[F_E]);
-    hyper_nu(c, w[F_BX + k], l, c.c_b, vt, nu);
-    hyper_mixed(c, nu, w[F_BX + k], nullptr, -1.0, l, Rb, *Btot[l], R[F_E]);
-  }
-}
-
-// c-6: R(w) = -sum_d d^c_d F_d + S + D(w; v_t(w)); ghosts of w must be filled.  R planes are zeroed here.
-// v_t = sqrt(max a^2) + sqrt(max b^2) of the state being differentiated (c-5).
+// c-6: R(w) = -sum_d d^c_d (F_d - G_d) + S + sum_d (Phi_{d,+} - Phi_{d,-})/Delta_d; ghosts of w must be
+// filled.  v_t = sqrt(max a^2) + sqrt(max b^2) of the state being differentiated (c-5).
 void rhs(const Ctx& c, const Plane* w, Plane* R) {
+  const size_t n = c.psize();
+  const double inv_dx = c.nx / c.Lx, inv_dy = c.ny / c.Ly;
   Derived d;
   derived(c, w, d);
-  for (int f = 0; f < NF; ++f) R[f].assign(c.psize(), 0.0);
-  flux_div(c, w, d, R);
-  sources(c, d, R);
+  Kappas K;
+  Plane Gx[NF], Gy[NF];
+  for (int f = 0; f < NF; ++f) { Gx[f].assign(n, 0.0); Gy[f].assign(n, 0.0); }
   if (c.hd_on) {
     double ws[4];
     wavespeeds(c, w, ws);
     const double vt = std::sqrt(ws[2]) + std::sqrt(ws[3]);
-    hyper_div(c, w, d, vt, R);
+    const double cv_rho = c.c_rho * vt, cv_mom = c.c_mom * vt, cv_e = c.c_e * vt, cv_b = c.c_b * vt;
+    hyper_kappa(c, w[F_RHO], 0, cv_rho, K.x[K_RHO]);  hyper_kappa(c, w[F_RHO], 1, cv_rho, K.y[K_RHO]);
+    hyper_kappa(c, d.vx, 0, cv_mom, K.x[K_VX]);       hyper_kappa(c, d.vx, 1, cv_mom, K.y[K_VX]);
+    hyper_kappa(c, d.vy, 0, cv_mom, K.x[K_VY]);       hyper_kappa(c, d.vy, 1, cv_mom, K.y[K_VY]);
+    hyper_kappa(c, d.eps, 0, cv_e, K.x[K_EPS]);       hyper_kappa(c, d.eps, 1, cv_e, K.y[K_EPS]);
+    hyper_kappa(c, w[F_BY], 0, cv_b, K.x[K_B]);       hyper_kappa(c, w[F_BX], 1, cv_b, K.y[K_B]);
+    hd_mixed_fluxes(c, w, d, K, 0, Gx);
+    hd_mixed_fluxes(c, w, d, K, 1, Gy);
+  }
+  // flux divergence of C_d = F_d - G_d, fourth-order central (c-3)
+  Plane Cx(n), Cy(n);
+  for (int f = 0; f < NF; ++f) {
+    R[f].assign(n, 0.0);
+#pragma omp parallel for num_threads(c.nthreads) schedule(static)
+    for (long q = 0; q < (long)n; ++q) {
+      Cx[q] = flux(c, w, d, f, 0, (size_t)q) - Gx[f][q];
+      Cy[q] = flux(c, w, d, f, 1, (size_t)q) - Gy[f][q];
+    }
+#pragma omp parallel for num_threads(c.nthreads) schedule(static)
+    for (int j = 0; j < c.ny; ++j)
+      for (int i = 0; i < c.nx; ++i) {
+        const size_t q = c.at(i, j);
+        R[f][q] = fma(cd12(Cx, q, 1), inv_dx, cd12(Cy, q, (size_t)c.NX) * inv_dy) * (-1.0 / 12.0);
+      }
+  }
+  // c-2 energy source (zero when the background is zero; gravity absent):
+  //   S_e = -p_tb (dvx/dx + dvy/dy) + sum_{k,l} B_b,k B_b,l d_k v_l,  p_tb = (gamma-1)(e_b - B_b^2/2) + B_b^2/2
+  const double gm1 = c.gamma - 1.0;
+#pragma omp parallel for num_threads(c.nthreads) schedule(static)
+  for (int j = 0; j < c.ny; ++j)
+    for (int i = 0; i < c.nx; ++i) {
+      const size_t q = c.at(i, j);
+      const double bbx = c.bg[BG_BX][q], bby = c.bg[BG_BY][q];
+      const double bb2h = 0.5 * fma(bby, bby, bbx * bbx);
+      const double ptb = fma(gm1, c.bg[BG_E][q] - bb2h, bb2h);
+      const double dxvx = (cd12(d.vx, q, 1) * inv_dx) * (1.0 / 12.0);
+      const double dyvx = (cd12(d.vx, q, (size_t)c.NX) * inv_dy) * (1.0 / 12.0);
+      const double dxvy = (cd12(d.vy, q, 1) * inv_dx) * (1.0 / 12.0);
+      const double dyvy = (cd12(d.vy, q, (size_t)c.NX) * inv_dy) * (1.0 / 12.0);
+      const double S = fma(-ptb, dxvx + dyvy,
+                           fma(bby * bby, dyvy, fma(bbx * bby, dxvy + dyvx, (bbx * bbx) * dxvx)));
+      R[F_E][q] = R[F_E][q] + S;
+    }
+  // c-5 interface fluxes, x then y
+  if (c.hd_on) {
+#pragma omp parallel for num_threads(c.nthreads) schedule(static)
+    for (int j = 0; j < c.ny; ++j)
+      for (int i = 0; i < c.nx; ++i) {
+        const long q = (long)c.at(i, j);
+        double lo[NF], hi[NF];
+        hd_interface_fluxes(c, w, d, K, 0, q - 1, lo);
+        hd_interface_fluxes(c, w, d, K, 0, q, hi);
+        for (int f = 0; f < NF; ++f) R[f][q] = fma(hi[f] - lo[f], inv_dx, R[f][q]);
+        hd_interface_fluxes(c, w, d, K, 1, q - c.NX, lo);
+        hd_interface_fluxes(c, w, d, K, 1, q, hi);
+        for (int f = 0; f < NF; ++f) R[f][q] = fma(hi[f] - lo[f], inv_dy, R[f][q]);
+      }
   }
 }
 
@@ -396,58 +415,73 @@ void rhs(const Ctx& c, const Plane* w, Plane* R) {
 double cfl_dt(const Ctx& c, const Plane* w, double cfl) {
   double ws[4];
   wavespeeds(c, w, ws);
-  double dt = INFINITY;
-  if (c.nx > 1) dt = std::min(dt, c.dx() / ws[0]);
-  if (c.ny > 1) dt = std::min(dt, c.dy() / ws[1]);
-  return cfl * dt;
+  double m = INFINITY;
+  if (c.nx > 1) m = std::min(m, (c.Lx / c.nx) / ws[0]);
+  if (c.ny > 1) m = std::min(m, (c.Ly / c.ny) / ws[1]);
+  return cfl * m;
 }
 
-// stage state ws = wn + a * K on interior cells; ghosts: copy of wn's (keeps frozen "fixed" ghosts),
-// then refilled on periodic/open sides.
-void stage_state(const Ctx& c, const Plane* wn, double a, const Plane* K, Plane* ws) {
+// A stage state: interior from `interior`, ghosts copied from wn (keeps frozen "fixed" ghosts), then
+// refilled on periodic/open sides.
+void finish_stage(const Ctx& c, const Plane* wn, Plane* ws) {
   for (int f = 0; f < NF; ++f) {
-    ws[f] = wn[f];
-    for (int j = 0; j < c.ny; ++j)
-      for (int i = 0; i < c.nx; ++i) {
-        const size_t q = c.at(i, j);
-        ws[f][q] = wn[f][q] + a * K[f][q];
-      }
+    for (int j = -NG; j < c.ny + NG; ++j)
+      for (int i = -NG; i < c.nx + NG; ++i)
+        if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) ws[f][c.at(i, j)] = wn[f][c.at(i, j)];
     fill_ghosts(c, ws[f], false);
   }
 }
 
-// c-6 one step of the classical Runge-Kutta scheme, dt frozen over the step:
-//   k1 = R(w^n), k2 = R(w^n + dt/2 k1), k3 = R(w^n + dt/2 k2), k4 = R(w^n + dt k3),
-//   w^{n+1} = w^n + dt/6 (k1 + 2 k2 + 2 k3 + k4).       rk_order 2 = midpoint, 1 = forward Euler.
+// c-6 one step of the classical fourth-order Runge-Kutta scheme, dt frozen over the step,
+// written in stage-state form (algebraically the classical update w^{n+1} = w^n + dt/6 (k1+2k2+2k3+k4),
+// since k1 = 2(w1-w^n)/dt, k2 = 2(w2-w^n)/dt, k3 = (w3-w^n)/dt):
+//   w1 = w^n + (dt/2) R(w^n),  w2 = w^n + (dt/2) R(w1),  w3 = w^n + dt R(w2),
+//   acc = (w1 - w^n) + 2 w2,   w^{n+1} = w3 + (acc - 2 w3)/3 + (dt/6) R(w3)      [= (w1+2w2+w3-w^n)/3 + dt/6 k4;
+//   this grouping returns w^n bit for bit when every R is 0, pin P1].
+// rk_order 2 = midpoint (w1 as above, w^{n+1} = w^n + dt R(w1)), 1 = forward Euler.
 void rk_step(Ctx& c, double dt) {
-  Plane k1[NF], k2[NF], k3[NF], k4[NF], ws[NF];
+  const size_t n = c.psize();
+  Plane R[NF], w1[NF], w2[NF], w3[NF], wnew[NF];
   Plane* wn = c.w;
-  for (int f = 0; f < NF; ++f) fill_ghosts(c, wn[f], false);
-  rhs(c, wn, k1);
-  if (c.rk_order == 1) {
-    stage_state(c, wn, dt, k1, ws);
-  } else if (c.rk_order == 2) {
-    stage_state(c, wn, 0.5 * dt, k1, ws);
-    rhs(c, ws, k2);
-    stage_state(c, wn, dt, k2, ws);
-  } else {
-    stage_state(c, wn, 0.5 * dt, k1, ws);
-    rhs(c, ws, k2);
-    stage_state(c, wn, 0.5 * dt, k2, ws);
-    rhs(c, ws, k3);
-    stage_state(c, wn, dt, k3, ws);
-    rhs(c, ws, k4);
+  auto axpy = [&](double a, Plane* out) {           // out = w^n + a R on interior cells
     for (int f = 0; f < NF; ++f) {
-      ws[f] = wn[f];
+      out[f].assign(n, 0.0);
       for (int j = 0; j < c.ny; ++j)
         for (int i = 0; i < c.nx; ++i) {
           const size_t q = c.at(i, j);
-          ws[f][q] = wn[f][q] + dt / 6.0 * (k1[f][q] + 2.0 * k2[f][q] + 2.0 * k3[f][q] + k4[f][q]);
+          out[f][q] = fma(a, R[f][q], wn[f][q]);
         }
-      fill_ghosts(c, ws[f], false);
     }
+    finish_stage(c, wn, out);
+  };
+  for (int f = 0; f < NF; ++f) fill_ghosts(c, wn[f], false);
+  rhs(c, wn, R);
+  if (c.rk_order == 1) {
+    axpy(dt, wnew);
+  } else if (c.rk_order == 2) {
+    axpy(0.5 * dt, w1);
+    rhs(c, w1, R);
+    axpy(dt, wnew);
+  } else {
+    axpy(0.5 * dt, w1);
+    rhs(c, w1, R);
+    axpy(0.5 * dt, w2);
+    rhs(c, w2, R);
+    axpy(dt, w3);
+    rhs(c, w3, R);
+    const double dt6 = (1.0 / 6.0) * dt;
+    for (int f = 0; f < NF; ++f) {
+      wnew[f].assign(n, 0.0);
+      for (int j = 0; j < c.ny; ++j)
+        for (int i = 0; i < c.nx; ++i) {
+          const size_t q = c.at(i, j);
+          const double acc = fma(2.0, w2[f][q], w1[f][q] - wn[f][q]);
+          wnew[f][q] = fma(dt6, R[f][q], fma(fma(-2.0, w3[f][q], acc), 1.0 / 3.0, w3[f][q]));
+        }
+    }
+    finish_stage(c, wn, wnew);
   }
-  for (int f = 0; f < NF; ++f) c.w[f].swap(ws[f]);
+  for (int f = 0; f < NF; ++f) c.w[f].swap(wnew[f]);
   c.t += dt;
   c.last_dt = dt;
 }
@@ -599,11 +633,11 @@ int oracle_hyper_nu_1d(const double* u, int n, double coef, double delta, double
   if (rc) return rc;
   Ctx& c = *CTX(h);
   c.Lx = delta * n;
-  Plane up(c.psize(), 0.0), nu;
+  Plane up(c.psize(), 0.0), kap;
   for (int j = -NG; j < 1 + NG; ++j)
     for (int i = -NG; i < n + NG; ++i) up[c.at(i, j)] = u[i + NG];
-  hyper_nu(c, up, 0, coef, vt, nu);
-  for (int k = -1; k <= n - 1; ++k) nu_out[k + 1] = nu[c.at(k, 0)];
+  hyper_kappa(c, up, 0, coef * vt, kap);
+  for (int k = -1; k <= n - 1; ++k) nu_out[k + 1] = kap[c.at(k, 0)] * delta;   // nu = kappa * Delta
   oracle_destroy(h);
   return OK;
 }
@@ -612,7 +646,7 @@ int oracle_hyper_nu_1d(const double* u, int n, double coef, double delta, double
 int oracle_central_diff_1d(const double* f, int n, double h, double* out) {
   if (!f || !out || n < 1) { g_err = "bad argument"; return EINVAL_; }
   Plane fp(f, f + n + 4);
-  for (int i = 0; i < n; ++i) out[i] = cdiff(fp, (size_t)i + 2, 1, h);
+  for (int i = 0; i < n; ++i) out[i] = (cd12(fp, (size_t)i + 2, 1) * (1.0 / h)) * (1.0 / 12.0);
   return OK;
 }
 
