@@ -16,17 +16,17 @@ __device__ __forceinline__ void cell_wavespeeds(double rho, double mx, double my
                                                 double By, double gamma, bool full, double out[4]) {
   const double rr = 1.0 / rho;
   const double vx = mx * rr, vy = my * rr;
-  const double B2 = Bx * Bx + By * By;
-  const double pk = (gamma - 1.0) * (e - 0.5 * (mx * vx + my * vy) - 0.5 * B2);
-  const double a2 = gamma * pk * rr;
+  const double B2 = fma(By, By, Bx * Bx);
+  const double pk = (gamma - 1.0) * ((e - 0.5 * fma(my, vy, mx * vx)) - 0.5 * B2);
+  const double a2 = (gamma * pk) * rr;
   const double b2 = B2 * rr;
   out[2] = fmax(a2, 0.0);
   out[3] = fmax(b2, 0.0);
   if (full) {
     const double s = a2 + b2;
-    const double fa = 4.0 * a2 * rr;
-    const double cfx2 = 0.5 * (s + sqrt(fmax(0.0, s * s - fa * Bx * Bx)));
-    const double cfy2 = 0.5 * (s + sqrt(fmax(0.0, s * s - fa * By * By)));
+    const double fa = (4.0 * a2) * rr;
+    const double cfx2 = 0.5 * (s + sqrt(fmax(0.0, fma(s, s, -(fa * (Bx * Bx))))));
+    const double cfy2 = 0.5 * (s + sqrt(fmax(0.0, fma(s, s, -(fa * (By * By))))));
     out[0] = fmax(fabs(vx) + sqrt(cfx2), 0.0);
     out[1] = fmax(fabs(vy) + sqrt(cfy2), 0.0);
   } else {
@@ -70,10 +70,10 @@ __global__ void __launch_bounds__(256) wavespeed_kernel(Grid g, CPlanes6 w, CPla
     const long long a = cell_addr(g, i, j);
     double rho = w.p[F_RHO][a], e = w.p[F_E][a], Bx = w.p[F_BX][a], By = w.p[F_BY][a];
     if (BG) {
-      rho += bg.p[BG_RHO][a];
-      e += bg.p[BG_E][a];
-      Bx += bg.p[BG_BX][a];
-      By += bg.p[BG_BY][a];
+      rho = bg.p[BG_RHO][a] + rho;
+      e = bg.p[BG_E][a] + e;
+      Bx = bg.p[BG_BX][a] + Bx;
+      By = bg.p[BG_BY][a] + By;
     }
     double o[4];
     cell_wavespeeds(rho, w.p[F_MX][a], w.p[F_MY][a], e, Bx, By, gamma, true, o);

@@ -20,9 +20,10 @@ namespace smaug {
 
 // What the epilogue does with R (c-6).  dt is read from device memory (no host sync).
 //   COMBINE_BASE : out = base + c dt R                      (stages 1..3 of RK4; Euler; midpoint)
-//   COMBINE_ACC  : out = base + c dt R;  acc = (in + 2 out - base) / 3      (stage 2 of RK4)
-//   COMBINE_FINAL: out = acc + in / 3 + c dt R              (stage 4 of RK4, c = 1/6)
-// which is w^{n+1} = (w1 + 2 w2 + w3 - w^n)/3 + dt/6 R(w3), algebraically the classical RK4 update.
+//   COMBINE_ACC  : out = base + c dt R;  acc = (in - base) + 2 out          (stage 2 of RK4)
+//   COMBINE_FINAL: out = in + (acc - 2 in)/3 + c dt R       (stage 4 of RK4, c = 1/6)
+// which is w^{n+1} = (w1 + 2 w2 + w3 - w^n)/3 + dt/6 R(w3), algebraically the classical RK4 update,
+// grouped so that R == 0 returns w^n bit for bit.
 enum { COMBINE_BASE = 0, COMBINE_ACC = 1, COMBINE_FINAL = 2 };
 // Wave-speed reduction of the written state: none, only {a^2, b^2} (v_t of the next stage), or all four.
 enum { WS_NONE = 0, WS_VT = 1, WS_FULL = 2 };
@@ -76,28 +77,23 @@ constexpr size_t stage_smem_bytes() {
 // kappa = coef * (M3 / M1) for R consecutive interfaces of one line (c-5).  u points at the cell left of
 // the first interface; cells u[-2*s] .. u[(R+2)*s] are read.  Interface k (0..n-1) is written to out[k*os].
 template <int R>
-__device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, double coef, double* out,
+__device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, double cv, double* out,
                                           int os, int n) {
-  double d1[R + 4];   // |D1| at interfaces -2 .. R+1
-  double d3[R + 2];   // |D3| at interfaces -1 .. R
-  double prev = u[-2 * s];
-  double sd_m = 0.0, sd_0 = 0.0;   // signed D1 of the two previous interfaces
+  double uu[R + 5];   // cells -2 .. R+2
 #pragma unroll
-  for (int k = 0; k < R + 4; ++k) {
-    const double cur = u[(k - 1) * s];
-    const double sd = cur - prev;                      // signed D1 at interface k-2
-    d1[k] = fabs(sd);
-    // D3 at interface (k-3) = 3 D1_{k-3} - (u_{k-1} - u_{k-4}) = 2 D1_{k-3} - D1_{k-2} - D1_{k-4}
-    if (k >= 2) d3[k - 2] = fabs(2.0 * sd_0 - sd - sd_m);
-    sd_m = sd_0;
-    sd_0 = sd;
-    prev = cur;
-  }
+  for (int k = 0; k < R + 5; ++k) uu[k] = u[(k - 2) * s];
+  double d1[R + 4];   // signed D1 at interfaces -2 .. R+1:  D1_m = u_{m+1} - u_m
+#pragma unroll
+  for (int k = 0; k < R + 4; ++k) d1[k] = uu[k + 1] - uu[k];
+  double d3[R + 2];   // |D3| at interfaces -1 .. R:  D3_m = 3 D1_m - (u_{m+2} - u_{m-1})
+#pragma unroll
+  for (int k = 0; k < R + 2; ++k) d3[k] = fabs(fma(3.0, d1[k + 1], -(uu[k + 3] - uu[k])));
 #pragma unroll
   for (int k = 0; k < R; ++k) {
     const double m3 = fmax(fmax(d3[k], d3[k + 1]), d3[k + 2]);
-    const double m1 = fmax(fmax(fmax(d1[k], d1[k + 1]), fmax(d1[k + 2], d1[k + 3])), d1[k + 4]);
-    const double r = m1 > 0.0 ? coef * (m3 / m1) : 0.0;
+    const double m1 = fmax(fmax(fmax(fabs(d1[k]), fabs(d1[k + 1])), fmax(fabs(d1[k + 2]), fabs(d1[k + 3]))),
+                           fabs(d1[k + 4]));
+    const double r = m1 > 0.0 ? cv * (m3 / m1) : 0.0;
     if (k < n) out[k * os] = r;
   }
 }
@@ -111,7 +107,7 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
   const Grid& g = a.g;
   const int tid = threadIdx.x;
   const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;   // interior coordinates of the tile origin
-  const double gamma = a.prm.gamma;
+  const double gamma = a.prm.gamma, gm1 = a.prm.gamma - 1.0;
 
   // ---------------------------------------------------------------- P1: stage derived planes + fluxes
   for (int idx = tid; idx < T::H * T::W; idx += NT) {
@@ -125,33 +121,42 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       rho_b = a.bg.p[BG_RHO][ga]; e_b = a.bg.p[BG_E][ga];
       Bbx = a.bg.p[BG_BX][ga];    Bby = a.bg.p[BG_BY][ga];
     }
-    const double rho = rhot + rho_b;
+    const double rho = BG ? rho_b + rhot : rhot;
     const double rr = 1.0 / rho;
     const double vx = mx * rr, vy = my * rr;
-    const double b2h = 0.5 * (bx * bx + by * by);
-    const double cross = BG ? Bbx * bx + Bby * by : 0.0;
-    const double eps = et - 0.5 * (mx * vx + my * vy) - cross - b2h;
-    const double ptt = (gamma - 1.0) * eps + cross + b2h;
-    const double Bx = bx + Bbx, By = by + Bby;
+    const double b2h = 0.5 * fma(by, by, bx * bx);
+    const double cross = BG ? fma(Bby, by, Bbx * bx) : 0.0;
+    const double ke = 0.5 * fma(my, vy, mx * vx);
+    const double eps = BG ? ((et - ke) - cross) - b2h : (et - ke) - b2h;
+    const double ptt = BG ? fma(gm1, eps, cross + b2h) : fma(gm1, eps, b2h);
+    const double Bx = BG ? Bbx + bx : bx, By = BG ? Bby + by : by;
     const int s = r * T::P + c;
     pl(S_RHO)[s] = rho; pl(S_VX)[s] = vx; pl(S_VY)[s] = vy;
     pl(S_EPS)[s] = eps; pl(S_BX)[s] = bx; pl(S_BY)[s] = by;
     if (BG) { pl(S_RHOT)[s] = rhot; pl(S_BXT)[s] = Bx; pl(S_BYT)[s] = By; }
-    const double btv = bx * vx + by * vy;                       // b~ . v
-    const double Bbv = BG ? Bbx * vx + Bby * vy : 0.0;          // B_b . v
-    const double h = et + e_b + ptt;
-    // F_x(rho, mx, my, e, by)      (c-2; F_x(bx) == 0)
-    pl(S_CX0 + C_RHO)[s] = mx;
-    pl(S_CX0 + C_MX)[s] = mx * vx - bx * bx - 2.0 * bx * Bbx + ptt;
-    pl(S_CX0 + C_MY)[s] = my * vx - by * bx - by * Bbx - Bby * bx;
-    pl(S_CX0 + C_E)[s] = vx * h - bx * btv - bx * Bbv - Bbx * btv;
-    pl(S_CX0 + C_B)[s] = vx * By - Bx * vy;
-    // F_y(rho, mx, my, e, bx)      (F_y(by) == 0)
-    pl(S_CY0 + C_RHO)[s] = my;
-    pl(S_CY0 + C_MX)[s] = mx * vy - bx * by - bx * Bby - Bbx * by;
-    pl(S_CY0 + C_MY)[s] = my * vy - by * by - 2.0 * by * Bby + ptt;
-    pl(S_CY0 + C_E)[s] = vy * h - by * btv - by * Bbv - Bby * btv;
-    pl(S_CY0 + C_B)[s] = vy * Bx - By * vx;
+    const double btv = fma(by, vy, bx * vx);                      // b~ . v
+    const double Bbv = BG ? fma(Bby, vy, Bbx * vx) : 0.0;         // B_b . v
+    const double h = BG ? (et + e_b) + ptt : et + ptt;
+    // F_x(rho, mx, my, e, by)      (c-2; F_x(bx) == 0); background terms are exact zeros without one
+    pl(S_CX0 + C_RHO)[s] = rho * vx;
+    pl(S_CY0 + C_RHO)[s] = rho * vy;
+    if (BG) {
+      pl(S_CX0 + C_MX)[s] = ((fma(mx, vx, -(bx * bx)) - bx * Bbx) - Bbx * bx) + ptt;
+      pl(S_CX0 + C_MY)[s] = (fma(my, vx, -(by * bx)) - by * Bbx) - Bby * bx;
+      pl(S_CX0 + C_E)[s] = (fma(vx, h, -(bx * btv)) - bx * Bbv) - Bbx * btv;
+      pl(S_CY0 + C_MX)[s] = (fma(mx, vy, -(bx * by)) - bx * Bby) - Bbx * by;
+      pl(S_CY0 + C_MY)[s] = ((fma(my, vy, -(by * by)) - by * Bby) - Bby * by) + ptt;
+      pl(S_CY0 + C_E)[s] = (fma(vy, h, -(by * btv)) - by * Bbv) - Bby * btv;
+    } else {
+      pl(S_CX0 + C_MX)[s] = fma(mx, vx, -(bx * bx)) + ptt;
+      pl(S_CX0 + C_MY)[s] = fma(my, vx, -(by * bx));
+      pl(S_CX0 + C_E)[s] = fma(vx, h, -(bx * btv));
+      pl(S_CY0 + C_MX)[s] = fma(mx, vy, -(bx * by));
+      pl(S_CY0 + C_MY)[s] = fma(my, vy, -(by * by)) + ptt;
+      pl(S_CY0 + C_E)[s] = fma(vy, h, -(by * btv));
+    }
+    pl(S_CX0 + C_B)[s] = fma(vx, By, -(Bx * vy));                 // F_x(by)
+    pl(S_CY0 + C_B)[s] = fma(vy, Bx, -(By * vx));                 // F_y(bx)
   }
   __syncthreads();
 
@@ -196,11 +201,11 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       const int s = r * T::P + c;
       const double kv = 0.5 * (pl(S_KY0 + K_VX)[s - T::P] + pl(S_KY0 + K_VX)[s]);   // nubar_y(vx)/Delta_y
       const double kb = 0.5 * (pl(S_KY0 + K_B)[s - T::P] + pl(S_KY0 + K_B)[s]);     // nubar_y(bx~)/Delta_y
-      const double gm = 0.5 * pl(S_RHO)[s] * kv * (cd12(pl(S_VX) + s, T::P) * (1.0 / 12.0));  // G^{my,x}
-      const double gb = -kb * (cd12(pl(S_BX) + s, T::P) * (1.0 / 12.0));                     // G^{by,x}
+      const double gm = ((0.5 * pl(S_RHO)[s]) * kv) * (cd12(pl(S_VX) + s, T::P) * (1.0 / 12.0));  // G(my;x)
+      const double gb = -(kb * (cd12(pl(S_BX) + s, T::P) * (1.0 / 12.0)));                        // G(by;x)
       pl(S_CX0 + C_MY)[s] -= gm;
       pl(S_CX0 + C_B)[s] -= gb;
-      pl(S_CX0 + C_E)[s] -= pl(S_VY)[s] * gm + pl(SBY)[s] * gb;
+      pl(S_CX0 + C_E)[s] -= fma(pl(S_VY)[s], gm, pl(SBY)[s] * gb);
     }
     // G_y (needs x-derivatives): staged rows 1 .. TH+4, tile columns
     for (int idx = tid; idx < (TH + 4) * TW; idx += NT) {
@@ -208,11 +213,11 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       const int s = r * T::P + c;
       const double kv = 0.5 * (pl(S_KX0 + K_VY)[s - 1] + pl(S_KX0 + K_VY)[s]);      // nubar_x(vy)/Delta_x
       const double kb = 0.5 * (pl(S_KX0 + K_B)[s - 1] + pl(S_KX0 + K_B)[s]);        // nubar_x(by~)/Delta_x
-      const double gm = 0.5 * pl(S_RHO)[s] * kv * (cd12(pl(S_VY) + s, 1) * (1.0 / 12.0));     // G^{mx,y}
-      const double gb = -kb * (cd12(pl(S_BY) + s, 1) * (1.0 / 12.0));                        // G^{bx,y}
+      const double gm = ((0.5 * pl(S_RHO)[s]) * kv) * (cd12(pl(S_VY) + s, 1) * (1.0 / 12.0));     // G(mx;y)
+      const double gb = -(kb * (cd12(pl(S_BY) + s, 1) * (1.0 / 12.0)));                           // G(bx;y)
       pl(S_CY0 + C_MX)[s] -= gm;
       pl(S_CY0 + C_B)[s] -= gb;
-      pl(S_CY0 + C_E)[s] -= pl(S_VX)[s] * gm + pl(SBX)[s] * gb;
+      pl(S_CY0 + C_E)[s] -= fma(pl(S_VX)[s], gm, pl(SBX)[s] * gb);
     }
     __syncthreads();
   }
@@ -228,13 +233,13 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
     if (i >= g.nx || j >= g.ny) continue;
     const int s = (ty + NG) * T::P + (tx + NG);
     double R[NF];
-    // central differences of the (mixed-flux-corrected) fluxes
-    R[F_RHO] = -(cd12(pl(S_CX0 + C_RHO) + s, 1) * idx_ + cd12(pl(S_CY0 + C_RHO) + s, T::P) * idy_) * (1.0 / 12.0);
-    R[F_MX] = -(cd12(pl(S_CX0 + C_MX) + s, 1) * idx_ + cd12(pl(S_CY0 + C_MX) + s, T::P) * idy_) * (1.0 / 12.0);
-    R[F_MY] = -(cd12(pl(S_CX0 + C_MY) + s, 1) * idx_ + cd12(pl(S_CY0 + C_MY) + s, T::P) * idy_) * (1.0 / 12.0);
-    R[F_E] = -(cd12(pl(S_CX0 + C_E) + s, 1) * idx_ + cd12(pl(S_CY0 + C_E) + s, T::P) * idy_) * (1.0 / 12.0);
-    R[F_BX] = -(cd12(pl(S_CY0 + C_B) + s, T::P) * idy_) * (1.0 / 12.0);
-    R[F_BY] = -(cd12(pl(S_CX0 + C_B) + s, 1) * idx_) * (1.0 / 12.0);
+    // central differences of the (mixed-flux-corrected) fluxes:  -(d^c_x C_x + d^c_y C_y)
+    R[F_RHO] = fma(cd12(pl(S_CX0 + C_RHO) + s, 1), idx_, cd12(pl(S_CY0 + C_RHO) + s, T::P) * idy_) * (-1.0 / 12.0);
+    R[F_MX] = fma(cd12(pl(S_CX0 + C_MX) + s, 1), idx_, cd12(pl(S_CY0 + C_MX) + s, T::P) * idy_) * (-1.0 / 12.0);
+    R[F_MY] = fma(cd12(pl(S_CX0 + C_MY) + s, 1), idx_, cd12(pl(S_CY0 + C_MY) + s, T::P) * idy_) * (-1.0 / 12.0);
+    R[F_E] = fma(cd12(pl(S_CX0 + C_E) + s, 1), idx_, cd12(pl(S_CY0 + C_E) + s, T::P) * idy_) * (-1.0 / 12.0);
+    R[F_BX] = (cd12(pl(S_CY0 + C_B) + s, T::P) * idy_) * (-1.0 / 12.0);          // F_x(bx) == 0
+    R[F_BY] = fma(cd12(pl(S_CX0 + C_B) + s, 1), idx_, 0.0) * (-1.0 / 12.0);       // F_y(by) == 0
 
     const long long ga = cell_addr(g, i, j);
     double rho_b = 0.0, e_b = 0.0, Bbx = 0.0, Bby = 0.0;
@@ -242,13 +247,15 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       rho_b = a.bg.p[BG_RHO][ga]; e_b = a.bg.p[BG_E][ga];
       Bbx = a.bg.p[BG_BX][ga];    Bby = a.bg.p[BG_BY][ga];
       // energy source S_e = -p_tb div v + B_b B_b : grad v      (c-2)
-      const double bb2h = 0.5 * (Bbx * Bbx + Bby * Bby);
-      const double ptb = (gamma - 1.0) * (e_b - bb2h) + bb2h;
-      const double dxvx = cd12(pl(S_VX) + s, 1) * idx_ * (1.0 / 12.0);
-      const double dyvx = cd12(pl(S_VX) + s, T::P) * idy_ * (1.0 / 12.0);
-      const double dxvy = cd12(pl(S_VY) + s, 1) * idx_ * (1.0 / 12.0);
-      const double dyvy = cd12(pl(S_VY) + s, T::P) * idy_ * (1.0 / 12.0);
-      R[F_E] += -ptb * (dxvx + dyvy) + (Bbx * Bbx * dxvx + Bbx * Bby * (dxvy + dyvx) + Bby * Bby * dyvy);
+      const double bb2h = 0.5 * fma(Bby, Bby, Bbx * Bbx);
+      const double ptb = fma(gm1, e_b - bb2h, bb2h);
+      const double dxvx = (cd12(pl(S_VX) + s, 1) * idx_) * (1.0 / 12.0);
+      const double dyvx = (cd12(pl(S_VX) + s, T::P) * idy_) * (1.0 / 12.0);
+      const double dxvy = (cd12(pl(S_VY) + s, 1) * idx_) * (1.0 / 12.0);
+      const double dyvy = (cd12(pl(S_VY) + s, T::P) * idy_) * (1.0 / 12.0);
+      const double S = fma(-ptb, dxvx + dyvy,
+                           fma(Bby * Bby, dyvy, fma(Bbx * Bby, dxvy + dyvx, (Bbx * Bbx) * dxvx)));
+      R[F_E] = R[F_E] + S;
     }
 
     if (HD) {
@@ -261,48 +268,55 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
           const int sa = s - 1 + side, sb = sa + 1;
           const double rbar = 0.5 * (pl(S_RHO)[sa] + pl(S_RHO)[sb]);
           const double p_rho = pl(S_KX0 + K_RHO)[sa] * (pl(SRT)[sb] - pl(SRT)[sa]);
-          const double p_mx = rbar * pl(S_KX0 + K_VX)[sa] * (pl(S_VX)[sb] - pl(S_VX)[sa]);
-          const double p_my = 0.5 * rbar * pl(S_KX0 + K_VY)[sa] * (pl(S_VY)[sb] - pl(S_VY)[sa]);
+          const double p_mx = (rbar * pl(S_KX0 + K_VX)[sa]) * (pl(S_VX)[sb] - pl(S_VX)[sa]);
+          const double p_my = ((0.5 * rbar) * pl(S_KX0 + K_VY)[sa]) * (pl(S_VY)[sb] - pl(S_VY)[sa]);
           const double p_eps = pl(S_KX0 + K_EPS)[sa] * (pl(S_EPS)[sb] - pl(S_EPS)[sa]);
           const double p_b = pl(S_KX0 + K_B)[sa] * (pl(S_BY)[sb] - pl(S_BY)[sa]);
           fx[side][C_RHO] = p_rho; fx[side][C_MX] = p_mx; fx[side][C_MY] = p_my; fx[side][C_B] = p_b;
-          fx[side][C_E] = p_eps + 0.5 * (pl(S_VX)[sa] + pl(S_VX)[sb]) * p_mx +
-                          0.5 * (pl(S_VY)[sa] + pl(S_VY)[sb]) * p_my +
-                          0.5 * (pl(SBY)[sa] + pl(SBY)[sb]) * p_b;
+          fx[side][C_E] = fma(0.5 * (pl(SBY)[sa] + pl(SBY)[sb]), p_b,
+                              fma(0.5 * (pl(S_VY)[sa] + pl(S_VY)[sb]), p_my,
+                                  fma(0.5 * (pl(S_VX)[sa] + pl(S_VX)[sb]), p_mx, p_eps)));
         }
         {
           const int sa = s + (side - 1) * T::P, sb = sa + T::P;
           const double rbar = 0.5 * (pl(S_RHO)[sa] + pl(S_RHO)[sb]);
           const double p_rho = pl(S_KY0 + K_RHO)[sa] * (pl(SRT)[sb] - pl(SRT)[sa]);
-          const double p_mx = 0.5 * rbar * pl(S_KY0 + K_VX)[sa] * (pl(S_VX)[sb] - pl(S_VX)[sa]);
-          const double p_my = rbar * pl(S_KY0 + K_VY)[sa] * (pl(S_VY)[sb] - pl(S_VY)[sa]);
+          const double p_mx = ((0.5 * rbar) * pl(S_KY0 + K_VX)[sa]) * (pl(S_VX)[sb] - pl(S_VX)[sa]);
+          const double p_my = (rbar * pl(S_KY0 + K_VY)[sa]) * (pl(S_VY)[sb] - pl(S_VY)[sa]);
           const double p_eps = pl(S_KY0 + K_EPS)[sa] * (pl(S_EPS)[sb] - pl(S_EPS)[sa]);
           const double p_b = pl(S_KY0 + K_B)[sa] * (pl(S_BX)[sb] - pl(S_BX)[sa]);
           fy[side][C_RHO] = p_rho; fy[side][C_MX] = p_mx; fy[side][C_MY] = p_my; fy[side][C_B] = p_b;
-          fy[side][C_E] = p_eps + 0.5 * (pl(S_VX)[sa] + pl(S_VX)[sb]) * p_mx +
-                          0.5 * (pl(S_VY)[sa] + pl(S_VY)[sb]) * p_my +
-                          0.5 * (pl(SBX)[sa] + pl(SBX)[sb]) * p_b;
+          fy[side][C_E] = fma(0.5 * (pl(SBX)[sa] + pl(SBX)[sb]), p_b,
+                              fma(0.5 * (pl(S_VY)[sa] + pl(S_VY)[sb]), p_my,
+                                  fma(0.5 * (pl(S_VX)[sa] + pl(S_VX)[sb]), p_mx, p_eps)));
         }
       }
-      R[F_RHO] += (fx[1][C_RHO] - fx[0][C_RHO]) * idx_ + (fy[1][C_RHO] - fy[0][C_RHO]) * idy_;
-      R[F_MX] += (fx[1][C_MX] - fx[0][C_MX]) * idx_ + (fy[1][C_MX] - fy[0][C_MX]) * idy_;
-      R[F_MY] += (fx[1][C_MY] - fx[0][C_MY]) * idx_ + (fy[1][C_MY] - fy[0][C_MY]) * idy_;
-      R[F_E] += (fx[1][C_E] - fx[0][C_E]) * idx_ + (fy[1][C_E] - fy[0][C_E]) * idy_;
-      R[F_BX] += (fy[1][C_B] - fy[0][C_B]) * idy_;
-      R[F_BY] += (fx[1][C_B] - fx[0][C_B]) * idx_;
+      R[F_RHO] = fma(fx[1][C_RHO] - fx[0][C_RHO], idx_, R[F_RHO]);
+      R[F_MX] = fma(fx[1][C_MX] - fx[0][C_MX], idx_, R[F_MX]);
+      R[F_MY] = fma(fx[1][C_MY] - fx[0][C_MY], idx_, R[F_MY]);
+      R[F_E] = fma(fx[1][C_E] - fx[0][C_E], idx_, R[F_E]);
+      R[F_BY] = fma(fx[1][C_B] - fx[0][C_B], idx_, R[F_BY]);
+      R[F_RHO] = fma(fy[1][C_RHO] - fy[0][C_RHO], idy_, R[F_RHO]);
+      R[F_MX] = fma(fy[1][C_MX] - fy[0][C_MX], idy_, R[F_MX]);
+      R[F_MY] = fma(fy[1][C_MY] - fy[0][C_MY], idy_, R[F_MY]);
+      R[F_E] = fma(fy[1][C_E] - fy[0][C_E], idy_, R[F_E]);
+      R[F_BX] = fma(fy[1][C_B] - fy[0][C_B], idy_, R[F_BX]);
     }
 
     // RK combine (c-6) and write
     double o[NF];
     if (a.combine == COMBINE_FINAL) {
 #pragma unroll
-      for (int f = 0; f < NF; ++f) o[f] = a.acc_in.p[f][ga] + a.in.p[f][ga] * (1.0 / 3.0) + cdt * R[f];
+      for (int f = 0; f < NF; ++f) {
+        const double w3 = a.in.p[f][ga];
+        o[f] = fma(cdt, R[f], fma(fma(-2.0, w3, a.acc_in.p[f][ga]), 1.0 / 3.0, w3));
+      }
     } else {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         const double b = a.base.p[f][ga];
-        o[f] = b + cdt * R[f];
-        if (a.combine == COMBINE_ACC) a.acc_out.p[f][ga] = (a.in.p[f][ga] + 2.0 * o[f] - b) * (1.0 / 3.0);
+        o[f] = fma(cdt, R[f], b);
+        if (a.combine == COMBINE_ACC) a.acc_out.p[f][ga] = fma(2.0, o[f], a.in.p[f][ga] - b);
       }
     }
 #pragma unroll
@@ -310,8 +324,11 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
 
     if (a.ws_mode != WS_NONE) {
       double w4[4];
-      cell_wavespeeds(o[F_RHO] + rho_b, o[F_MX], o[F_MY], o[F_E] + e_b, o[F_BX] + Bbx, o[F_BY] + Bby, gamma,
-                      a.ws_mode == WS_FULL, w4);
+      if (BG)
+        cell_wavespeeds(rho_b + o[F_RHO], o[F_MX], o[F_MY], e_b + o[F_E], Bbx + o[F_BX], Bby + o[F_BY], gamma,
+                        a.ws_mode == WS_FULL, w4);
+      else
+        cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, a.ws_mode == WS_FULL, w4);
 #pragma unroll
       for (int k = 0; k < 4; ++k) wsmax[k] = fmax(wsmax[k], w4[k]);
     }

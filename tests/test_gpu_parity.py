@@ -48,10 +48,17 @@ def cpu_run(oracle_mod, w, bc, gamma, steps, cfl=0.3, bg=None, threads=8, **para
     return out, t, ws
 
 
-def check(a, ta, wsa, b, tb, wsb, tol=TOL):
+def check(a, ta, wsa, b, tb, wsb, tol=TOL, exact=True):
+    """Bar: rel L2 <= 1e-10 per field.  Because both sides implement the same IEEE operation sequence
+    (the arithmetic contract) the results are in fact bit-identical, and `exact`
+    asserts that too: the scheme amplifies any rounding-level mismatch to ~1e-8 within 40 steps, so an
+    exact match is the only robust way to hold 1e-10 at the configured step counts."""
     err = si.rel_l2(a, b)
     assert np.isfinite(a).all()
     assert (err <= tol).all(), err
+    if exact:
+        assert np.array_equal(a, b), (err, np.abs(a - b).max())
+        assert ta == tb and list(wsa) == list(wsb)
     assert abs(ta[0] - tb[0]) <= 1e-12 * abs(tb[0]) and abs(ta[1] - tb[1]) <= 1e-12 * abs(tb[1])
     assert np.allclose(wsa, wsb, rtol=1e-11, atol=0)
     return err
