@@ -33,7 +33,7 @@ int fail(int code, const std::string& msg) {
   } while (0)
 
 // Tile / launch configuration of the fused stage kernel.
-constexpr int TW = 32, TH = 16, NT = 256;
+constexpr int TW = 32, TH = 16, NT = 512;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -133,7 +133,7 @@ int launch_wavespeeds(smaug_ctx* c, const Planes6& w, int set) {
 template <bool BG, bool HD>
 int launch_stage_t(smaug_ctx* c, const StageArgs& a) {
   static bool configured = false;
-  constexpr size_t smem = stage_smem_bytes<TW, TH, BG>();
+  constexpr size_t smem = Tile<TW, TH, BG>::BYTES;
   auto kern = stage_kernel<TW, TH, NT, BG, HD>;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -441,7 +441,7 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (int rc = check_ctx(c)) return rc;
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
   out[0] = TW; out[1] = TH; out[2] = NT;
-  out[3] = (int)(c->has_bg ? stage_smem_bytes<TW, TH, true>() : stage_smem_bytes<TW, TH, false>());
+  out[3] = (int)(c->has_bg ? Tile<TW, TH, true>::BYTES : Tile<TW, TH, false>::BYTES);
   out[4] = c->last_ctas;
   return SMAUG_OK;
 }

@@ -4,14 +4,17 @@
 // planes; the flux divergence (c-2, c-3), the hyperdiffusion coefficients and fluxes (c-5), the energy
 // source (c-2), the RK combine (c-6) and the wave-speed maxima of the state just written (c-4) are all
 // computed in this one pass -- the state is read once and written once per stage.
+// Every value follows the arithmetic contract of DESIGN.md section 4 (explicit fma, -fmad=false), so the
+// result is bit-identical to the oracle's.
 //
 // Phases (separated by __syncthreads):
-//   P1  load w (+ background) for tile + halo 3, compute rho, 1/rho, v, eps~, p~_t, store the six HD
-//       scalars (+ totals when a background exists) and the cell-centred fluxes F_x, F_y in smem
+//   P1  load w (+ background) for tile + halo 3, compute rho, 1/rho, v, eps~, p~_t; store the six HD
+//       scalars (+ totals when a background exists) and the cell-centred fluxes F_x, F_y where needed
 //   P2  hyperviscosity ratios kappa = c_u v_t M3/M1 at the x- and y-interfaces, computed in register runs
-//       of R interfaces per thread (sliding |D1| / |D3| windows, no redundant differences)
+//       (one thread slides the |D1| / |D3| windows along R consecutive interfaces: no redundant differences)
 //   P3  cell-centred mixed (cross) fluxes G and their energy companions, folded into F_x, F_y
-//   P4  per cell: interface-flux differences, central differences of (F - G), source, RK combine, write,
+//   P3b interface (diffusive) fluxes Phi, once per interface, written over the kappa planes
+//   P4  per cell: central differences of (F - G), interface-flux differences, source, RK combine, write,
 //       wave-speed maxima -> warp shuffles -> one atomicMax pass per CTA
 #pragma once
 #include "smaug_aux_kernels.cuh"
@@ -45,54 +48,67 @@ struct StageArgs {
   int ws_mode;
 };
 
-template <int TW_, int TH_>
+constexpr int odd_up(int v) { return (v % 2 == 0) ? v + 1 : v; }   // odd pitch: conflict-free columns
+
+// Shared-memory layout of one tile.  Staged cell (r, c), r in [0, TH+6), c in [0, TW+6), is interior
+// cell (x0 + c - 3, y0 + r - 3).
+template <int TW_, int TH_, bool BG>
 struct Tile {
   static constexpr int TW = TW_, TH = TH_;
-  static constexpr int W = TW + 2 * NG, H = TH + 2 * NG;   // staged extent
-  static constexpr int P = (W % 2 == 0) ? W + 1 : W;       // odd row pitch -> conflict-free column access
-  static constexpr int PLANE = P * H;
+  static constexpr int W = TW + 2 * NG, H = TH + 2 * NG;
+  // U planes: H x W, all staged cells
+  static constexpr int PU = odd_up(W), U_PLANE = PU * H, NU = BG ? 9 : 6;
+  // KX planes (kappa, later Phi, at x-interfaces (c | c+1), c = 2 .. TW+2): rows r = 1 .. TH+4
+  static constexpr int PKX = odd_up(TW + 1), KX_PLANE = PKX * (TH + 4);
+  // KY planes (y-interfaces (r | r+1), r = 2 .. TH+2): columns c = 1 .. TW+4
+  static constexpr int PKY = odd_up(TW + 4), KY_PLANE = PKY * (TH + 1);
+  // CX planes (F_x - G_x): tile rows, columns c = 1 .. TW+4;   CY planes: rows r = 1 .. TH+4, tile columns
+  static constexpr int PCX = odd_up(TW + 4), CX_PLANE = PCX * TH;
+  static constexpr int PCY = odd_up(TW), CY_PLANE = PCY * (TH + 4);
+  static constexpr int OFF_U = 0;
+  static constexpr int OFF_KX = OFF_U + NU * U_PLANE;
+  static constexpr int OFF_KY = OFF_KX + 5 * KX_PLANE;
+  static constexpr int OFF_CX = OFF_KY + 5 * KY_PLANE;
+  static constexpr int OFF_CY = OFF_CX + 5 * CX_PLANE;
+  static constexpr int OFF_RED = OFF_CY + 5 * CY_PLANE;
+  static constexpr int TOTAL = OFF_RED + 4 * 32;
+  static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
+  __device__ static int u(int r, int c) { return r * PU + c; }
+  __device__ static int kx(int r, int c) { return (r - 1) * PKX + (c - 2); }
+  __device__ static int ky(int r, int c) { return (r - 2) * PKY + (c - 1); }
+  __device__ static int cx(int r, int c) { return (r - NG) * PCX + (c - 1); }
+  __device__ static int cy(int r, int c) { return (r - 1) * PCY + (c - NG); }
 };
 
-// plane indices inside the dynamic shared memory
-enum {
-  S_RHO = 0,  // total rho
-  S_VX, S_VY, S_EPS, S_BX, S_BY,      // HD scalars v, eps~, b~   (rho~ = S_RHO when there is no background)
-  S_KX0,                              // 5 planes: kappa at x-interfaces for rho~, vx, vy, eps~, by~
-  S_KY0 = S_KX0 + 5,                  // 5 planes: kappa at y-interfaces for rho~, vx, vy, eps~, bx~
-  S_CX0 = S_KY0 + 5,                  // 5 planes: F_x - G_x for rho, mx, my, e, by
-  S_CY0 = S_CX0 + 5,                  // 5 planes: F_y - G_y for rho, mx, my, e, bx
-  S_NOBG_END = S_CY0 + 5,
-  S_RHOT = S_NOBG_END,                // background only: rho~ (perturbed), total Bx, total By
-  S_BXT, S_BYT,
-  S_BG_END
-};
-enum { K_RHO = 0, K_VX = 1, K_VY = 2, K_EPS = 3, K_B = 4 };
+enum { U_RHO = 0, U_VX, U_VY, U_EPS, U_BX, U_BY, U_RHOT, U_BXT, U_BYT };   // last three: background only
+enum { K_RHO = 0, K_VX = 1, K_VY = 2, K_EPS = 3, K_B = 4 };                 // kappa families; Phi components
 enum { C_RHO = 0, C_MX = 1, C_MY = 2, C_E = 3, C_B = 4 };
 
-template <int TW, int TH, bool BG>
-constexpr size_t stage_smem_bytes() {
-  return (size_t)(BG ? S_BG_END : S_NOBG_END) * Tile<TW, TH>::PLANE * sizeof(double) + 4 * 32 * sizeof(double);
-}
+// max of two non-negative doubles: one DSETP + two selects (fmax() costs ~7 instructions on sm_100a
+// because of its NaN-quieting semantics).  max is exact, so any evaluation order is bit-safe.
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
-// kappa = coef * (M3 / M1) for R consecutive interfaces of one line (c-5).  u points at the cell left of
-// the first interface; cells u[-2*s] .. u[(R+2)*s] are read.  Interface k (0..n-1) is written to out[k*os].
+// kappa = cv * (M3 / M1) for n <= R consecutive interfaces of one line (c-5).  u points at the cell left of
+// the first interface (interface k lies between cells k and k+1); cells -2 .. R+2 are read with stride s.
+// Sliding windows: D1_m = u_{m+1} - u_m;  D3_m = 3 D1_m - (u_{m+2} - u_{m-1});  M3 over m-1..m+1, M1 over m-2..m+2.
 template <int R>
 __device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, double cv, double* out,
                                           int os, int n) {
-  double uu[R + 5];   // cells -2 .. R+2
+  double uu[R + 5];
 #pragma unroll
   for (int k = 0; k < R + 5; ++k) uu[k] = u[(k - 2) * s];
-  double d1[R + 4];   // signed D1 at interfaces -2 .. R+1:  D1_m = u_{m+1} - u_m
+  double d1[R + 4];
 #pragma unroll
-  for (int k = 0; k < R + 4; ++k) d1[k] = uu[k + 1] - uu[k];
-  double d3[R + 2];   // |D3| at interfaces -1 .. R:  D3_m = 3 D1_m - (u_{m+2} - u_{m-1})
+  for (int k = 0; k < R + 4; ++k) d1[k] = uu[k + 1] - uu[k];                       // interface k-2
+  double d3[R + 2];
 #pragma unroll
-  for (int k = 0; k < R + 2; ++k) d3[k] = fabs(fma(3.0, d1[k + 1], -(uu[k + 3] - uu[k])));
+  for (int k = 0; k < R + 2; ++k) d3[k] = fabs(fma(3.0, d1[k + 1], -(uu[k + 3] - uu[k])));   // interface k-1
+#pragma unroll
+  for (int k = 0; k < R + 4; ++k) d1[k] = fabs(d1[k]);
 #pragma unroll
   for (int k = 0; k < R; ++k) {
-    const double m3 = fmax(fmax(d3[k], d3[k + 1]), d3[k + 2]);
-    const double m1 = fmax(fmax(fmax(fabs(d1[k]), fabs(d1[k + 1])), fmax(fabs(d1[k + 2]), fabs(d1[k + 3]))),
-                           fabs(d1[k + 4]));
+    const double m3 = dmax(dmax(d3[k], d3[k + 1]), d3[k + 2]);
+    const double m1 = dmax(dmax(dmax(d1[k], d1[k + 1]), dmax(d1[k + 2], d1[k + 3])), d1[k + 4]);
     const double r = m1 > 0.0 ? cv * (m3 / m1) : 0.0;
     if (k < n) out[k * os] = r;
   }
@@ -100,10 +116,14 @@ __device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, d
 
 template <int TW, int TH, int NT, bool BG, bool HD>
 __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
-  using T = Tile<TW, TH>;
+  using T = Tile<TW, TH, BG>;
   extern __shared__ double smem[];
-  double* const red_sh = smem + (size_t)(BG ? S_BG_END : S_NOBG_END) * T::PLANE;
-  auto pl = [&](int k) { return smem + (size_t)k * T::PLANE; };
+  double* const U = smem + T::OFF_U;
+  double* const KX = smem + T::OFF_KX;
+  double* const KY = smem + T::OFF_KY;
+  double* const CX = smem + T::OFF_CX;
+  double* const CY = smem + T::OFF_CY;
+  double* const red_sh = smem + T::OFF_RED;
   const Grid& g = a.g;
   const int tid = threadIdx.x;
   const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;   // interior coordinates of the tile origin
@@ -130,94 +150,177 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
     const double eps = BG ? ((et - ke) - cross) - b2h : (et - ke) - b2h;
     const double ptt = BG ? fma(gm1, eps, cross + b2h) : fma(gm1, eps, b2h);
     const double Bx = BG ? Bbx + bx : bx, By = BG ? Bby + by : by;
-    const int s = r * T::P + c;
-    pl(S_RHO)[s] = rho; pl(S_VX)[s] = vx; pl(S_VY)[s] = vy;
-    pl(S_EPS)[s] = eps; pl(S_BX)[s] = bx; pl(S_BY)[s] = by;
-    if (BG) { pl(S_RHOT)[s] = rhot; pl(S_BXT)[s] = Bx; pl(S_BYT)[s] = By; }
-    const double btv = fma(by, vy, bx * vx);                      // b~ . v
-    const double Bbv = BG ? fma(Bby, vy, Bbx * vx) : 0.0;         // B_b . v
-    const double h = BG ? (et + e_b) + ptt : et + ptt;
-    // F_x(rho, mx, my, e, by)      (c-2; F_x(bx) == 0); background terms are exact zeros without one
-    pl(S_CX0 + C_RHO)[s] = rho * vx;
-    pl(S_CY0 + C_RHO)[s] = rho * vy;
+    const int s = T::u(r, c);
+    U[U_RHO * T::U_PLANE + s] = rho; U[U_VX * T::U_PLANE + s] = vx; U[U_VY * T::U_PLANE + s] = vy;
+    U[U_EPS * T::U_PLANE + s] = eps; U[U_BX * T::U_PLANE + s] = bx; U[U_BY * T::U_PLANE + s] = by;
     if (BG) {
-      pl(S_CX0 + C_MX)[s] = ((fma(mx, vx, -(bx * bx)) - bx * Bbx) - Bbx * bx) + ptt;
-      pl(S_CX0 + C_MY)[s] = (fma(my, vx, -(by * bx)) - by * Bbx) - Bby * bx;
-      pl(S_CX0 + C_E)[s] = (fma(vx, h, -(bx * btv)) - bx * Bbv) - Bbx * btv;
-      pl(S_CY0 + C_MX)[s] = (fma(mx, vy, -(bx * by)) - bx * Bby) - Bbx * by;
-      pl(S_CY0 + C_MY)[s] = ((fma(my, vy, -(by * by)) - by * Bby) - Bby * by) + ptt;
-      pl(S_CY0 + C_E)[s] = (fma(vy, h, -(by * btv)) - by * Bbv) - Bby * btv;
-    } else {
-      pl(S_CX0 + C_MX)[s] = fma(mx, vx, -(bx * bx)) + ptt;
-      pl(S_CX0 + C_MY)[s] = fma(my, vx, -(by * bx));
-      pl(S_CX0 + C_E)[s] = fma(vx, h, -(bx * btv));
-      pl(S_CY0 + C_MX)[s] = fma(mx, vy, -(bx * by));
-      pl(S_CY0 + C_MY)[s] = fma(my, vy, -(by * by)) + ptt;
-      pl(S_CY0 + C_E)[s] = fma(vy, h, -(by * btv));
+      U[U_RHOT * T::U_PLANE + s] = rhot; U[U_BXT * T::U_PLANE + s] = Bx; U[U_BYT * T::U_PLANE + s] = By;
     }
-    pl(S_CX0 + C_B)[s] = fma(vx, By, -(Bx * vy));                 // F_x(by)
-    pl(S_CY0 + C_B)[s] = fma(vy, Bx, -(By * vx));                 // F_y(bx)
+    const bool in_rows = r >= NG && r < NG + TH, in_cols = c >= NG && c < NG + TW;
+    const bool need_x = in_rows && c >= 1 && c <= TW + 4, need_y = in_cols && r >= 1 && r <= TH + 4;
+    if (need_x || need_y) {
+      const double btv = fma(by, vy, bx * vx);                      // b~ . v
+      const double Bbv = BG ? fma(Bby, vy, Bbx * vx) : 0.0;         // B_b . v
+      const double h = BG ? (et + e_b) + ptt : et + ptt;
+      if (need_x) {   // F_x(rho, mx, my, e, by)   (c-2; F_x(bx) == 0)
+        double* cxp = CX + T::cx(r, c);
+        cxp[C_RHO * T::CX_PLANE] = rho * vx;
+        if (BG) {
+          cxp[C_MX * T::CX_PLANE] = ((fma(mx, vx, -(bx * bx)) - bx * Bbx) - Bbx * bx) + ptt;
+          cxp[C_MY * T::CX_PLANE] = (fma(my, vx, -(by * bx)) - by * Bbx) - Bby * bx;
+          cxp[C_E * T::CX_PLANE] = (fma(vx, h, -(bx * btv)) - bx * Bbv) - Bbx * btv;
+        } else {
+          cxp[C_MX * T::CX_PLANE] = fma(mx, vx, -(bx * bx)) + ptt;
+          cxp[C_MY * T::CX_PLANE] = fma(my, vx, -(by * bx));
+          cxp[C_E * T::CX_PLANE] = fma(vx, h, -(bx * btv));
+        }
+        cxp[C_B * T::CX_PLANE] = fma(vx, By, -(Bx * vy));
+      }
+      if (need_y) {   // F_y(rho, mx, my, e, bx)   (F_y(by) == 0)
+        double* cyp = CY + T::cy(r, c);
+        cyp[C_RHO * T::CY_PLANE] = rho * vy;
+        if (BG) {
+          cyp[C_MX * T::CY_PLANE] = (fma(mx, vy, -(bx * by)) - bx * Bby) - Bbx * by;
+          cyp[C_MY * T::CY_PLANE] = ((fma(my, vy, -(by * by)) - by * Bby) - Bby * by) + ptt;
+          cyp[C_E * T::CY_PLANE] = (fma(vy, h, -(by * btv)) - by * Bbv) - Bby * btv;
+        } else {
+          cyp[C_MX * T::CY_PLANE] = fma(mx, vy, -(bx * by));
+          cyp[C_MY * T::CY_PLANE] = fma(my, vy, -(by * by)) + ptt;
+          cyp[C_E * T::CY_PLANE] = fma(vy, h, -(by * btv));
+        }
+        cyp[C_B * T::CY_PLANE] = fma(vy, Bx, -(By * vx));
+      }
+    }
   }
   __syncthreads();
 
+  constexpr int URT = BG ? U_RHOT : U_RHO, UBXT = BG ? U_BXT : U_BX, UBYT = BG ? U_BYT : U_BY;
   if (HD) {
     // v_t = sqrt(max a^2) + sqrt(max b^2) of the input state (c-5)
     const double vt = sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][2])) +
                       sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][3]));
-    const double coef[5] = {a.prm.c_rho * vt, a.prm.c_mom * vt, a.prm.c_mom * vt, a.prm.c_e * vt,
-                            a.prm.c_b * vt};
     // ------------------------------------------------------------ P2: kappa at interfaces, register runs
-    // x-interfaces (c | c+1), c = 2 .. TW+2, on staged rows 1 .. TH+4; runs of RX interfaces.
+    // x-interfaces (c | c+1), c = 2 .. TW+2.  Families rho~, vx, eps~ on tile rows; vy, by~ on rows 1 .. TH+4.
     {
-      constexpr int RX = 11, NRUN = (TW + 1 + RX - 1) / RX, ROWS = TH + 4;
-      const int usrc[5] = {BG ? S_RHOT : S_RHO, S_VX, S_VY, S_EPS, S_BY};
-      for (int it = tid; it < 5 * NRUN * ROWS; it += NT) {
-        const int f = it / (NRUN * ROWS), rem = it - f * (NRUN * ROWS);
-        const int run = rem / ROWS, r = 1 + (rem - run * ROWS);
+      constexpr int RX = 11, NRUN = (TW + 1 + RX - 1) / RX;
+      constexpr int N_TILE = 3 * TH * NRUN, N_WIDE = 2 * (TH + 4) * NRUN;
+      for (int it = tid; it < N_TILE + N_WIDE; it += NT) {
+        int f, run, r;
+        if (it < N_TILE) {
+          const int q = it / TH;
+          r = NG + (it - q * TH);
+          f = q / NRUN; run = q - f * NRUN;
+          f = f == 0 ? K_RHO : (f == 1 ? K_VX : K_EPS);
+        } else {
+          const int it2 = it - N_TILE, q = it2 / (TH + 4);
+          r = 1 + (it2 - q * (TH + 4));
+          f = q / NRUN; run = q - f * NRUN;
+          f = f == 0 ? K_VY : K_B;
+        }
+        const int up = f == K_RHO ? URT : (f == K_VX ? U_VX : (f == K_VY ? U_VY : (f == K_EPS ? U_EPS : U_BY)));
+        const double cf = f == K_RHO ? a.prm.c_rho : (f == K_EPS ? a.prm.c_e : (f == K_B ? a.prm.c_b : a.prm.c_mom));
         const int c0 = 2 + run * RX;
-        kappa_run<RX>(pl(usrc[f]) + r * T::P + c0, 1, coef[f], pl(S_KX0 + f) + r * T::P + c0, 1,
+        kappa_run<RX>(U + up * T::U_PLANE + T::u(r, c0), 1, cf * vt, KX + f * T::KX_PLANE + T::kx(r, c0), 1,
                       min(RX, TW + 3 - c0));
       }
     }
-    // y-interfaces (r | r+1), r = 2 .. TH+2, on staged columns 1 .. TW+4; runs of RY interfaces.
+    // y-interfaces (r | r+1), r = 2 .. TH+2.  Families rho~, vy, eps~ on tile columns; vx, bx~ on columns 1 .. TW+4.
     {
-      constexpr int RY = 9, NRUN = (TH + 1 + RY - 1) / RY, COLS = TW + 4;
-      const int usrc[5] = {BG ? S_RHOT : S_RHO, S_VX, S_VY, S_EPS, S_BX};
-      for (int it = tid; it < 5 * NRUN * COLS; it += NT) {
-        const int f = it / (NRUN * COLS), rem = it - f * (NRUN * COLS);
-        const int run = rem / COLS, c = 1 + (rem - run * COLS);
+      constexpr int RY = 9, NRUN = (TH + 1 + RY - 1) / RY;
+      constexpr int N_TILE = 3 * TW * NRUN, N_WIDE = 2 * (TW + 4) * NRUN;
+      for (int it = tid; it < N_TILE + N_WIDE; it += NT) {
+        int f, run, c;
+        if (it < N_TILE) {
+          const int q = it / TW;
+          c = NG + (it - q * TW);
+          f = q / NRUN; run = q - f * NRUN;
+          f = f == 0 ? K_RHO : (f == 1 ? K_VY : K_EPS);
+        } else {
+          const int it2 = it - N_TILE, q = it2 / (TW + 4);
+          c = 1 + (it2 - q * (TW + 4));
+          f = q / NRUN; run = q - f * NRUN;
+          f = f == 0 ? K_VX : K_B;
+        }
+        const int up = f == K_RHO ? URT : (f == K_VX ? U_VX : (f == K_VY ? U_VY : (f == K_EPS ? U_EPS : U_BX)));
+        const double cf = f == K_RHO ? a.prm.c_rho : (f == K_EPS ? a.prm.c_e : (f == K_B ? a.prm.c_b : a.prm.c_mom));
         const int r0 = 2 + run * RY;
-        kappa_run<RY>(pl(usrc[f]) + r0 * T::P + c, T::P, coef[f], pl(S_KY0 + f) + r0 * T::P + c, T::P,
-                      min(RY, TH + 3 - r0));
+        kappa_run<RY>(U + up * T::U_PLANE + T::u(r0, c), T::PU, cf * vt, KY + f * T::KY_PLANE + T::ky(r0, c),
+                      T::PKY, min(RY, TH + 3 - r0));
       }
     }
     __syncthreads();
 
     // ------------------------------------------------------------ P3: mixed fluxes folded into F (c-5)
-    const int SBX = BG ? S_BXT : S_BX, SBY = BG ? S_BYT : S_BY;
-    // G_x (needs y-derivatives): tile rows, staged columns 1 .. TW+4
+    // G(. ; x) needs y-derivatives: tile rows, staged columns 1 .. TW+4
     for (int idx = tid; idx < TH * (TW + 4); idx += NT) {
-      const int r = NG + idx / (TW + 4), c = 1 + idx % (TW + 4);
-      const int s = r * T::P + c;
-      const double kv = 0.5 * (pl(S_KY0 + K_VX)[s - T::P] + pl(S_KY0 + K_VX)[s]);   // nubar_y(vx)/Delta_y
-      const double kb = 0.5 * (pl(S_KY0 + K_B)[s - T::P] + pl(S_KY0 + K_B)[s]);     // nubar_y(bx~)/Delta_y
-      const double gm = ((0.5 * pl(S_RHO)[s]) * kv) * (cd12(pl(S_VX) + s, T::P) * (1.0 / 12.0));  // G(my;x)
-      const double gb = -(kb * (cd12(pl(S_BX) + s, T::P) * (1.0 / 12.0)));                        // G(by;x)
-      pl(S_CX0 + C_MY)[s] -= gm;
-      pl(S_CX0 + C_B)[s] -= gb;
-      pl(S_CX0 + C_E)[s] -= fma(pl(S_VY)[s], gm, pl(SBY)[s] * gb);
+      const int q = idx / (TW + 4);
+      const int r = NG + q, c = 1 + (idx - q * (TW + 4));
+      const int s = T::u(r, c), k = T::ky(r, c);
+      const double kv = 0.5 * (KY[K_VX * T::KY_PLANE + k - T::PKY] + KY[K_VX * T::KY_PLANE + k]);
+      const double kb = 0.5 * (KY[K_B * T::KY_PLANE + k - T::PKY] + KY[K_B * T::KY_PLANE + k]);
+      const double gm = ((0.5 * U[U_RHO * T::U_PLANE + s]) * kv) *
+                        (cd12(U + U_VX * T::U_PLANE + s, T::PU) * (1.0 / 12.0));          // G(my ; x)
+      const double gb = -(kb * (cd12(U + U_BX * T::U_PLANE + s, T::PU) * (1.0 / 12.0)));   // G(by ; x)
+      double* cxp = CX + T::cx(r, c);
+      cxp[C_MY * T::CX_PLANE] -= gm;
+      cxp[C_B * T::CX_PLANE] -= gb;
+      cxp[C_E * T::CX_PLANE] -= fma(U[U_VY * T::U_PLANE + s], gm, U[UBYT * T::U_PLANE + s] * gb);
     }
-    // G_y (needs x-derivatives): staged rows 1 .. TH+4, tile columns
+    // G(. ; y) needs x-derivatives: staged rows 1 .. TH+4, tile columns
     for (int idx = tid; idx < (TH + 4) * TW; idx += NT) {
-      const int r = 1 + idx / TW, c = NG + idx % TW;
-      const int s = r * T::P + c;
-      const double kv = 0.5 * (pl(S_KX0 + K_VY)[s - 1] + pl(S_KX0 + K_VY)[s]);      // nubar_x(vy)/Delta_x
-      const double kb = 0.5 * (pl(S_KX0 + K_B)[s - 1] + pl(S_KX0 + K_B)[s]);        // nubar_x(by~)/Delta_x
-      const double gm = ((0.5 * pl(S_RHO)[s]) * kv) * (cd12(pl(S_VY) + s, 1) * (1.0 / 12.0));     // G(mx;y)
-      const double gb = -(kb * (cd12(pl(S_BY) + s, 1) * (1.0 / 12.0)));                           // G(bx;y)
-      pl(S_CY0 + C_MX)[s] -= gm;
-      pl(S_CY0 + C_B)[s] -= gb;
-      pl(S_CY0 + C_E)[s] -= fma(pl(S_VX)[s], gm, pl(SBX)[s] * gb);
+      const int q = idx / TW;
+      const int r = 1 + q, c = NG + (idx - q * TW);
+      const int s = T::u(r, c), k = T::kx(r, c);
+      const double kv = 0.5 * (KX[K_VY * T::KX_PLANE + k - 1] + KX[K_VY * T::KX_PLANE + k]);
+      const double kb = 0.5 * (KX[K_B * T::KX_PLANE + k - 1] + KX[K_B * T::KX_PLANE + k]);
+      const double gm = ((0.5 * U[U_RHO * T::U_PLANE + s]) * kv) *
+                        (cd12(U + U_VY * T::U_PLANE + s, 1) * (1.0 / 12.0));               // G(mx ; y)
+      const double gb = -(kb * (cd12(U + U_BY * T::U_PLANE + s, 1) * (1.0 / 12.0)));        // G(bx ; y)
+      double* cyp = CY + T::cy(r, c);
+      cyp[C_MX * T::CY_PLANE] -= gm;
+      cyp[C_B * T::CY_PLANE] -= gb;
+      cyp[C_E * T::CY_PLANE] -= fma(U[U_VX * T::U_PLANE + s], gm, U[UBXT * T::U_PLANE + s] * gb);
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------ P3b: interface fluxes, once per interface
+    // Phi = g kappa (q_b - q_a), written over kappa.  x-interfaces (c | c+1), c = 2 .. TW+2, tile rows.
+    for (int idx = tid; idx < TH * (TW + 1); idx += NT) {
+      const int q = idx / (TW + 1);
+      const int r = NG + q, c = 2 + (idx - q * (TW + 1));
+      const int sa = T::u(r, c), sb = sa + 1;
+      double* kp = KX + T::kx(r, c);
+      const double rbar = 0.5 * (U[U_RHO * T::U_PLANE + sa] + U[U_RHO * T::U_PLANE + sb]);
+      const double vxa = U[U_VX * T::U_PLANE + sa], vxb = U[U_VX * T::U_PLANE + sb];
+      const double vya = U[U_VY * T::U_PLANE + sa], vyb = U[U_VY * T::U_PLANE + sb];
+      const double p_rho = kp[K_RHO * T::KX_PLANE] * (U[URT * T::U_PLANE + sb] - U[URT * T::U_PLANE + sa]);
+      const double p_mx = (rbar * kp[K_VX * T::KX_PLANE]) * (vxb - vxa);
+      const double p_my = ((0.5 * rbar) * kp[K_VY * T::KX_PLANE]) * (vyb - vya);
+      const double p_eps = kp[K_EPS * T::KX_PLANE] * (U[U_EPS * T::U_PLANE + sb] - U[U_EPS * T::U_PLANE + sa]);
+      const double p_b = kp[K_B * T::KX_PLANE] * (U[U_BY * T::U_PLANE + sb] - U[U_BY * T::U_PLANE + sa]);
+      const double Bbar = 0.5 * (U[UBYT * T::U_PLANE + sa] + U[UBYT * T::U_PLANE + sb]);
+      kp[C_RHO * T::KX_PLANE] = p_rho; kp[C_MX * T::KX_PLANE] = p_mx; kp[C_MY * T::KX_PLANE] = p_my;
+      kp[C_B * T::KX_PLANE] = p_b;
+      kp[C_E * T::KX_PLANE] = fma(Bbar, p_b, fma(0.5 * (vya + vyb), p_my, fma(0.5 * (vxa + vxb), p_mx, p_eps)));
+    }
+    // y-interfaces (r | r+1), r = 2 .. TH+2, tile columns.
+    for (int idx = tid; idx < (TH + 1) * TW; idx += NT) {
+      const int q = idx / TW;
+      const int r = 2 + q, c = NG + (idx - q * TW);
+      const int sa = T::u(r, c), sb = sa + T::PU;
+      double* kp = KY + T::ky(r, c);
+      const double rbar = 0.5 * (U[U_RHO * T::U_PLANE + sa] + U[U_RHO * T::U_PLANE + sb]);
+      const double vxa = U[U_VX * T::U_PLANE + sa], vxb = U[U_VX * T::U_PLANE + sb];
+      const double vya = U[U_VY * T::U_PLANE + sa], vyb = U[U_VY * T::U_PLANE + sb];
+      const double p_rho = kp[K_RHO * T::KY_PLANE] * (U[URT * T::U_PLANE + sb] - U[URT * T::U_PLANE + sa]);
+      const double p_mx = ((0.5 * rbar) * kp[K_VX * T::KY_PLANE]) * (vxb - vxa);
+      const double p_my = (rbar * kp[K_VY * T::KY_PLANE]) * (vyb - vya);
+      const double p_eps = kp[K_EPS * T::KY_PLANE] * (U[U_EPS * T::U_PLANE + sb] - U[U_EPS * T::U_PLANE + sa]);
+      const double p_b = kp[K_B * T::KY_PLANE] * (U[U_BX * T::U_PLANE + sb] - U[U_BX * T::U_PLANE + sa]);
+      const double Bbar = 0.5 * (U[UBXT * T::U_PLANE + sa] + U[UBXT * T::U_PLANE + sb]);
+      kp[C_RHO * T::KY_PLANE] = p_rho; kp[C_MX * T::KY_PLANE] = p_mx; kp[C_MY * T::KY_PLANE] = p_my;
+      kp[C_B * T::KY_PLANE] = p_b;
+      kp[C_E * T::KY_PLANE] = fma(Bbar, p_b, fma(0.5 * (vya + vyb), p_my, fma(0.5 * (vxa + vxb), p_mx, p_eps)));
     }
     __syncthreads();
   }
@@ -231,15 +334,17 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
     const int ty = idx / TW, tx = idx - ty * TW;
     const int i = x0 + tx, j = y0 + ty;
     if (i >= g.nx || j >= g.ny) continue;
-    const int s = (ty + NG) * T::P + (tx + NG);
+    const int r = ty + NG, c = tx + NG;
+    const double* cxp = CX + T::cx(r, c);
+    const double* cyp = CY + T::cy(r, c);
     double R[NF];
     // central differences of the (mixed-flux-corrected) fluxes:  -(d^c_x C_x + d^c_y C_y)
-    R[F_RHO] = fma(cd12(pl(S_CX0 + C_RHO) + s, 1), idx_, cd12(pl(S_CY0 + C_RHO) + s, T::P) * idy_) * (-1.0 / 12.0);
-    R[F_MX] = fma(cd12(pl(S_CX0 + C_MX) + s, 1), idx_, cd12(pl(S_CY0 + C_MX) + s, T::P) * idy_) * (-1.0 / 12.0);
-    R[F_MY] = fma(cd12(pl(S_CX0 + C_MY) + s, 1), idx_, cd12(pl(S_CY0 + C_MY) + s, T::P) * idy_) * (-1.0 / 12.0);
-    R[F_E] = fma(cd12(pl(S_CX0 + C_E) + s, 1), idx_, cd12(pl(S_CY0 + C_E) + s, T::P) * idy_) * (-1.0 / 12.0);
-    R[F_BX] = (cd12(pl(S_CY0 + C_B) + s, T::P) * idy_) * (-1.0 / 12.0);          // F_x(bx) == 0
-    R[F_BY] = fma(cd12(pl(S_CX0 + C_B) + s, 1), idx_, 0.0) * (-1.0 / 12.0);       // F_y(by) == 0
+    R[F_RHO] = fma(cd12(cxp + C_RHO * T::CX_PLANE, 1), idx_, cd12(cyp + C_RHO * T::CY_PLANE, T::PCY) * idy_) * (-1.0 / 12.0);
+    R[F_MX] = fma(cd12(cxp + C_MX * T::CX_PLANE, 1), idx_, cd12(cyp + C_MX * T::CY_PLANE, T::PCY) * idy_) * (-1.0 / 12.0);
+    R[F_MY] = fma(cd12(cxp + C_MY * T::CX_PLANE, 1), idx_, cd12(cyp + C_MY * T::CY_PLANE, T::PCY) * idy_) * (-1.0 / 12.0);
+    R[F_E] = fma(cd12(cxp + C_E * T::CX_PLANE, 1), idx_, cd12(cyp + C_E * T::CY_PLANE, T::PCY) * idy_) * (-1.0 / 12.0);
+    R[F_BX] = (cd12(cyp + C_B * T::CY_PLANE, T::PCY) * idy_) * (-1.0 / 12.0);         // F_x(bx) == 0
+    R[F_BY] = fma(cd12(cxp + C_B * T::CX_PLANE, 1), idx_, 0.0) * (-1.0 / 12.0);        // F_y(by) == 0
 
     const long long ga = cell_addr(g, i, j);
     double rho_b = 0.0, e_b = 0.0, Bbx = 0.0, Bby = 0.0;
@@ -247,60 +352,31 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       rho_b = a.bg.p[BG_RHO][ga]; e_b = a.bg.p[BG_E][ga];
       Bbx = a.bg.p[BG_BX][ga];    Bby = a.bg.p[BG_BY][ga];
       // energy source S_e = -p_tb div v + B_b B_b : grad v      (c-2)
+      const int s = T::u(r, c);
       const double bb2h = 0.5 * fma(Bby, Bby, Bbx * Bbx);
       const double ptb = fma(gm1, e_b - bb2h, bb2h);
-      const double dxvx = (cd12(pl(S_VX) + s, 1) * idx_) * (1.0 / 12.0);
-      const double dyvx = (cd12(pl(S_VX) + s, T::P) * idy_) * (1.0 / 12.0);
-      const double dxvy = (cd12(pl(S_VY) + s, 1) * idx_) * (1.0 / 12.0);
-      const double dyvy = (cd12(pl(S_VY) + s, T::P) * idy_) * (1.0 / 12.0);
+      const double dxvx = (cd12(U + U_VX * T::U_PLANE + s, 1) * idx_) * (1.0 / 12.0);
+      const double dyvx = (cd12(U + U_VX * T::U_PLANE + s, T::PU) * idy_) * (1.0 / 12.0);
+      const double dxvy = (cd12(U + U_VY * T::U_PLANE + s, 1) * idx_) * (1.0 / 12.0);
+      const double dyvy = (cd12(U + U_VY * T::U_PLANE + s, T::PU) * idy_) * (1.0 / 12.0);
       const double S = fma(-ptb, dxvx + dyvy,
                            fma(Bby * Bby, dyvy, fma(Bbx * Bby, dxvy + dyvx, (Bbx * Bbx) * dxvx)));
       R[F_E] = R[F_E] + S;
     }
 
     if (HD) {
-      const int SRT = BG ? S_RHOT : S_RHO, SBX = BG ? S_BXT : S_BX, SBY = BG ? S_BYT : S_BY;
-      // interface fluxes Phi = g kappa (q_b - q_a) at the two x- and the two y-interfaces of the cell
-      double fx[2][5], fy[2][5];   // [side][rho, mx, my, e, b]
-#pragma unroll
-      for (int side = 0; side < 2; ++side) {
-        {
-          const int sa = s - 1 + side, sb = sa + 1;
-          const double rbar = 0.5 * (pl(S_RHO)[sa] + pl(S_RHO)[sb]);
-          const double p_rho = pl(S_KX0 + K_RHO)[sa] * (pl(SRT)[sb] - pl(SRT)[sa]);
-          const double p_mx = (rbar * pl(S_KX0 + K_VX)[sa]) * (pl(S_VX)[sb] - pl(S_VX)[sa]);
-          const double p_my = ((0.5 * rbar) * pl(S_KX0 + K_VY)[sa]) * (pl(S_VY)[sb] - pl(S_VY)[sa]);
-          const double p_eps = pl(S_KX0 + K_EPS)[sa] * (pl(S_EPS)[sb] - pl(S_EPS)[sa]);
-          const double p_b = pl(S_KX0 + K_B)[sa] * (pl(S_BY)[sb] - pl(S_BY)[sa]);
-          fx[side][C_RHO] = p_rho; fx[side][C_MX] = p_mx; fx[side][C_MY] = p_my; fx[side][C_B] = p_b;
-          fx[side][C_E] = fma(0.5 * (pl(SBY)[sa] + pl(SBY)[sb]), p_b,
-                              fma(0.5 * (pl(S_VY)[sa] + pl(S_VY)[sb]), p_my,
-                                  fma(0.5 * (pl(S_VX)[sa] + pl(S_VX)[sb]), p_mx, p_eps)));
-        }
-        {
-          const int sa = s + (side - 1) * T::P, sb = sa + T::P;
-          const double rbar = 0.5 * (pl(S_RHO)[sa] + pl(S_RHO)[sb]);
-          const double p_rho = pl(S_KY0 + K_RHO)[sa] * (pl(SRT)[sb] - pl(SRT)[sa]);
-          const double p_mx = ((0.5 * rbar) * pl(S_KY0 + K_VX)[sa]) * (pl(S_VX)[sb] - pl(S_VX)[sa]);
-          const double p_my = (rbar * pl(S_KY0 + K_VY)[sa]) * (pl(S_VY)[sb] - pl(S_VY)[sa]);
-          const double p_eps = pl(S_KY0 + K_EPS)[sa] * (pl(S_EPS)[sb] - pl(S_EPS)[sa]);
-          const double p_b = pl(S_KY0 + K_B)[sa] * (pl(S_BX)[sb] - pl(S_BX)[sa]);
-          fy[side][C_RHO] = p_rho; fy[side][C_MX] = p_mx; fy[side][C_MY] = p_my; fy[side][C_B] = p_b;
-          fy[side][C_E] = fma(0.5 * (pl(SBX)[sa] + pl(SBX)[sb]), p_b,
-                              fma(0.5 * (pl(S_VY)[sa] + pl(S_VY)[sb]), p_my,
-                                  fma(0.5 * (pl(S_VX)[sa] + pl(S_VX)[sb]), p_mx, p_eps)));
-        }
-      }
-      R[F_RHO] = fma(fx[1][C_RHO] - fx[0][C_RHO], idx_, R[F_RHO]);
-      R[F_MX] = fma(fx[1][C_MX] - fx[0][C_MX], idx_, R[F_MX]);
-      R[F_MY] = fma(fx[1][C_MY] - fx[0][C_MY], idx_, R[F_MY]);
-      R[F_E] = fma(fx[1][C_E] - fx[0][C_E], idx_, R[F_E]);
-      R[F_BY] = fma(fx[1][C_B] - fx[0][C_B], idx_, R[F_BY]);
-      R[F_RHO] = fma(fy[1][C_RHO] - fy[0][C_RHO], idy_, R[F_RHO]);
-      R[F_MX] = fma(fy[1][C_MX] - fy[0][C_MX], idy_, R[F_MX]);
-      R[F_MY] = fma(fy[1][C_MY] - fy[0][C_MY], idy_, R[F_MY]);
-      R[F_E] = fma(fy[1][C_E] - fy[0][C_E], idy_, R[F_E]);
-      R[F_BX] = fma(fy[1][C_B] - fy[0][C_B], idy_, R[F_BX]);
+      const double* px = KX + T::kx(r, c);      // interface (c | c+1); (c-1 | c) is at px[-1]
+      const double* py = KY + T::ky(r, c);      // interface (r | r+1); (r-1 | r) is at py[-PKY]
+      R[F_RHO] = fma(px[C_RHO * T::KX_PLANE] - px[C_RHO * T::KX_PLANE - 1], idx_, R[F_RHO]);
+      R[F_MX] = fma(px[C_MX * T::KX_PLANE] - px[C_MX * T::KX_PLANE - 1], idx_, R[F_MX]);
+      R[F_MY] = fma(px[C_MY * T::KX_PLANE] - px[C_MY * T::KX_PLANE - 1], idx_, R[F_MY]);
+      R[F_E] = fma(px[C_E * T::KX_PLANE] - px[C_E * T::KX_PLANE - 1], idx_, R[F_E]);
+      R[F_BY] = fma(px[C_B * T::KX_PLANE] - px[C_B * T::KX_PLANE - 1], idx_, R[F_BY]);
+      R[F_RHO] = fma(py[C_RHO * T::KY_PLANE] - py[C_RHO * T::KY_PLANE - T::PKY], idy_, R[F_RHO]);
+      R[F_MX] = fma(py[C_MX * T::KY_PLANE] - py[C_MX * T::KY_PLANE - T::PKY], idy_, R[F_MX]);
+      R[F_MY] = fma(py[C_MY * T::KY_PLANE] - py[C_MY * T::KY_PLANE - T::PKY], idy_, R[F_MY]);
+      R[F_E] = fma(py[C_E * T::KY_PLANE] - py[C_E * T::KY_PLANE - T::PKY], idy_, R[F_E]);
+      R[F_BX] = fma(py[C_B * T::KY_PLANE] - py[C_B * T::KY_PLANE - T::PKY], idy_, R[F_BX]);
     }
 
     // RK combine (c-6) and write
@@ -330,7 +406,7 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       else
         cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, a.ws_mode == WS_FULL, w4);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) wsmax[k] = fmax(wsmax[k], w4[k]);
+      for (int k = 0; k < 4; ++k) wsmax[k] = dmax(wsmax[k], w4[k]);
     }
   }
   if (a.ws_mode != WS_NONE)
