@@ -35,7 +35,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in _sources() + [os.path.join(INCLUDE, "smaug.h")])
     if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        extra = os.environ.get("SMAUG_NVCC_EXTRA", "").split()     # e.g. -DSMAUG_TW=24 for tuning sweeps
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu")]
         subprocess.run(cmd, check=True)
     return LIB_PATH

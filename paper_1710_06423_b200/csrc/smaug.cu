@@ -33,7 +33,16 @@ int fail(int code, const std::string& msg) {
   } while (0)
 
 // Tile / launch configuration of the fused stage kernel.
-constexpr int TW = 32, TH = 16, NT = 512;
+#ifndef SMAUG_TW
+#define SMAUG_TW 32
+#endif
+#ifndef SMAUG_TH
+#define SMAUG_TH 16
+#endif
+#ifndef SMAUG_NT
+#define SMAUG_NT 512
+#endif
+constexpr int TW = SMAUG_TW, TH = SMAUG_TH, NT = SMAUG_NT;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
