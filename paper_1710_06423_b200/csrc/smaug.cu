@@ -12,7 +12,7 @@
 #include <string>
 #include <vector>
 
-#include "smaug_stage_kernel.cuh"
+#include "smaug_march_kernel.cuh"
 
 using namespace smaug;
 
@@ -97,6 +97,7 @@ struct smaug_ctx {
   double stage_ms = 0;
   long long stage_launches = 0;
   bool pending_status = false;
+  bool use_march = true;    // streaming kernel when applicable (SMAUG_PARAM_KERNEL 0 forces the tile kernel)
 };
 
 namespace {
@@ -163,7 +164,44 @@ int launch_stage_t(smaug_ctx* c, const StageArgs& a) {
   return SMAUG_OK;
 }
 
+#ifndef SMAUG_MARCH_NT
+#define SMAUG_MARCH_NT 256
+#endif
+constexpr int MARCH_NT = SMAUG_MARCH_NT;
+
+// Streaming form (smaug_march_kernel.cuh): no background, hyperdiffusion on.
+int launch_march(smaug_ctx* c, const StageArgs& a) {
+  static bool configured = false;
+  constexpr size_t smem = MarchSmem<MARCH_NT>::BYTES;
+  auto kern = march_kernel<MARCH_NT>;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  const int W = MARCH_NT - 2 * NG;
+  const int strips = (c->g.nx + W - 1) / W;
+  const int target = 148 * 8;
+  int nchunks = std::max(1, (target + strips - 1) / strips);
+  MarchGeom mg;
+  mg.rows_per_cta = std::max(32, (c->g.ny + nchunks - 1) / nchunks);
+  nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
+  dim3 grid(strips, nchunks);
+  c->last_ctas = strips * nchunks;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing && c->ev_used + 2 <= c->ev.size()) {
+    e0 = c->ev[c->ev_used++];
+    e1 = c->ev[c->ev_used++];
+    CU(cudaEventRecord(e0, c->stream));
+  }
+  kern<<<grid, MARCH_NT, smem, c->stream>>>(a, mg);
+  if (e1) CU(cudaEventRecord(e1, c->stream));
+  c->launches++;
+  CU(cudaGetLastError());
+  return SMAUG_OK;
+}
+
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
+  if (!c->has_bg && c->hd_on && c->use_march) return launch_march(c, a);
   if (c->has_bg) return c->hd_on ? launch_stage_t<true, true>(c, a) : launch_stage_t<true, false>(c, a);
   return c->hd_on ? launch_stage_t<false, true>(c, a) : launch_stage_t<false, false>(c, a);
 }
@@ -363,6 +401,7 @@ int smaug_set_param(smaug_ctx* c, int key, double v) {
     case SMAUG_PARAM_C_B: if (!(v >= 0)) break; c->c_b = v; return SMAUG_OK;
     case SMAUG_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c->rk_order = (int)v; return SMAUG_OK;
     case SMAUG_PARAM_FIXED_DT: if (!(v >= 0)) break; c->fixed_dt = v; return SMAUG_OK;
+    case SMAUG_PARAM_KERNEL: c->use_march = v != 0.0; return SMAUG_OK;
     default: return fail(SMAUG_EINVAL, "unknown parameter key");
   }
   return fail(SMAUG_EINVAL, "parameter value out of range");

@@ -40,6 +40,7 @@ def gpu_run(pkg, w, bc, gamma, steps, cfl=0.3, bg=None, host=True, chunks=1, **p
 
 def cpu_run(oracle_mod, w, bc, gamma, steps, cfl=0.3, bg=None, threads=8, **params):
     ny, nx = w.shape[1:]
+    params = {k: v for k, v in params.items() if k != "kernel"}     # kernel choice is a GPU-only switch
     o = oracle_mod.Oracle(nx, ny, gamma, bc, bg=bg, threads=threads, **params)
     o.set_state(w)
     o.step(steps, cfl)
@@ -117,7 +118,7 @@ def test_boundary_kinds_with_background(gpu, oracle_mod, bc):
 
 @pytest.mark.parametrize("params", [dict(hd_on=0), dict(rk_order=2), dict(rk_order=1, hd_on=1),
                                     dict(fixed_dt=1e-4), dict(c_rho=0.1, c_mom=0.2, c_e=0.05, c_b=0.3),
-                                    dict(lx=2.0, ly=0.5)])
+                                    dict(lx=2.0, ly=0.5), dict(kernel=0), dict(kernel=0, rk_order=2)])
 def test_parameters(gpu, oracle_mod, params):
     w, bc, gamma = si.orszag_tang(64, 48)
     a = gpu_run(gpu, w, bc, gamma, 10, **params)
