@@ -14,7 +14,7 @@ namespace smaug {
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void cell_wavespeeds(double rho, double mx, double my, double e, double Bx,
                                                 double By, double gamma, bool full, double out[4]) {
-  const double rr = 1.0 / rho;
+  const double rr = drcp(rho);
   const double vx = mx * rr, vy = my * rr;
   const double B2 = fma(By, By, Bx * Bx);
   const double pk = (gamma - 1.0) * ((e - 0.5 * fma(my, vy, mx * vx)) - 0.5 * B2);

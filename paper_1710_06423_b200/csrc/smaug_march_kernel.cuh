@@ -43,13 +43,13 @@ struct MarchSmem {
 __device__ __forceinline__ double kappa6(double u0, double u1, double u2, double u3, double u4, double u5,
                                          double cv, double& d1_mid) {
   const double a0 = u1 - u0, a1 = u2 - u1, a2 = u3 - u2, a3 = u4 - u3, a4 = u5 - u4;   // D1 at -2 .. +2
-  const double t0 = fabs(fma(3.0, a1, -(u3 - u0)));     // D3 at interface -1
-  const double t1 = fabs(fma(3.0, a2, -(u4 - u1)));     // D3 at interface  0
-  const double t2 = fabs(fma(3.0, a3, -(u5 - u2)));     // D3 at interface +1
+  const double t0 = dabs(fma(3.0, a1, -(u3 - u0)));     // D3 at interface -1
+  const double t1 = dabs(fma(3.0, a2, -(u4 - u1)));     // D3 at interface  0
+  const double t2 = dabs(fma(3.0, a3, -(u5 - u2)));     // D3 at interface +1
   const double m3 = dmax(dmax(t0, t1), t2);
-  const double m1 = dmax(dmax(dmax(fabs(a0), fabs(a1)), dmax(fabs(a2), fabs(a3))), fabs(a4));
+  const double m1 = dmax(dmax(dmax(dabs(a0), dabs(a1)), dmax(dabs(a2), dabs(a3))), dabs(a4));
   d1_mid = a2;
-  return m1 > 0.0 ? cv * (m3 / m1) : 0.0;
+  return m1 > 0.0 ? cv * ratio_div(m3, m1) : 0.0;
 }
 
 __device__ __forceinline__ double cd12v(double m2, double m1, double p1, double p2) {
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
     }
 
     // ------------------------------------------------------------------ head: derived quantities of row r
-    const double rr = 1.0 / rho;
+    const double rr = drcp(rho);
     const double vx = mx * rr, vy = my * rr;
     const double b2h = 0.5 * fma(by, by, bx * bx);
     const double ke = 0.5 * fma(my, vy, mx * vx);

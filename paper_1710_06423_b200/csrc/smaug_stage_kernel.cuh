@@ -87,6 +87,10 @@ enum { C_RHO = 0, C_MX = 1, C_MY = 2, C_E = 3, C_B = 4 };
 // max of two non-negative doubles: one DSETP + two selects (fmax() costs ~7 instructions on sm_100a
 // because of its NaN-quieting semantics).  max is exact, so any evaluation order is bit-safe.
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+// |x| as one integer op on the high word (keeps the fp64 pipe free; bit-identical to fabs)
+__device__ __forceinline__ double dabs(double x) {
+  return __hiloint2double(__double2hiint(x) & 0x7fffffff, __double2loint(x));
+}
 
 // kappa = cv * (M3 / M1) for n <= R consecutive interfaces of one line (c-5).  u points at the cell left of
 // the first interface (interface k lies between cells k and k+1); cells -2 .. R+2 are read with stride s.
@@ -102,14 +106,14 @@ __device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, d
   for (int k = 0; k < R + 4; ++k) d1[k] = uu[k + 1] - uu[k];                       // interface k-2
   double d3[R + 2];
 #pragma unroll
-  for (int k = 0; k < R + 2; ++k) d3[k] = fabs(fma(3.0, d1[k + 1], -(uu[k + 3] - uu[k])));   // interface k-1
+  for (int k = 0; k < R + 2; ++k) d3[k] = dabs(fma(3.0, d1[k + 1], -(uu[k + 3] - uu[k])));   // interface k-1
 #pragma unroll
-  for (int k = 0; k < R + 4; ++k) d1[k] = fabs(d1[k]);
+  for (int k = 0; k < R + 4; ++k) d1[k] = dabs(d1[k]);
 #pragma unroll
   for (int k = 0; k < R; ++k) {
     const double m3 = dmax(dmax(d3[k], d3[k + 1]), d3[k + 2]);
     const double m1 = dmax(dmax(dmax(d1[k], d1[k + 1]), dmax(d1[k + 2], d1[k + 3])), d1[k + 4]);
-    const double r = m1 > 0.0 ? cv * (m3 / m1) : 0.0;
+    const double r = m1 > 0.0 ? cv * ratio_div(m3, m1) : 0.0;
     if (k < n) out[k * os] = r;
   }
 }
@@ -142,7 +146,7 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
       Bbx = a.bg.p[BG_BX][ga];    Bby = a.bg.p[BG_BY][ga];
     }
     const double rho = BG ? rho_b + rhot : rhot;
-    const double rr = 1.0 / rho;
+    const double rr = drcp(rho);
     const double vx = mx * rr, vy = my * rr;
     const double b2h = 0.5 * fma(by, by, bx * bx);
     const double cross = BG ? fma(Bby, by, Bbx * bx) : 0.0;
