@@ -33,8 +33,10 @@ struct MarchSmem {
   static constexpr int OFF_CXP = OFF_UP + 5 * PW;     // 5 planes: C_x of the tail row
   static constexpr int OFF_PK = OFF_CXP + 5 * PW;     // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
   static constexpr int OFF_DXR = OFF_PK + 7 * PW;     // ring 4 rows x 5: Phi_x differences (thread-private)
-  static constexpr int OFF_CYR = OFF_DXR + 4 * 5 * NT;  // ring 8 rows x 5: C_y (thread-private)
-  static constexpr int OFF_RED = OFF_CYR + 8 * 5 * NT;
+  static constexpr int OFF_CYR = OFF_DXR + 4 * 5 * NT;  // ring 6 rows x 5: C_y (thread-private)
+  static constexpr int OFF_INR = OFF_CYR + 6 * 5 * NT;  // ring 4 rows x 6: cp.async landing zone of the input rows
+  static constexpr int OFF_TLR = OFF_INR + 4 * 6 * NT;  // ring 4 rows x 3: raw mx, my, e of the rows r-3 .. r
+  static constexpr int OFF_RED = OFF_TLR + 4 * 3 * NT;
   static constexpr int TOTAL = OFF_RED + 4 * 32;
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
 };
@@ -52,6 +54,14 @@ __device__ __forceinline__ double kappa6(double u0, double u1, double u2, double
   return m1 > 0.0 ? cv * ratio_div(m3, m1) : 0.0;
 }
 
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 __device__ __forceinline__ double cd12v(double m2, double m1, double p1, double p2) {
   return fma(8.0, p1 - m1, -(p2 - m2));
 }
@@ -65,6 +75,8 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
   double* const PK = smem + S::OFF_PK;
   double* const DXR = smem + S::OFF_DXR;
   double* const CYR = smem + S::OFF_CYR;
+  double* const INR = smem + S::OFF_INR;
+  double* const TLR = smem + S::OFF_TLR;
   double* const red_sh = smem + S::OFF_RED;
   constexpr int PW = S::PW;
   const Grid& g = a.g;
@@ -96,43 +108,31 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
   double wsmax[4] = {0.0, 0.0, 0.0, 0.0};
 
   const long long colbase = (long long)NG * g.pitch + (cl + XOFF);   // address of (cl, row 0)
-  // software prefetch of the next head row
-  double nw[NF];
-  {
-    const long long ga = colbase + (long long)min(ystart - NG, g.ny + NG - 1) * g.pitch;
+  // the input rows arrive two steps ahead through cp.async into a thread-private ring (no registers held)
+  auto fetch_row = [&](int row) {
+    const long long ga = colbase + (long long)min(row, g.ny + NG - 1) * g.pitch;
+    const int slot = (row + 4096) & 3;
 #pragma unroll
-    for (int f = 0; f < NF; ++f) nw[f] = a.in.p[f][ga];
-  }
+    for (int f = 0; f < NF; ++f) cp_async8(INR + (slot * NF + f) * NT + tid, a.in.p[f] + ga);
+    cp_async_commit();
+  };
+  fetch_row(ystart - NG);
+  fetch_row(ystart - NG + 1);
+  int s6 = 0;                                             // ring slot (mod 6) of row r in CYR
 
 #pragma unroll 1
   for (int r = ystart - NG; r < yend + NG; ++r) {
     const int j = r - NG;                                 // tail (output) row
     const bool tail_on = j >= ystart;                     // uniform over the CTA
     const bool ky_on = r >= ystart + NG - 1;              // six rows of history are valid
-    const double rho = nw[F_RHO], mx = nw[F_MX], my = nw[F_MY], et = nw[F_E], bx = nw[F_BX], by = nw[F_BY];
-    // prefetch row r+1
-    {
-      const long long ga = colbase + (long long)min(r + 1, g.ny + NG - 1) * g.pitch;
-#pragma unroll
-      for (int f = 0; f < NF; ++f) nw[f] = a.in.p[f][ga];
-    }
-    // tail-row raw values for F_x(j) and the combine (same lines were touched three steps ago: L1/L2 hits)
+    cp_async_wait<1>();                                   // row r has landed (row r+1 may be in flight)
+    const int slot4 = (r + 4096) & 3;
+    const double rho = INR[(slot4 * NF + F_RHO) * NT + tid], mx = INR[(slot4 * NF + F_MX) * NT + tid];
+    const double my = INR[(slot4 * NF + F_MY) * NT + tid], et = INR[(slot4 * NF + F_E) * NT + tid];
+    const double bx = INR[(slot4 * NF + F_BX) * NT + tid], by = INR[(slot4 * NF + F_BY) * NT + tid];
+    fetch_row(r + 2);
+    TLR[(slot4 * 3 + 0) * NT + tid] = mx; TLR[(slot4 * 3 + 1) * NT + tid] = my; TLR[(slot4 * 3 + 2) * NT + tid] = et;
     const long long gj = colbase + (long long)max(j, -NG) * g.pitch;
-    double jmx = 0.0, jmy = 0.0, jet = 0.0, jbase[NF], jacc[NF], jin[NF];
-    if (tail_on) {
-      jmx = a.in.p[F_MX][gj]; jmy = a.in.p[F_MY][gj]; jet = a.in.p[F_E][gj];
-      if (combine == COMBINE_FINAL) {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
-      } else {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
-        if (combine == COMBINE_ACC) {
-#pragma unroll
-          for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
-        }
-      }
-    }
 
     // ------------------------------------------------------------------ head: derived quantities of row r
     const double rr = drcp(rho);
@@ -185,6 +185,8 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
       const double gm = ((0.5 * hr[2]) * kv) * (cd12v(hvx[0], hvx[1], hvx[3], hvx[4]) * (1.0 / 12.0));
       const double gb = -(kb * (cd12v(hbx[0], hbx[1], hbx[3], hbx[4]) * (1.0 / 12.0)));
       // F_x(rho, mx, my, e, by) of row j
+      const int js = (j + 4096) & 3;
+      const double jmx = TLR[(js * 3 + 0) * NT + tid], jmy = TLR[(js * 3 + 1) * NT + tid], jet = TLR[(js * 3 + 2) * NT + tid];
       const double jrho = hr[2], jvx = hvx[2], jvy = hvy[2], jeps = he[2], jbx = hbx[2], jby = hby[0];
       const double jb2h = 0.5 * fma(jby, jby, jbx * jbx);
       const double jptt = fma(gm1, jeps, jb2h);
@@ -197,6 +199,22 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
       CXP[C_B * PW + tp] = fma(jvx, jby, -(jbx * jvy)) - gb;
     }
     __syncthreads();
+
+    // operands of the RK combine for row j: issued here, consumed at the end of the step
+    double jbase[NF], jacc[NF], jin[NF];
+    if (tail_on) {
+      if (combine == COMBINE_FINAL) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
+      } else {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
+        if (combine == COMBINE_ACC) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
+        }
+      }
+    }
 
     // ------------------------------------------------------------------ head: x-interface (ci | ci+1) of row r
     double px[5], kxv, kxb, dcx_vy, dcx_by;
@@ -241,7 +259,6 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
     __syncthreads();
 
     // ------------------------------------------------------------------ head: Phi_x difference, G(. ; y), C_y(r)
-    const int slot4 = (r + 4096) & 3, slot8 = (r + 4096) & 7;
     {
       const double kvl = PK[5 * PW + tp - 1], kbl = PK[6 * PW + tp - 1];
 #pragma unroll
@@ -250,15 +267,17 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
       const double kb = 0.5 * (kbl + kxb);
       const double gm = ((0.5 * rho) * kv) * (dcx_vy * (1.0 / 12.0));      // G(mx ; y)
       const double gb = -(kb * (dcx_by * (1.0 / 12.0)));                   // G(bx ; y)
-      CYR[(slot8 * 5 + C_RHO) * NT + tid] = cyn[C_RHO];
-      CYR[(slot8 * 5 + C_MX) * NT + tid] = cyn[C_MX] - gm;
-      CYR[(slot8 * 5 + C_MY) * NT + tid] = cyn[C_MY];
-      CYR[(slot8 * 5 + C_E) * NT + tid] = cyn[C_E] - fma(vx, gm, bx * gb);
-      CYR[(slot8 * 5 + C_B) * NT + tid] = cyn[C_B] - gb;
+      CYR[(s6 * 5 + C_RHO) * NT + tid] = cyn[C_RHO];
+      CYR[(s6 * 5 + C_MX) * NT + tid] = cyn[C_MX] - gm;
+      CYR[(s6 * 5 + C_MY) * NT + tid] = cyn[C_MY];
+      CYR[(s6 * 5 + C_E) * NT + tid] = cyn[C_E] - fma(vx, gm, bx * gb);
+      CYR[(s6 * 5 + C_B) * NT + tid] = cyn[C_B] - gb;
     }
     // ------------------------------------------------------------------ tail C: assemble R(j), combine, write
     if (tail_on) {
-      const int jm2 = (j - 2 + 4096) & 7, jm1 = (j - 1 + 4096) & 7, jp1 = (j + 1 + 4096) & 7, jp2 = (j + 2 + 4096) & 7;
+      // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-6 ring
+      const int jm2 = s6 + 1 >= 6 ? s6 - 5 : s6 + 1, jm1 = s6 + 2 >= 6 ? s6 - 4 : s6 + 2;
+      const int jp1 = s6 + 4 >= 6 ? s6 - 2 : s6 + 4, jp2 = s6 + 5 >= 6 ? s6 - 1 : s6 + 5;
       double cdy[5];
 #pragma unroll
       for (int f = 0; f < 5; ++f)
@@ -309,7 +328,9 @@ __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const M
 #pragma unroll
     for (int f = 0; f < 5; ++f) py_prev[f] = py[f];
     kyv_prev = kyv; kyb_prev = kyb;
+    s6 = s6 == 5 ? 0 : s6 + 1;
   }
+  cp_async_wait<0>();
   if (ws_mode != WS_NONE)
     block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], ws_mode == WS_FULL ? 0 : 2);
 }
