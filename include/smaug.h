@@ -108,7 +108,8 @@ int smaug_get_wavespeeds(smaug_ctx* ctx, double out[4]);
 int smaug_get_launch_count(smaug_ctx* ctx, long long* n);
 
 /* Algorithmic / launch facts of the fused stage kernel, for the roofline report:
- * out = { tile_w, tile_h, threads, dynamic_smem_bytes, ctas_last_launch }. */
+ * out = { tile_w, tile_h, threads, dynamic_smem_bytes, ctas_last_launch }; the streaming kernel reports
+ * its strip width as tile_w and 1 as tile_h (it marches row by row). */
 int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
 
 /* Device time, in milliseconds, spent in the fused stage kernels (summed over launches) and the number of

@@ -488,8 +488,13 @@ int smaug_get_launch_count(smaug_ctx* c, long long* n) {
 int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (int rc = check_ctx(c)) return rc;
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
-  out[0] = TW; out[1] = TH; out[2] = NT;
-  out[3] = (int)(c->has_bg ? Tile<TW, TH, true>::BYTES : Tile<TW, TH, false>::BYTES);
+  if (!c->has_bg && c->hd_on && c->use_march) {   // streaming kernel: a strip of NT-6 columns, marched row by row
+    out[0] = MARCH_NT - 2 * NG; out[1] = 1; out[2] = MARCH_NT;
+    out[3] = (int)MarchSmem<MARCH_NT>::BYTES;
+  } else {
+    out[0] = TW; out[1] = TH; out[2] = NT;
+    out[3] = (int)(c->has_bg ? Tile<TW, TH, true>::BYTES : Tile<TW, TH, false>::BYTES);
+  }
   out[4] = c->last_ctas;
   return SMAUG_OK;
 }
