@@ -58,8 +58,9 @@ enum { /* keys of smaug_set_param */
   SMAUG_PARAM_C_B = 6,      /*   0.02 */
   SMAUG_PARAM_RK_ORDER = 7, /* 4 (default), 2 (midpoint) or 1 (forward Euler) */
   SMAUG_PARAM_FIXED_DT = 8, /* > 0: use this dt instead of the CFL step; 0 (default): CFL */
-  SMAUG_PARAM_KERNEL = 9    /* 1 (default): streaming stage kernel where applicable; 0: always the tile kernel.
-                               Both are bit-identical; the switch exists for tests and profiling. */
+  SMAUG_PARAM_KERNEL = 9    /* 2 (default): role-split streaming stage kernel where applicable (no background,
+                               hyperdiffusion on); 1: single-role streaming kernel where applicable; 0: always the
+                               tile kernel.  All are bit-identical; the switch exists for tests and profiling. */
 };
 
 /* Bytes of device memory a context for an nx-by-ny grid needs (has_bg != 0: a background is given).

@@ -12,7 +12,7 @@
 #include <string>
 #include <vector>
 
-#include "smaug_march_kernel.cuh"
+#include "smaug_split_kernel.cuh"
 
 using namespace smaug;
 
@@ -97,7 +97,9 @@ struct smaug_ctx {
   double stage_ms = 0;
   long long stage_launches = 0;
   bool pending_status = false;
-  bool use_march = true;    // streaming kernel when applicable (SMAUG_PARAM_KERNEL 0 forces the tile kernel)
+  int kernel_mode = 2;      // SMAUG_PARAM_KERNEL: 2 role-split streaming kernel, 1 single-role streaming kernel
+                            // (both only without background and with hyperdiffusion), 0 always the tile kernel
+  int n_sm = 148;
 };
 
 namespace {
@@ -200,8 +202,68 @@ int launch_march(smaug_ctx* c, const StageArgs& a) {
   return SMAUG_OK;
 }
 
+#ifndef SMAUG_SPLIT_NC
+#define SMAUG_SPLIT_NC 256
+#endif
+constexpr int SPLIT_NC = SMAUG_SPLIT_NC;
+
+// Chunk height of a streaming kernel: every CTA costs (rows + 6) row steps and CTAs run in waves of n_sm,
+// so pick the chunk count that minimises waves * (rows + 6).
+int pick_rows_per_cta(int ny, int strips, int n_sm) {
+  int best_rows = ny;
+  long long best_cost = -1;
+  for (int k = 1; k <= 64; ++k) {
+    int nch = std::max(1, n_sm * k / strips);
+    int rows = std::max(std::min(ny, 16), (ny + nch - 1) / nch);
+    nch = (ny + rows - 1) / rows;
+    const long long waves = ((long long)strips * nch + n_sm - 1) / n_sm;
+    const long long cost = waves * (rows + 2 * NG);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_rows = rows; }
+  }
+  return best_rows;
+}
+
+template <int COMBINE, int WS>
+int launch_split_t(smaug_ctx* c, const StageArgs& a) {
+  static bool configured = false;
+  constexpr size_t smem = SplitSmem<SPLIT_NC>::BYTES;
+  auto kern = split_kernel<SPLIT_NC, COMBINE, WS>;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  const int W = SPLIT_NC - 8;
+  const int strips = (c->g.nx + W - 1) / W;
+  MarchGeom mg;
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm);
+  const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
+  dim3 grid(strips, nchunks);
+  c->last_ctas = strips * nchunks;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing && c->ev_used + 2 <= c->ev.size()) {
+    e0 = c->ev[c->ev_used++];
+    e1 = c->ev[c->ev_used++];
+    CU(cudaEventRecord(e0, c->stream));
+  }
+  kern<<<grid, SPLIT_NC + SPLIT_NC / 2, smem, c->stream>>>(a, mg);
+  if (e1) CU(cudaEventRecord(e1, c->stream));
+  c->launches++;
+  CU(cudaGetLastError());
+  return SMAUG_OK;
+}
+
+// Role-split streaming form (smaug_split_kernel.cuh): no background, hyperdiffusion on.
+int launch_split(smaug_ctx* c, const StageArgs& a) {
+  if (a.combine == COMBINE_BASE && a.ws_mode == WS_VT) return launch_split_t<COMBINE_BASE, WS_VT>(c, a);
+  if (a.combine == COMBINE_ACC && a.ws_mode == WS_VT) return launch_split_t<COMBINE_ACC, WS_VT>(c, a);
+  if (a.combine == COMBINE_FINAL && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_FINAL, WS_FULL>(c, a);
+  if (a.combine == COMBINE_BASE && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_BASE, WS_FULL>(c, a);
+  return fail(SMAUG_EINVAL, "split kernel: unsupported combine / wave-speed mode");
+}
+
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
-  if (!c->has_bg && c->hd_on && c->use_march) return launch_march(c, a);
+  if (!c->has_bg && c->hd_on && c->kernel_mode == 2) return launch_split(c, a);
+  if (!c->has_bg && c->hd_on && c->kernel_mode == 1) return launch_march(c, a);
   if (c->has_bg) return c->hd_on ? launch_stage_t<true, true>(c, a) : launch_stage_t<true, false>(c, a);
   return c->hd_on ? launch_stage_t<false, true>(c, a) : launch_stage_t<false, false>(c, a);
 }
@@ -327,6 +389,12 @@ int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], con
   }
   smaug_ctx* c = new (std::nothrow) smaug_ctx();
   if (!c) return fail(SMAUG_ENOMEM, "host allocation failed");
+  {
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
+      c->n_sm = n_sm;
+  }
   c->has_bg = bg != nullptr;
   c->L = make_layout(nx, ny, c->has_bg);
   c->g.nx = nx; c->g.ny = ny; c->g.pitch = c->L.pitch; c->g.plane = c->L.plane;
@@ -401,7 +469,7 @@ int smaug_set_param(smaug_ctx* c, int key, double v) {
     case SMAUG_PARAM_C_B: if (!(v >= 0)) break; c->c_b = v; return SMAUG_OK;
     case SMAUG_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c->rk_order = (int)v; return SMAUG_OK;
     case SMAUG_PARAM_FIXED_DT: if (!(v >= 0)) break; c->fixed_dt = v; return SMAUG_OK;
-    case SMAUG_PARAM_KERNEL: c->use_march = v != 0.0; return SMAUG_OK;
+    case SMAUG_PARAM_KERNEL: if (v != 0 && v != 1 && v != 2) break; c->kernel_mode = (int)v; return SMAUG_OK;
     default: return fail(SMAUG_EINVAL, "unknown parameter key");
   }
   return fail(SMAUG_EINVAL, "parameter value out of range");
@@ -488,7 +556,10 @@ int smaug_get_launch_count(smaug_ctx* c, long long* n) {
 int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (int rc = check_ctx(c)) return rc;
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
-  if (!c->has_bg && c->hd_on && c->use_march) {   // streaming kernel: a strip of NT-6 columns, marched row by row
+  if (!c->has_bg && c->hd_on && c->kernel_mode == 2) {   // role-split streaming kernel: a strip of NC-8 columns
+    out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
+    out[3] = (int)SplitSmem<SPLIT_NC>::BYTES;
+  } else if (!c->has_bg && c->hd_on && c->kernel_mode == 1) {   // streaming kernel: a strip of NT-6 columns
     out[0] = MARCH_NT - 2 * NG; out[1] = 1; out[2] = MARCH_NT;
     out[3] = (int)MarchSmem<MARCH_NT>::BYTES;
   } else {

@@ -51,7 +51,7 @@ __device__ __forceinline__ double kappa6(double u0, double u1, double u2, double
   const double m3 = dmax(dmax(t0, t1), t2);
   const double m1 = dmax(dmax(dmax(dabs(a0), dabs(a1)), dmax(dabs(a2), dabs(a3))), dabs(a4));
   d1_mid = a2;
-  return m1 > 0.0 ? cv * ratio_div(m3, m1) : 0.0;
+  return kappa_ratio(m3, m1, cv);
 }
 
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {

@@ -1,0 +1,387 @@
+// smaug_split_kernel.cuh -- the role-split streaming form of the fused stage kernel (no background,
+// hyperdiffusion on: the benchmark configurations).  Same arithmetic contract as every other stage kernel
+// (DESIGN.md section 4): bit-identical to the oracle.
+//
+// One CTA owns a strip of NC columns (NC - 8 of them produce output, 4 halo columns on each side so that
+// column pairs are 16-byte aligned) and marches down a chunk of rows, newest ("head") row r, output ("tail")
+// row j = r - 3.  The work of a row is split between two kinds of warps:
+//
+//   X warps (NC/2 threads, TWO adjacent columns per thread) do everything that is local to the head row or
+//   differences along x:  derived quantities, F_x, F_y, the five kappa_x / Phi_x (the |D1| / |D3| windows of
+//   the two interfaces of a pair share their differences and partial maxima, neighbours come in as 128-bit
+//   shared-memory loads), the mixed fluxes G(.;y), C_y = F_y - G.  They own the cp.async input ring and hold
+//   no row history at all.
+//   Y warps (NC threads, one column each) do everything that differences along y or assembles the result:
+//   six-row register histories of rho, vx, vy, eps, bx, the five kappa_y / Phi_y, the mixed fluxes G(.;x),
+//   C_x = F_x - G, the central differences of C_x and C_y, R, the RK combine, the store, the wave-speed maxima.
+//
+// X is a pure producer for Y; the hand-over goes through shared memory: one-row planes UP (derived head row)
+// and PK (Phi_x, kappa_x), and thread-column rings CXR/BYR (F_x -> C_x, by; 5 rows), DXR (Phi_x differences;
+// 4 rows), CYR (C_y; 6 rows).  Two CTA-wide barriers per row (A: UP/CXR published, B: PK/C_x published) order
+// every write against every read (ring depths chosen so that a slot is never rewritten in the barrier
+// interval in which it is read).  12 warps per SM at <= 168 registers instead of 8 at 240.
+#pragma once
+#include "smaug_march_kernel.cuh"
+
+namespace smaug {
+
+template <int NC>
+struct SplitSmem {
+  static constexpr int PW = NC + 8;                     // padded plane width (index c + 4)
+  static constexpr int OFF_UP = 0;                      // 6 planes: rho, vx, vy, eps, by, bx of the head row
+  static constexpr int OFF_PK = OFF_UP + 6 * PW;        // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
+  static constexpr int OFF_CXR = OFF_PK + 7 * PW;       // ring 5 rows x 5 planes: F_x, then C_x
+  static constexpr int OFF_BYR = OFF_CXR + 25 * PW;     // ring 5 rows: by
+  static constexpr int OFF_DXR = OFF_BYR + 5 * NC;      // ring 4 rows x 5: Phi_x differences
+  static constexpr int OFF_CYR = OFF_DXR + 20 * NC;     // ring 6 rows x 5: C_y
+  static constexpr int OFF_INR = OFF_CYR + 30 * NC;     // ring 3 rows x 6: cp.async landing zone (X threads)
+  static constexpr int OFF_RED = OFF_INR + 18 * NC;
+  static constexpr int TOTAL = OFF_RED + 4 * 32;
+  static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
+};
+
+__device__ __forceinline__ void cp_async16(double* smem_dst, const double* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ double2 lds2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void sts2(double* p, double x, double y) { *reinterpret_cast<double2*>(p) = make_double2(x, y); }
+template <int NTHREADS>
+__device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
+
+// the operand of larger magnitude (max and abs are exact, so |amax| chains equal max-of-abs chains bit for bit;
+// the comparisons take |.| as a free source modifier)
+__device__ __forceinline__ double amax(double a, double b) { return fabs(a) > fabs(b) ? a : b; }
+
+// kappa at the TWO adjacent interfaces (u[2] | u[3]) and (u[3] | u[4]) of the seven cells u[0..6] (c-5).
+// d0, d1: the first differences across the two interfaces.
+__device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0, double& k1, double& d0,
+                                       double& d1) {
+  double a[6], t[4];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) a[k] = u[k + 1] - u[k];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) t[k] = fma(3.0, a[k + 1], -(u[k + 3] - u[k]));
+  const double tm = amax(t[1], t[2]);
+  const double am = amax(amax(a[1], a[2]), amax(a[3], a[4]));
+  const double m3_0 = dabs(amax(t[0], tm)), m3_1 = dabs(amax(tm, t[3]));
+  const double m1_0 = dabs(amax(a[0], am)), m1_1 = dabs(amax(am, a[5]));
+  k0 = kappa_ratio(m3_0, m1_0, cv);
+  k1 = kappa_ratio(m3_1, m1_1, cv);
+  d0 = a[2];
+  d1 = a[3];
+}
+
+// kappa at ONE interface from six cells, max chains with free |.| modifiers (same value as kappa6)
+__device__ __forceinline__ double kappa6m(double u0, double u1, double u2, double u3, double u4, double u5,
+                                          double cv, double& d1_mid) {
+  const double a0 = u1 - u0, a1 = u2 - u1, a2 = u3 - u2, a3 = u4 - u3, a4 = u5 - u4;
+  const double t0 = fma(3.0, a1, -(u3 - u0));
+  const double t1 = fma(3.0, a2, -(u4 - u1));
+  const double t2 = fma(3.0, a3, -(u5 - u2));
+  const double m3 = dabs(amax(amax(t0, t1), t2));
+  const double m1 = dabs(amax(amax(amax(a0, a1), amax(a2, a3)), a4));
+  d1_mid = a2;
+  return kappa_ratio(m3, m1, cv);
+}
+
+template <int NC, int COMBINE, int WS>
+__global__ void __launch_bounds__(NC + NC / 2, 1) split_kernel(const StageArgs a, const MarchGeom mg) {
+  using S = SplitSmem<NC>;
+  constexpr int PW = S::PW, NXT = NC / 2, NTH = NC + NC / 2;
+  extern __shared__ __align__(16) double smem[];
+  double* const UP = smem + S::OFF_UP;
+  double* const PK = smem + S::OFF_PK;
+  double* const CXR = smem + S::OFF_CXR;
+  double* const BYR = smem + S::OFF_BYR;
+  double* const DXR = smem + S::OFF_DXR;
+  double* const CYR = smem + S::OFF_CYR;
+  double* const INR = smem + S::OFF_INR;
+  double* const red_sh = smem + S::OFF_RED;
+  const Grid& g = a.g;
+  const int tid = threadIdx.x;
+  constexpr int W = NC - 8;
+  const int x0 = blockIdx.x * W;
+  const int ystart = blockIdx.y * mg.rows_per_cta;
+  const int yend = min(ystart + mg.rows_per_cta, g.ny);
+  double wsmax[4] = {0.0, 0.0, 0.0, 0.0};
+
+  if (tid < NXT) {
+    // =================================================================== X role: columns c0, c0 + 1
+    const int c0 = 2 * tid, tp = c0 + 4;
+    const double gm1 = a.prm.gamma - 1.0;
+    const double vt = sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][2])) +
+                      sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][3]));
+    const double cv_rho = a.prm.c_rho * vt, cv_mom = a.prm.c_mom * vt, cv_e = a.prm.c_e * vt, cv_b = a.prm.c_b * vt;
+    const int gcol = min(x0 - 4 + c0 + XOFF, g.pitch - 2);            // even => 16-byte aligned pairs
+    const long long colbase = (long long)NG * g.pitch + gcol;
+    auto fetch_row = [&](int row, int slot) {
+      const long long ga = colbase + (long long)min(row, g.ny + NG - 1) * g.pitch;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) cp_async16(INR + (slot * NF + f) * NC + c0, a.in.p[f] + ga);
+      cp_async_commit();
+    };
+    fetch_row(ystart - NG, 0);
+    fetch_row(ystart - NG + 1, 1);
+    int s3 = 0, s4 = 0, s5 = 0, s6 = 0;     // ring slots of row r (mod 3, 4, 5, 6)
+
+#pragma unroll 1
+    for (int r = ystart - NG; r < yend + NG; ++r) {
+      cp_async_wait<1>();
+      double rho[2], mx[2], my[2], et[2], bx[2], by[2];
+      {
+        const double* in = INR + s3 * NF * NC + c0;
+        const double2 q0 = lds2(in + F_RHO * NC), q1 = lds2(in + F_MX * NC), q2 = lds2(in + F_MY * NC);
+        const double2 q3 = lds2(in + F_E * NC), q4 = lds2(in + F_BX * NC), q5 = lds2(in + F_BY * NC);
+        rho[0] = q0.x; rho[1] = q0.y; mx[0] = q1.x; mx[1] = q1.y; my[0] = q2.x; my[1] = q2.y;
+        et[0] = q3.x; et[1] = q3.y; bx[0] = q4.x; bx[1] = q4.y; by[0] = q5.x; by[1] = q5.y;
+      }
+      fetch_row(r + 2, s3 >= 1 ? s3 - 1 : 2);             // slot of row r + 2 = slot of row r - 1
+      // ---------------------------------------------------------------- derived quantities, F_x, F_y of row r
+      double vx[2], vy[2], eps[2], cyn[2][5], fx[2][5];
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        const double rr = drcp(rho[q]);
+        vx[q] = mx[q] * rr; vy[q] = my[q] * rr;
+        const double b2h = 0.5 * fma(by[q], by[q], bx[q] * bx[q]);
+        const double ke = 0.5 * fma(my[q], vy[q], mx[q] * vx[q]);
+        eps[q] = (et[q] - ke) - b2h;
+        const double ptt = fma(gm1, eps[q], b2h);
+        const double btv = fma(by[q], vy[q], bx[q] * vx[q]);
+        const double h = et[q] + ptt;
+        cyn[q][C_RHO] = rho[q] * vy[q];
+        cyn[q][C_MX] = fma(mx[q], vy[q], -(bx[q] * by[q]));
+        cyn[q][C_MY] = fma(my[q], vy[q], -(by[q] * by[q])) + ptt;
+        cyn[q][C_E] = fma(vy[q], h, -(by[q] * btv));
+        cyn[q][C_B] = fma(vy[q], bx[q], -(by[q] * vx[q]));
+        fx[q][C_RHO] = rho[q] * vx[q];
+        fx[q][C_MX] = fma(mx[q], vx[q], -(bx[q] * bx[q])) + ptt;
+        fx[q][C_MY] = fma(my[q], vx[q], -(by[q] * bx[q]));
+        fx[q][C_E] = fma(vx[q], h, -(bx[q] * btv));
+        fx[q][C_B] = fma(vx[q], by[q], -(bx[q] * vy[q]));
+      }
+      sts2(UP + 0 * PW + tp, rho[0], rho[1]); sts2(UP + 1 * PW + tp, vx[0], vx[1]);
+      sts2(UP + 2 * PW + tp, vy[0], vy[1]);   sts2(UP + 3 * PW + tp, eps[0], eps[1]);
+      sts2(UP + 4 * PW + tp, by[0], by[1]);   sts2(UP + 5 * PW + tp, bx[0], bx[1]);
+#pragma unroll
+      for (int f = 0; f < 5; ++f) sts2(CXR + (s5 * 5 + f) * PW + tp, fx[0][f], fx[1][f]);
+      sts2(BYR + s5 * NC + c0, by[0], by[1]);
+      cta_barrier<NTH>();                                             // ---- A
+
+      // ---------------------------------------------------------------- x-interfaces (c0|c0+1), (c0+1|c0+2)
+      double px[2][5], kxv[2], kxb[2], dcx_vy[2], dcx_by[2];
+      {
+        double u[7], k0, k1, d0, d1;
+        auto gather = [&](int plane, double o0, double o1) {
+          const double2 l = lds2(UP + plane * PW + tp - 2), rgt = lds2(UP + plane * PW + tp + 2);
+          u[0] = l.x; u[1] = l.y; u[2] = o0; u[3] = o1; u[4] = rgt.x; u[5] = rgt.y;
+          u[6] = UP[plane * PW + tp + 4];
+        };
+        gather(0, rho[0], rho[1]);
+        kappa7(u, cv_rho, k0, k1, d0, d1);
+        const double rbar0 = 0.5 * (u[2] + u[3]), rbar1 = 0.5 * (u[3] + u[4]);
+        px[0][C_RHO] = k0 * d0; px[1][C_RHO] = k1 * d1;
+        gather(1, vx[0], vx[1]);
+        kappa7(u, cv_mom, k0, k1, d0, d1);
+        px[0][C_MX] = (rbar0 * k0) * d0; px[1][C_MX] = (rbar1 * k1) * d1;
+        const double vxbar0 = 0.5 * (u[2] + u[3]), vxbar1 = 0.5 * (u[3] + u[4]);
+        gather(2, vy[0], vy[1]);
+        kappa7(u, cv_mom, kxv[0], kxv[1], d0, d1);
+        px[0][C_MY] = ((0.5 * rbar0) * kxv[0]) * d0; px[1][C_MY] = ((0.5 * rbar1) * kxv[1]) * d1;
+        const double vybar0 = 0.5 * (u[2] + u[3]), vybar1 = 0.5 * (u[3] + u[4]);
+        dcx_vy[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_vy[1] = cd12v(u[1], u[2], u[4], u[5]);
+        gather(3, eps[0], eps[1]);
+        kappa7(u, cv_e, k0, k1, d0, d1);
+        const double p_eps0 = k0 * d0, p_eps1 = k1 * d1;
+        gather(4, by[0], by[1]);
+        kappa7(u, cv_b, kxb[0], kxb[1], d0, d1);
+        px[0][C_B] = kxb[0] * d0; px[1][C_B] = kxb[1] * d1;
+        dcx_by[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_by[1] = cd12v(u[1], u[2], u[4], u[5]);
+        px[0][C_E] = fma(0.5 * (u[2] + u[3]), px[0][C_B], fma(vybar0, px[0][C_MY], fma(vxbar0, px[0][C_MX], p_eps0)));
+        px[1][C_E] = fma(0.5 * (u[3] + u[4]), px[1][C_B], fma(vybar1, px[1][C_MY], fma(vxbar1, px[1][C_MX], p_eps1)));
+      }
+#pragma unroll
+      for (int f = 0; f < 5; ++f) sts2(PK + f * PW + tp, px[0][f], px[1][f]);
+      sts2(PK + 5 * PW + tp, kxv[0], kxv[1]);
+      sts2(PK + 6 * PW + tp, kxb[0], kxb[1]);
+      cta_barrier<NTH>();                                             // ---- B
+
+      // ---------------------------------------------------------------- Phi_x differences, G(.;y), C_y of row r
+      {
+        const double kvl = PK[5 * PW + tp - 1], kbl = PK[6 * PW + tp - 1];
+#pragma unroll
+        for (int f = 0; f < 5; ++f)
+          sts2(DXR + (s4 * 5 + f) * NC + c0, px[0][f] - PK[f * PW + tp - 1], px[1][f] - px[0][f]);
+        const double kv0 = 0.5 * (kvl + kxv[0]), kv1 = 0.5 * (kxv[0] + kxv[1]);
+        const double kb0 = 0.5 * (kbl + kxb[0]), kb1 = 0.5 * (kxb[0] + kxb[1]);
+        const double gm0 = ((0.5 * rho[0]) * kv0) * (dcx_vy[0] * (1.0 / 12.0));      // G(mx ; y)
+        const double gm1_ = ((0.5 * rho[1]) * kv1) * (dcx_vy[1] * (1.0 / 12.0));
+        const double gb0 = -(kb0 * (dcx_by[0] * (1.0 / 12.0)));                       // G(bx ; y)
+        const double gb1 = -(kb1 * (dcx_by[1] * (1.0 / 12.0)));
+        double* cy = CYR + s6 * 5 * NC + c0;
+        sts2(cy + C_RHO * NC, cyn[0][C_RHO], cyn[1][C_RHO]);
+        sts2(cy + C_MX * NC, cyn[0][C_MX] - gm0, cyn[1][C_MX] - gm1_);
+        sts2(cy + C_MY * NC, cyn[0][C_MY], cyn[1][C_MY]);
+        sts2(cy + C_E * NC, cyn[0][C_E] - fma(vx[0], gm0, bx[0] * gb0), cyn[1][C_E] - fma(vx[1], gm1_, bx[1] * gb1));
+        sts2(cy + C_B * NC, cyn[0][C_B] - gb0, cyn[1][C_B] - gb1);
+      }
+      s3 = s3 == 2 ? 0 : s3 + 1;
+      s4 = (s4 + 1) & 3;
+      s5 = s5 == 4 ? 0 : s5 + 1;
+      s6 = s6 == 5 ? 0 : s6 + 1;
+    }
+    cp_async_wait<0>();
+  } else {
+    // =================================================================== Y role: column c
+    const int c = tid - NXT, tp = c + 4;
+    const int ci = x0 - 4 + c;
+    const int cl = min(ci, g.nx + NG - 1);
+    const bool col_out = c >= 4 && c < NC - 4 && ci < g.nx;
+    const double gamma = a.prm.gamma;
+    const double idx_ = a.prm.inv_dx, idy_ = a.prm.inv_dy;
+    const double vt = sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][2])) +
+                      sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][3]));
+    const double cv_rho = a.prm.c_rho * vt, cv_mom = a.prm.c_mom * vt, cv_e = a.prm.c_e * vt, cv_b = a.prm.c_b * vt;
+    const double cdt = a.c * a.sc->dt;
+    const long long colbase = (long long)NG * g.pitch + (cl + XOFF);
+    // six-row histories (index 0 = row r-5 ... 5 = row r)
+    double hr[6], hvx[6], hvy[6], he[6], hbx[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { hr[k] = 1.0; hvx[k] = 0.0; hvy[k] = 0.0; he[k] = 0.0; hbx[k] = 0.0; }
+    double py_prev[5] = {0.0, 0.0, 0.0, 0.0, 0.0};        // Phi_y at interface (j-1 | j)
+    double kyv_prev = 0.0, kyb_prev = 0.0;                 // kappa_y(vx), kappa_y(bx) at (j-1 | j)
+    int s4 = 1, s5 = 2, s6 = 0;                            // slots of row j in DXR, CXR; of row r in CYR
+    // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
+
+#pragma unroll 1
+    for (int r = ystart - NG; r < yend + NG; ++r) {
+      const int j = r - NG;
+      const bool tail_on = j >= ystart;
+      const bool ky_on = r >= ystart + NG - 1;
+      const long long gj = colbase + (long long)max(j, -NG) * g.pitch;
+      // operands of the RK combine for row j: issued here, consumed at the end of the step
+      double jbase[NF], jacc[NF], jin[NF];
+      if (tail_on) {
+        if (COMBINE == COMBINE_FINAL) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
+        } else {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
+          if (COMBINE == COMBINE_ACC) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
+          }
+        }
+      }
+      cta_barrier<NTH>();                                             // ---- A
+#pragma unroll
+      for (int k = 0; k < 5; ++k) { hr[k] = hr[k + 1]; hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; he[k] = he[k + 1]; hbx[k] = hbx[k + 1]; }
+      hr[5] = UP[0 * PW + tp]; hvx[5] = UP[1 * PW + tp]; hvy[5] = UP[2 * PW + tp]; he[5] = UP[3 * PW + tp];
+      hbx[5] = UP[5 * PW + tp];
+
+      // ---------------------------------------------------------------- y-interface (j | j+1)
+      double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      double kyv = 0.0, kyb = 0.0;
+      if (ky_on) {
+        double d_rho, d_vx, d_vy, d_e, d_bx;
+        const double k_rho = kappa6m(hr[0], hr[1], hr[2], hr[3], hr[4], hr[5], cv_rho, d_rho);
+        kyv = kappa6m(hvx[0], hvx[1], hvx[2], hvx[3], hvx[4], hvx[5], cv_mom, d_vx);
+        const double k_vy = kappa6m(hvy[0], hvy[1], hvy[2], hvy[3], hvy[4], hvy[5], cv_mom, d_vy);
+        const double k_e = kappa6m(he[0], he[1], he[2], he[3], he[4], he[5], cv_e, d_e);
+        kyb = kappa6m(hbx[0], hbx[1], hbx[2], hbx[3], hbx[4], hbx[5], cv_b, d_bx);
+        const double rbar = 0.5 * (hr[2] + hr[3]);
+        const double p_rho = k_rho * d_rho;
+        const double p_mx = ((0.5 * rbar) * kyv) * d_vx;
+        const double p_my = (rbar * k_vy) * d_vy;
+        const double p_eps = k_e * d_e;
+        const double p_b = kyb * d_bx;
+        py[C_RHO] = p_rho; py[C_MX] = p_mx; py[C_MY] = p_my; py[C_B] = p_b;
+        py[C_E] = fma(0.5 * (hbx[2] + hbx[3]), p_b,
+                      fma(0.5 * (hvy[2] + hvy[3]), p_my, fma(0.5 * (hvx[2] + hvx[3]), p_mx, p_eps)));
+      }
+      if (tail_on) {
+        // G(my ; x), G(by ; x) and their energy companion at row j (histories index 2); C_x = F_x - G
+        const double kv = 0.5 * (kyv_prev + kyv);
+        const double kb = 0.5 * (kyb_prev + kyb);
+        const double gm = ((0.5 * hr[2]) * kv) * (cd12v(hvx[0], hvx[1], hvx[3], hvx[4]) * (1.0 / 12.0));
+        const double gb = -(kb * (cd12v(hbx[0], hbx[1], hbx[3], hbx[4]) * (1.0 / 12.0)));
+        double* cx = CXR + s5 * 5 * PW + tp;
+        const double jby = BYR[s5 * NC + c];
+        cx[C_MY * PW] = cx[C_MY * PW] - gm;
+        cx[C_E * PW] = cx[C_E * PW] - fma(hvy[2], gm, jby * gb);
+        cx[C_B * PW] = cx[C_B * PW] - gb;
+      }
+      cta_barrier<NTH>();                                             // ---- B
+
+      // ---------------------------------------------------------------- assemble R(j), combine, write
+      if (tail_on) {
+        const double* cx = CXR + s5 * 5 * PW + tp;
+        double R[NF];
+        {
+          double cdx[5];
+#pragma unroll
+          for (int f = 0; f < 5; ++f) cdx[f] = cd12v(cx[f * PW - 2], cx[f * PW - 1], cx[f * PW + 1], cx[f * PW + 2]);
+          // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-6 ring
+          const int jm2 = s6 + 1 >= 6 ? s6 - 5 : s6 + 1, jm1 = s6 + 2 >= 6 ? s6 - 4 : s6 + 2;
+          const int jp1 = s6 + 4 >= 6 ? s6 - 2 : s6 + 4, jp2 = s6 + 5 >= 6 ? s6 - 1 : s6 + 5;
+          double cdy[5];
+#pragma unroll
+          for (int f = 0; f < 5; ++f)
+            cdy[f] = cd12v(CYR[(jm2 * 5 + f) * NC + c], CYR[(jm1 * 5 + f) * NC + c], CYR[(jp1 * 5 + f) * NC + c],
+                           CYR[(jp2 * 5 + f) * NC + c]);
+          R[F_RHO] = fma(cdx[C_RHO], idx_, cdy[C_RHO] * idy_) * (-1.0 / 12.0);
+          R[F_MX] = fma(cdx[C_MX], idx_, cdy[C_MX] * idy_) * (-1.0 / 12.0);
+          R[F_MY] = fma(cdx[C_MY], idx_, cdy[C_MY] * idy_) * (-1.0 / 12.0);
+          R[F_E] = fma(cdx[C_E], idx_, cdy[C_E] * idy_) * (-1.0 / 12.0);
+          R[F_BX] = (cdy[C_B] * idy_) * (-1.0 / 12.0);
+          R[F_BY] = fma(cdx[C_B], idx_, 0.0) * (-1.0 / 12.0);
+        }
+        const double* dx = DXR + s4 * 5 * NC + c;
+        R[F_RHO] = fma(dx[C_RHO * NC], idx_, R[F_RHO]);
+        R[F_MX] = fma(dx[C_MX * NC], idx_, R[F_MX]);
+        R[F_MY] = fma(dx[C_MY * NC], idx_, R[F_MY]);
+        R[F_E] = fma(dx[C_E * NC], idx_, R[F_E]);
+        R[F_BY] = fma(dx[C_B * NC], idx_, R[F_BY]);
+        R[F_RHO] = fma(py[C_RHO] - py_prev[C_RHO], idy_, R[F_RHO]);
+        R[F_MX] = fma(py[C_MX] - py_prev[C_MX], idy_, R[F_MX]);
+        R[F_MY] = fma(py[C_MY] - py_prev[C_MY], idy_, R[F_MY]);
+        R[F_E] = fma(py[C_E] - py_prev[C_E], idy_, R[F_E]);
+        R[F_BX] = fma(py[C_B] - py_prev[C_B], idy_, R[F_BX]);
+
+        double o[NF];
+        if (COMBINE == COMBINE_FINAL) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) o[f] = fma(cdt, R[f], fma(fma(-2.0, jin[f], jacc[f]), 1.0 / 3.0, jin[f]));
+        } else {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) o[f] = fma(cdt, R[f], jbase[f]);
+        }
+        if (col_out && j < yend) {
+          const long long go = (long long)(j + NG) * g.pitch + (ci + XOFF);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) a.out.p[f][go] = o[f];
+          if (COMBINE == COMBINE_ACC) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) a.acc_out.p[f][go] = fma(2.0, o[f], jin[f] - jbase[f]);
+          }
+          if (WS != WS_NONE) {
+            double w4[4];
+            cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, WS == WS_FULL, w4);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) wsmax[k] = dmax(wsmax[k], w4[k]);
+          }
+        }
+      }
+#pragma unroll
+      for (int f = 0; f < 5; ++f) py_prev[f] = py[f];
+      kyv_prev = kyv; kyb_prev = kyb;
+      s4 = (s4 + 1) & 3;
+      s5 = s5 == 4 ? 0 : s5 + 1;
+      s6 = s6 == 5 ? 0 : s6 + 1;
+    }
+  }
+  if (WS != WS_NONE) block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], WS == WS_FULL ? 0 : 2);
+}
+
+}  // namespace smaug

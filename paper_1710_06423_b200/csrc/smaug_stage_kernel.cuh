@@ -113,7 +113,7 @@ __device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, d
   for (int k = 0; k < R; ++k) {
     const double m3 = dmax(dmax(d3[k], d3[k + 1]), d3[k + 2]);
     const double m1 = dmax(dmax(dmax(d1[k], d1[k + 1]), dmax(d1[k + 2], d1[k + 3])), d1[k + 4]);
-    const double r = m1 > 0.0 ? cv * ratio_div(m3, m1) : 0.0;
+    const double r = kappa_ratio(m3, m1, cv);
     if (k < n) out[k * os] = r;
   }
 }

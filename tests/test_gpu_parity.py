@@ -65,8 +65,8 @@ def check(a, ta, wsa, b, tb, wsb, tol=TOL, exact=True):
     return err
 
 
-# sizes span several 32x16 tiles plus ragged tails in both directions
-@pytest.mark.parametrize("nx,ny,steps", [(70, 45, 20), (32, 16, 10), (33, 17, 10), (200, 200, 40)])
+# sizes span several 32x16 tiles / 248-column strips plus ragged tails in both directions
+@pytest.mark.parametrize("nx,ny,steps", [(70, 45, 20), (32, 16, 10), (33, 17, 10), (200, 200, 40), (520, 70, 6)])
 def test_orszag_tang_parity(gpu, oracle_mod, nx, ny, steps):
     w, bc, gamma = si.orszag_tang(nx, ny)
     a = gpu_run(gpu, w, bc, gamma, steps)
@@ -118,7 +118,8 @@ def test_boundary_kinds_with_background(gpu, oracle_mod, bc):
 
 @pytest.mark.parametrize("params", [dict(hd_on=0), dict(rk_order=2), dict(rk_order=1, hd_on=1),
                                     dict(fixed_dt=1e-4), dict(c_rho=0.1, c_mom=0.2, c_e=0.05, c_b=0.3),
-                                    dict(lx=2.0, ly=0.5), dict(kernel=0), dict(kernel=0, rk_order=2)])
+                                    dict(lx=2.0, ly=0.5), dict(kernel=0), dict(kernel=0, rk_order=2),
+                                    dict(kernel=1), dict(kernel=1, rk_order=2), dict(kernel=2, rk_order=1)])
 def test_parameters(gpu, oracle_mod, params):
     w, bc, gamma = si.orszag_tang(64, 48)
     a = gpu_run(gpu, w, bc, gamma, 10, **params)
