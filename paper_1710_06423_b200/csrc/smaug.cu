@@ -203,7 +203,7 @@ int launch_march(smaug_ctx* c, const StageArgs& a) {
 }
 
 #ifndef SMAUG_SPLIT_NC
-#define SMAUG_SPLIT_NC 256
+#define SMAUG_SPLIT_NC 128
 #endif
 constexpr int SPLIT_NC = SMAUG_SPLIT_NC;
 
@@ -235,7 +235,7 @@ int launch_split_t(smaug_ctx* c, const StageArgs& a) {
   const int W = SPLIT_NC - 8;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
-  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm);
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * (SPLIT_NC <= 128 ? 2 : 1));
   const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
   dim3 grid(strips, nchunks);
   c->last_ctas = strips * nchunks;

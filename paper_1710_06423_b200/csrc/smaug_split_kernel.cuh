@@ -9,8 +9,8 @@
 //   X warps (NC/2 threads, TWO adjacent columns per thread) do everything that is local to the head row or
 //   differences along x:  derived quantities, F_x, F_y, the five kappa_x / Phi_x (the |D1| / |D3| windows of
 //   the two interfaces of a pair share their differences and partial maxima, neighbours come in as 128-bit
-//   shared-memory loads), the mixed fluxes G(.;y), C_y = F_y - G.  They own the cp.async input ring and hold
-//   no row history at all.
+//   shared-memory loads), the mixed fluxes G(.;y), C_y = F_y - G.  They read the input rows (128-bit loads, one row
+//   ahead, held in registers) and hold no row history at all.
 //   Y warps (NC threads, one column each) do everything that differences along y or assembles the result:
 //   six-row register histories of rho, vx, vy, eps, bx, the five kappa_y / Phi_y, the mixed fluxes G(.;x),
 //   C_x = F_x - G, the central differences of C_x and C_y, R, the RK combine, the store, the wave-speed maxima.
@@ -34,8 +34,7 @@ struct SplitSmem {
   static constexpr int OFF_BYR = OFF_CXR + 25 * PW;     // ring 5 rows: by
   static constexpr int OFF_DXR = OFF_BYR + 5 * NC;      // ring 4 rows x 5: Phi_x differences
   static constexpr int OFF_CYR = OFF_DXR + 20 * NC;     // ring 6 rows x 5: C_y
-  static constexpr int OFF_INR = OFF_CYR + 30 * NC;     // ring 3 rows x 6: cp.async landing zone (X threads)
-  static constexpr int OFF_RED = OFF_INR + 18 * NC;
+  static constexpr int OFF_RED = OFF_CYR + 30 * NC;
   static constexpr int TOTAL = OFF_RED + 4 * 32;
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
 };
@@ -86,7 +85,7 @@ __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, doubl
 }
 
 template <int NC, int COMBINE, int WS>
-__global__ void __launch_bounds__(NC + NC / 2, 1) split_kernel(const StageArgs a, const MarchGeom mg) {
+__global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(const StageArgs a, const MarchGeom mg) {
   using S = SplitSmem<NC>;
   constexpr int PW = S::PW, NXT = NC / 2, NTH = NC + NC / 2;
   extern __shared__ __align__(16) double smem[];
@@ -96,7 +95,6 @@ __global__ void __launch_bounds__(NC + NC / 2, 1) split_kernel(const StageArgs a
   double* const BYR = smem + S::OFF_BYR;
   double* const DXR = smem + S::OFF_DXR;
   double* const CYR = smem + S::OFF_CYR;
-  double* const INR = smem + S::OFF_INR;
   double* const red_sh = smem + S::OFF_RED;
   const Grid& g = a.g;
   const int tid = threadIdx.x;
@@ -115,28 +113,24 @@ __global__ void __launch_bounds__(NC + NC / 2, 1) split_kernel(const StageArgs a
     const double cv_rho = a.prm.c_rho * vt, cv_mom = a.prm.c_mom * vt, cv_e = a.prm.c_e * vt, cv_b = a.prm.c_b * vt;
     const int gcol = min(x0 - 4 + c0 + XOFF, g.pitch - 2);            // even => 16-byte aligned pairs
     const long long colbase = (long long)NG * g.pitch + gcol;
-    auto fetch_row = [&](int row, int slot) {
+    // the input rows arrive one step ahead as 128-bit loads held in registers (one row step is several
+    // thousand cycles, far above the HBM latency); the state being read is never written by this launch
+    double2 q[NF];
+    auto load_row = [&](int row) {
       const long long ga = colbase + (long long)min(row, g.ny + NG - 1) * g.pitch;
 #pragma unroll
-      for (int f = 0; f < NF; ++f) cp_async16(INR + (slot * NF + f) * NC + c0, a.in.p[f] + ga);
-      cp_async_commit();
+      for (int f = 0; f < NF; ++f) q[f] = __ldg(reinterpret_cast<const double2*>(a.in.p[f] + ga));
     };
-    fetch_row(ystart - NG, 0);
-    fetch_row(ystart - NG + 1, 1);
-    int s3 = 0, s4 = 0, s5 = 0, s6 = 0;     // ring slots of row r (mod 3, 4, 5, 6)
+    load_row(ystart - NG);
+    int s4 = 0, s5 = 0, s6 = 0;     // ring slots of row r (mod 4, 5, 6)
 
 #pragma unroll 1
     for (int r = ystart - NG; r < yend + NG; ++r) {
-      cp_async_wait<1>();
       double rho[2], mx[2], my[2], et[2], bx[2], by[2];
-      {
-        const double* in = INR + s3 * NF * NC + c0;
-        const double2 q0 = lds2(in + F_RHO * NC), q1 = lds2(in + F_MX * NC), q2 = lds2(in + F_MY * NC);
-        const double2 q3 = lds2(in + F_E * NC), q4 = lds2(in + F_BX * NC), q5 = lds2(in + F_BY * NC);
-        rho[0] = q0.x; rho[1] = q0.y; mx[0] = q1.x; mx[1] = q1.y; my[0] = q2.x; my[1] = q2.y;
-        et[0] = q3.x; et[1] = q3.y; bx[0] = q4.x; bx[1] = q4.y; by[0] = q5.x; by[1] = q5.y;
-      }
-      fetch_row(r + 2, s3 >= 1 ? s3 - 1 : 2);             // slot of row r + 2 = slot of row r - 1
+      rho[0] = q[F_RHO].x; rho[1] = q[F_RHO].y; mx[0] = q[F_MX].x; mx[1] = q[F_MX].y;
+      my[0] = q[F_MY].x; my[1] = q[F_MY].y; et[0] = q[F_E].x; et[1] = q[F_E].y;
+      bx[0] = q[F_BX].x; bx[1] = q[F_BX].y; by[0] = q[F_BY].x; by[1] = q[F_BY].y;
+      load_row(r + 1);
       // ---------------------------------------------------------------- derived quantities, F_x, F_y of row r
       double vx[2], vy[2], eps[2], cyn[2][5], fx[2][5];
 #pragma unroll
@@ -225,12 +219,10 @@ __global__ void __launch_bounds__(NC + NC / 2, 1) split_kernel(const StageArgs a
         sts2(cy + C_E * NC, cyn[0][C_E] - fma(vx[0], gm0, bx[0] * gb0), cyn[1][C_E] - fma(vx[1], gm1_, bx[1] * gb1));
         sts2(cy + C_B * NC, cyn[0][C_B] - gb0, cyn[1][C_B] - gb1);
       }
-      s3 = s3 == 2 ? 0 : s3 + 1;
       s4 = (s4 + 1) & 3;
       s5 = s5 == 4 ? 0 : s5 + 1;
       s6 = s6 == 5 ? 0 : s6 + 1;
     }
-    cp_async_wait<0>();
   } else {
     // =================================================================== Y role: column c
     const int c = tid - NXT, tp = c + 4;
@@ -253,7 +245,7 @@ __global__ void __launch_bounds__(NC + NC / 2, 1) split_kernel(const StageArgs a
     int s4 = 1, s5 = 2, s6 = 0;                            // slots of row j in DXR, CXR; of row r in CYR
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
-#pragma unroll 1
+#pragma unroll 2
     for (int r = ystart - NG; r < yend + NG; ++r) {
       const int j = r - NG;
       const bool tail_on = j >= ystart;
