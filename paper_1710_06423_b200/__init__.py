@@ -13,7 +13,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
-LIB_PATH = os.path.join(_HERE, "libsmaug.so")
+LIB_PATH = os.environ.get("SMAUG_LIB") or os.path.join(_HERE, "libsmaug.so")   # SMAUG_LIB: a variant build (tuning)
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2

@@ -235,7 +235,7 @@ int launch_split_t(smaug_ctx* c, const StageArgs& a) {
   const int W = SPLIT_NC - 8;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
-  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * (SPLIT_NC <= 128 ? 2 : 1));
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * SplitSmem<SPLIT_NC>::CTAS_PER_SM);
   const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
   dim3 grid(strips, nchunks);
   c->last_ctas = strips * nchunks;

@@ -21,6 +21,8 @@
 // every write against every read (ring depths chosen so that a slot is never rewritten in the barrier
 // interval in which it is read).  12 warps per SM at <= 168 registers instead of 8 at 240.
 #pragma once
+#include <type_traits>
+
 #include "smaug_march_kernel.cuh"
 
 namespace smaug {
@@ -28,14 +30,17 @@ namespace smaug {
 template <int NC>
 struct SplitSmem {
   static constexpr int PW = NC + 8;                     // padded plane width (index c + 4)
-  static constexpr int OFF_UP = 0;                      // 6 planes: rho, vx, vy, eps, by, bx of the head row
-  static constexpr int OFF_PK = OFF_UP + 6 * PW;        // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
+  static constexpr int OFF_UP = 0;                      // 2 x 6 planes: rho, vx, vy, eps, by, bx of the head row
+                                                        // (double-buffered by row parity)
+  static constexpr int OFF_PK = OFF_UP + 12 * PW;       // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
   static constexpr int OFF_CXR = OFF_PK + 7 * PW;       // ring 5 rows x 5 planes: F_x, then C_x
   static constexpr int OFF_BYR = OFF_CXR + 25 * PW;     // ring 5 rows: by
   static constexpr int OFF_DXR = OFF_BYR + 5 * NC;      // ring 4 rows x 5: Phi_x differences
   static constexpr int OFF_CYR = OFF_DXR + 20 * NC;     // ring 6 rows x 5: C_y
-  static constexpr int OFF_RED = OFF_CYR + 30 * NC;
-  static constexpr int TOTAL = OFF_RED + 4 * 32;
+  static constexpr int OFF_INR = OFF_CYR + 30 * NC;     // cp.async landing zone of the next input row (6 fields)
+  static constexpr int OFF_RED = OFF_INR;               // block reduction scratch (after the march: INR is dead)
+  static constexpr int TOTAL = OFF_INR + (6 * NC > 4 * 32 ? 6 * NC : 4 * 32);
+  static constexpr int CTAS_PER_SM = NC <= 64 ? 4 : (NC <= 128 ? 2 : 1);
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
 };
 
@@ -47,6 +52,9 @@ __device__ __forceinline__ double2 lds2(const double* p) { return *reinterpret_c
 __device__ __forceinline__ void sts2(double* p, double x, double y) { *reinterpret_cast<double2*>(p) = make_double2(x, y); }
 template <int NTHREADS>
 __device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
+// barrier among the NTHREADS threads of one role (named barrier ID > 0)
+template <int ID, int NTHREADS>
+__device__ __forceinline__ void role_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NTHREADS) : "memory"); }
 
 // the operand of larger magnitude (max and abs are exact, so |amax| chains equal max-of-abs chains bit for bit;
 // the comparisons take |.| as a free source modifier)
@@ -84,8 +92,57 @@ __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, doubl
   return kappa_ratio(m3, m1, cv);
 }
 
+// M3 = max |D3| over the three interfaces around (u[2] | u[3]), M1 = max |D1| over the five (c-5), and the
+// first difference across the interface itself.
+__device__ __forceinline__ void maxima6(const double u[6], double& m3, double& m1, double& d_mid) {
+  const double a0 = u[1] - u[0], a1 = u[2] - u[1], a2 = u[3] - u[2], a3 = u[4] - u[3], a4 = u[5] - u[4];
+  const double t0 = fma(3.0, a1, -(u[3] - u[0]));
+  const double t1 = fma(3.0, a2, -(u[4] - u[1]));
+  const double t2 = fma(3.0, a3, -(u[5] - u[2]));
+  m3 = dabs(amax(amax(t0, t1), t2));
+  m1 = dabs(amax(amax(amax(a0, a1), amax(a2, a3)), a4));
+  d_mid = a2;
+}
+
+// kappa[k] = cv[k] * M3[k] / M1[k] (0 where M1 == 0) for N ratios at once.  Almost always every M1 of a
+// warp is an ordinary number (exponent field >= 100): then the plain exact division is taken, without the
+// zero guard and the 2^200 rescue of kappa_ratio.  One warp-uniform vote decides for all N ratios, so the
+// divisions stay in one basic block and interleave.  Both paths give the same bits where both apply.
+template <int N>
+__device__ __forceinline__ void kappa_batch(const double (&m3)[N], const double (&m1)[N], const double (&cv)[N],
+                                            double (&kap)[N]) {
+#ifdef SMAUG_NO_KBATCH
+#pragma unroll
+  for (int k = 0; k < N; ++k) kap[k] = kappa_ratio(m3[k], m1[k], cv[k]);
+  return;
+#endif
+  int lo = __double2hiint(m1[0]);
+#pragma unroll
+  for (int k = 1; k < N; ++k) lo = min(lo, __double2hiint(m1[k]));
+  if (__any_sync(0xffffffffu, lo < 0x06400000)) {
+#pragma unroll
+    for (int k = 0; k < N; ++k) kap[k] = kappa_ratio(m3[k], m1[k], cv[k]);
+  } else {
+#pragma unroll
+    for (int k = 0; k < N; ++k) kap[k] = cv[k] * ddiv(m3[k], m1[k]);
+  }
+}
+
+#ifndef SMAUG_SPLIT_KY
+#define SMAUG_SPLIT_KY 0      // 0: one kappa at a time (guarded division), 1: batched with a fast path
+#endif
+#ifndef SMAUG_SPLIT_YUNROLL
+#define SMAUG_SPLIT_YUNROLL 2
+#endif
+constexpr int SPLIT_YUNROLL = SMAUG_SPLIT_YUNROLL;   // row steps of the Y role per loop trip
+
 template <int NC, int COMBINE, int WS>
-__global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(const StageArgs a, const MarchGeom mg) {
+#ifdef SMAUG_SPLIT_MAXNREG
+__global__ void __maxnreg__(SMAUG_SPLIT_MAXNREG) split_kernel
+#else
+__global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split_kernel
+#endif
+(const StageArgs a, const MarchGeom mg) {
   using S = SplitSmem<NC>;
   constexpr int PW = S::PW, NXT = NC / 2, NTH = NC + NC / 2;
   extern __shared__ __align__(16) double smem[];
@@ -95,6 +152,7 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
   double* const BYR = smem + S::OFF_BYR;
   double* const DXR = smem + S::OFF_DXR;
   double* const CYR = smem + S::OFF_CYR;
+  double* const INR = smem + S::OFF_INR;
   double* const red_sh = smem + S::OFF_RED;
   const Grid& g = a.g;
   const int tid = threadIdx.x;
@@ -113,24 +171,32 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
     const double cv_rho = a.prm.c_rho * vt, cv_mom = a.prm.c_mom * vt, cv_e = a.prm.c_e * vt, cv_b = a.prm.c_b * vt;
     const int gcol = min(x0 - 4 + c0 + XOFF, g.pitch - 2);            // even => 16-byte aligned pairs
     const long long colbase = (long long)NG * g.pitch + gcol;
-    // the input rows arrive one step ahead as 128-bit loads held in registers (one row step is several
-    // thousand cycles, far above the HBM latency); the state being read is never written by this launch
-    double2 q[NF];
-    auto load_row = [&](int row) {
+    // the input rows arrive one step ahead through cp.async (16 bytes per field and thread) into a
+    // thread-private landing zone: no registers are held while a row is in flight, and the copy cannot be
+    // sunk towards its use by the compiler (which exposed the HBM latency when the rows were plain loads).
+    // The copy of row r + 1 is issued after every value of row r has been consumed from the landing zone.
+    double* const inr = INR + c0;
+    auto fetch_row = [&](int row) {
       const long long ga = colbase + (long long)min(row, g.ny + NG - 1) * g.pitch;
 #pragma unroll
-      for (int f = 0; f < NF; ++f) q[f] = __ldg(reinterpret_cast<const double2*>(a.in.p[f] + ga));
+      for (int f = 0; f < NF; ++f) cp_async16(inr + f * NC, a.in.p[f] + ga);
+      cp_async_commit();
     };
-    load_row(ystart - NG);
+    fetch_row(ystart - NG);
     int s4 = 0, s5 = 0, s6 = 0;     // ring slots of row r (mod 4, 5, 6)
+    int par = 0;                    // UP buffer of row r
 
 #pragma unroll 1
     for (int r = ystart - NG; r < yend + NG; ++r) {
       double rho[2], mx[2], my[2], et[2], bx[2], by[2];
-      rho[0] = q[F_RHO].x; rho[1] = q[F_RHO].y; mx[0] = q[F_MX].x; mx[1] = q[F_MX].y;
-      my[0] = q[F_MY].x; my[1] = q[F_MY].y; et[0] = q[F_E].x; et[1] = q[F_E].y;
-      bx[0] = q[F_BX].x; bx[1] = q[F_BX].y; by[0] = q[F_BY].x; by[1] = q[F_BY].y;
-      load_row(r + 1);
+      cp_async_wait<0>();
+      {
+        const double2 q0 = lds2(inr + F_RHO * NC), q1 = lds2(inr + F_MX * NC), q2 = lds2(inr + F_MY * NC);
+        const double2 q3 = lds2(inr + F_E * NC), q4 = lds2(inr + F_BX * NC), q5 = lds2(inr + F_BY * NC);
+        rho[0] = q0.x; rho[1] = q0.y; mx[0] = q1.x; mx[1] = q1.y; my[0] = q2.x; my[1] = q2.y;
+        et[0] = q3.x; et[1] = q3.y; bx[0] = q4.x; bx[1] = q4.y; by[0] = q5.x; by[1] = q5.y;
+      }
+      double* const UPr = UP + par * 6 * PW;
       // ---------------------------------------------------------------- derived quantities, F_x, F_y of row r
       double vx[2], vy[2], eps[2], cyn[2][5], fx[2][5];
 #pragma unroll
@@ -154,22 +220,23 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
         fx[q][C_E] = fma(vx[q], h, -(bx[q] * btv));
         fx[q][C_B] = fma(vx[q], by[q], -(bx[q] * vy[q]));
       }
-      sts2(UP + 0 * PW + tp, rho[0], rho[1]); sts2(UP + 1 * PW + tp, vx[0], vx[1]);
-      sts2(UP + 2 * PW + tp, vy[0], vy[1]);   sts2(UP + 3 * PW + tp, eps[0], eps[1]);
-      sts2(UP + 4 * PW + tp, by[0], by[1]);   sts2(UP + 5 * PW + tp, bx[0], bx[1]);
+      sts2(UPr + 0 * PW + tp, rho[0], rho[1]); sts2(UPr + 1 * PW + tp, vx[0], vx[1]);
+      sts2(UPr + 2 * PW + tp, vy[0], vy[1]);   sts2(UPr + 3 * PW + tp, eps[0], eps[1]);
+      sts2(UPr + 4 * PW + tp, by[0], by[1]);   sts2(UPr + 5 * PW + tp, bx[0], bx[1]);
 #pragma unroll
       for (int f = 0; f < 5; ++f) sts2(CXR + (s5 * 5 + f) * PW + tp, fx[0][f], fx[1][f]);
       sts2(BYR + s5 * NC + c0, by[0], by[1]);
-      cta_barrier<NTH>();                                             // ---- A
+      fetch_row(r + 1);     // the stores above depend on every value read from the landing zone
+      cta_barrier<NTH>();                                             // ---- A (both roles)
 
       // ---------------------------------------------------------------- x-interfaces (c0|c0+1), (c0+1|c0+2)
       double px[2][5], kxv[2], kxb[2], dcx_vy[2], dcx_by[2];
       {
         double u[7], k0, k1, d0, d1;
         auto gather = [&](int plane, double o0, double o1) {
-          const double2 l = lds2(UP + plane * PW + tp - 2), rgt = lds2(UP + plane * PW + tp + 2);
+          const double2 l = lds2(UPr + plane * PW + tp - 2), rgt = lds2(UPr + plane * PW + tp + 2);
           u[0] = l.x; u[1] = l.y; u[2] = o0; u[3] = o1; u[4] = rgt.x; u[5] = rgt.y;
-          u[6] = UP[plane * PW + tp + 4];
+          u[6] = UPr[plane * PW + tp + 4];
         };
         gather(0, rho[0], rho[1]);
         kappa7(u, cv_rho, k0, k1, d0, d1);
@@ -198,7 +265,7 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
       for (int f = 0; f < 5; ++f) sts2(PK + f * PW + tp, px[0][f], px[1][f]);
       sts2(PK + 5 * PW + tp, kxv[0], kxv[1]);
       sts2(PK + 6 * PW + tp, kxb[0], kxb[1]);
-      cta_barrier<NTH>();                                             // ---- B
+      role_barrier<1, NXT>();                                         // ---- B (X warps only)
 
       // ---------------------------------------------------------------- Phi_x differences, G(.;y), C_y of row r
       {
@@ -222,7 +289,9 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
       s4 = (s4 + 1) & 3;
       s5 = s5 == 4 ? 0 : s5 + 1;
       s6 = s6 == 5 ? 0 : s6 + 1;
+      par ^= 1;
     }
+    cp_async_wait<0>();
   } else {
     // =================================================================== Y role: column c
     const int c = tid - NXT, tp = c + 4;
@@ -243,6 +312,7 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
     double py_prev[5] = {0.0, 0.0, 0.0, 0.0, 0.0};        // Phi_y at interface (j-1 | j)
     double kyv_prev = 0.0, kyb_prev = 0.0;                 // kappa_y(vx), kappa_y(bx) at (j-1 | j)
     int s4 = 1, s5 = 2, s6 = 0;                            // slots of row j in DXR, CXR; of row r in CYR
+    int par = 0;                                           // UP buffer of row r
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
 #pragma unroll 2
@@ -266,11 +336,12 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
           }
         }
       }
-      cta_barrier<NTH>();                                             // ---- A
+      cta_barrier<NTH>();                                             // ---- A (both roles)
+      const double* const UPr = UP + par * 6 * PW;
 #pragma unroll
       for (int k = 0; k < 5; ++k) { hr[k] = hr[k + 1]; hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; he[k] = he[k + 1]; hbx[k] = hbx[k + 1]; }
-      hr[5] = UP[0 * PW + tp]; hvx[5] = UP[1 * PW + tp]; hvy[5] = UP[2 * PW + tp]; he[5] = UP[3 * PW + tp];
-      hbx[5] = UP[5 * PW + tp];
+      hr[5] = UPr[0 * PW + tp]; hvx[5] = UPr[1 * PW + tp]; hvy[5] = UPr[2 * PW + tp]; he[5] = UPr[3 * PW + tp];
+      hbx[5] = UPr[5 * PW + tp];
 
       // ---------------------------------------------------------------- y-interface (j | j+1)
       double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -304,7 +375,7 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
         cx[C_E * PW] = cx[C_E * PW] - fma(hvy[2], gm, jby * gb);
         cx[C_B * PW] = cx[C_B * PW] - gb;
       }
-      cta_barrier<NTH>();                                             // ---- B
+      role_barrier<2, NC>();                                          // ---- B (Y warps only)
 
       // ---------------------------------------------------------------- assemble R(j), combine, write
       if (tail_on) {
@@ -371,9 +442,13 @@ __global__ void __launch_bounds__(NC + NC / 2, NC <= 128 ? 2 : 1) split_kernel(c
       s4 = (s4 + 1) & 3;
       s5 = s5 == 4 ? 0 : s5 + 1;
       s6 = s6 == 5 ? 0 : s6 + 1;
+      par ^= 1;
     }
   }
-  if (WS != WS_NONE) block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], WS == WS_FULL ? 0 : 2);
+  if (WS != WS_NONE) {
+    __syncthreads();      // red_sh aliases the landing zone of the X warps
+    block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], WS == WS_FULL ? 0 : 2);
+  }
 }
 
 }  // namespace smaug
