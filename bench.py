@@ -43,6 +43,13 @@ WORKLOADS = {
 # accumulator; stage 4 reads it:  96 + 192 + 144 + 144 = 576 B (SURVEY 8(d) counts 624 for its variant).
 BYTES_PER_CELL_UPDATE = 576.0
 STAGES_PER_STEP = 4
+# Second ceiling, reported beside the HBM roofline: fp64-pipe thread-instructions the
+# split kernel executes per output cell and stage (DFMA + DADD + DMUL + DSETP, static SASS count of the two
+# role loops: 398 per column pair in the X loop + 552 per two rows in the Y loop, times 128/120 for the strip
+# halo), against 64 fp64 lanes per SM and clock.
+FP64_INSTR_PER_CELL_STAGE = (398 / 2 + 552 / 2) * 128 / 120
+FP64_LANES_PER_SM = 64
+N_SM = 148
 METRIC = "fp64 MHD cell-updates/s"
 UNIT = "cell-updates/s"
 
@@ -249,10 +256,15 @@ def run_ours(args):
             "hbm_gbs_algorithmic": value / world * BYTES_PER_CELL_UPDATE / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": (achieved / peak) if achieved else None, "traffic": ncu_traffic(name),
-                         "peak_source": peak_src, "kernel": "smaug::march_kernel<256> (fused RK stage)",
+                         "peak_source": peak_src, "kernel": f"smaug::{sim.kernel_name()} (fused RK stage)",
                          "bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_launch_ms,
                          "launches_timed": stage_n, "stage_kernel_share_of_step": stage_ms / ms,
                          "launch": info},
+            "fp64_pipe": ({"achieved": FP64_INSTR_PER_CELL_STAGE * cells / (avg_launch_ms * 1e-3) / 1e12,
+                           "peak": N_SM * FP64_LANES_PER_SM * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12,
+                           "unit": "T fp64-instr/s", "instr_per_cell_stage": FP64_INSTR_PER_CELL_STAGE,
+                           "note": "secondary ceiling; only meaningful for split_kernel<128>"}
+                          if stage_n else None),
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
                     "d2h_bytes_per_step": state_bytes / K,
                     "note": "smaug_set_state(host) + smaug_step(K) + smaug_get_state(host), pinned host memory"},
@@ -260,6 +272,8 @@ def run_ours(args):
             "clocks": clocks,
             "sim": {"t": t_sim, "last_dt": dt_last, "finite": finite},
         }
+        if line["fp64_pipe"]:
+            line["fp64_pipe"]["frac"] = line["fp64_pipe"]["achieved"] / line["fp64_pipe"]["peak"]
         if not args.no_cpu_baseline and world == 1:
             n_s, steps_s = 1000, 6
             rate, el = oracle_rate(n_s, steps_s, threads=1)

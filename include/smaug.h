@@ -113,6 +113,11 @@ int smaug_get_launch_count(smaug_ctx* ctx, long long* n);
  * its strip width as tile_w and 1 as tile_h (it marches row by row). */
 int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
 
+/* Name of the fused stage kernel the context's current parameters select (static string, never NULL;
+ * "?" for a NULL context): "split_kernel<128>" (role-split streaming form), "march_kernel<256>"
+ * (single-role streaming form) or "stage_kernel<32,16,512>" (tiled form: background and/or no hyperdiffusion). */
+const char* smaug_get_kernel_name(smaug_ctx* ctx);
+
 /* Device time, in milliseconds, spent in the fused stage kernels (summed over launches) and the number of
  * those launches, measured with CUDA events on the context's stream when enabled with
  * smaug_set_kernel_timing(ctx, 1).  Reading synchronises the stream.  */

@@ -70,6 +70,8 @@ def lib() -> C.CDLL:
         L.smaug_get_wavespeeds.argtypes = [vp, dp]
         L.smaug_get_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.smaug_get_kernel_info.argtypes = [vp, C.POINTER(C.c_int)]
+        L.smaug_get_kernel_name.argtypes = [vp]
+        L.smaug_get_kernel_name.restype = C.c_char_p
         L.smaug_set_kernel_timing.argtypes = [vp, C.c_int]
         L.smaug_get_kernel_timing.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.smaug_destroy.argtypes = [vp]
@@ -170,6 +172,9 @@ class Smaug:
         o = (C.c_int * 5)()
         _check(lib().smaug_get_kernel_info(self._h, o))
         return dict(tile_w=o[0], tile_h=o[1], threads=o[2], smem_bytes=o[3], ctas=o[4])
+
+    def kernel_name(self):
+        return lib().smaug_get_kernel_name(self._h).decode()
 
     def set_kernel_timing(self, on=True):
         _check(lib().smaug_set_kernel_timing(self._h, int(on)))

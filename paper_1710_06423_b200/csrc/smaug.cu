@@ -377,6 +377,8 @@ int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], con
   if (!bc) return fail(SMAUG_EINVAL, "bc is NULL");
   if (nx < 1 || ny < 1) return fail(SMAUG_EINVAL, "nx and ny must be >= 1");
   if (!(gamma > 1.0)) return fail(SMAUG_EINVAL, "gamma must be > 1");
+  if (((long long)nx + XOFF + NG + 15) * ((long long)ny + 2 * NG) >= (1LL << 31))
+    return fail(SMAUG_EINVAL, "grid too large: a padded plane must have fewer than 2^31 cells");
   for (int s = 0; s < 4; ++s)
     if (bc[s] < 0 || bc[s] > 2) return fail(SMAUG_EINVAL, "unknown boundary kind");
   for (int ax = 0; ax < 2; ++ax)
@@ -568,6 +570,13 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   }
   out[4] = c->last_ctas;
   return SMAUG_OK;
+}
+
+const char* smaug_get_kernel_name(smaug_ctx* c) {
+  if (!c) return "?";
+  if (!c->has_bg && c->hd_on && c->kernel_mode == 2) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
+  if (!c->has_bg && c->hd_on && c->kernel_mode == 1) return "march_kernel<256>";
+  return "stage_kernel<32,16,512>";
 }
 
 int smaug_set_kernel_timing(smaug_ctx* c, int on) {

@@ -60,10 +60,26 @@ __device__ __forceinline__ void role_barrier() { asm volatile("bar.sync %0, %1;"
 // the comparisons take |.| as a free source modifier)
 __device__ __forceinline__ double amax(double a, double b) { return fabs(a) > fabs(b) ? a : b; }
 
+// kappa = cv * M3 / M1 in two forms with the same bits wherever both apply (c-5):
+//   GUARD = true : kappa_ratio -- zero guard and the 2^200 rescue for tiny / denormal M1;
+//   GUARD = false: the plain exact division, valid when M1 is an ordinary number (exponent field >= 100);
+//                  `lo` collects the smallest high word of the M1 seen, so that the caller can tell afterwards
+//                  whether every ratio of the row step was ordinary.  Where M1 is not, the unguarded result is
+//                  garbage (possibly NaN) and the caller recomputes the whole section with GUARD = true:
+//                  speculate on the common case, keep every division of a step in one basic block.
+template <bool GUARD>
+__device__ __forceinline__ double kappa_q(double m3, double m1, double cv, int& lo) {
+  if (GUARD) return kappa_ratio(m3, m1, cv);
+  lo = min(lo, __double2hiint(m1));
+  return cv * ddiv(m3, m1);
+}
+constexpr int ORDINARY_HI = 0x06400000;     // high word of 2^-923: below it ratio_div rescales
+
 // kappa at the TWO adjacent interfaces (u[2] | u[3]) and (u[3] | u[4]) of the seven cells u[0..6] (c-5).
 // d0, d1: the first differences across the two interfaces.
+template <bool GUARD>
 __device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0, double& k1, double& d0,
-                                       double& d1) {
+                                       double& d1, int& lo) {
   double a[6], t[4];
 #pragma unroll
   for (int k = 0; k < 6; ++k) a[k] = u[k + 1] - u[k];
@@ -73,15 +89,16 @@ __device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0,
   const double am = amax(amax(a[1], a[2]), amax(a[3], a[4]));
   const double m3_0 = dabs(amax(t[0], tm)), m3_1 = dabs(amax(tm, t[3]));
   const double m1_0 = dabs(amax(a[0], am)), m1_1 = dabs(amax(am, a[5]));
-  k0 = kappa_ratio(m3_0, m1_0, cv);
-  k1 = kappa_ratio(m3_1, m1_1, cv);
+  k0 = kappa_q<GUARD>(m3_0, m1_0, cv, lo);
+  k1 = kappa_q<GUARD>(m3_1, m1_1, cv, lo);
   d0 = a[2];
   d1 = a[3];
 }
 
 // kappa at ONE interface from six cells, max chains with free |.| modifiers (same value as kappa6)
+template <bool GUARD>
 __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, double u3, double u4, double u5,
-                                          double cv, double& d1_mid) {
+                                          double cv, double& d1_mid, int& lo) {
   const double a0 = u1 - u0, a1 = u2 - u1, a2 = u3 - u2, a3 = u4 - u3, a4 = u5 - u4;
   const double t0 = fma(3.0, a1, -(u3 - u0));
   const double t1 = fma(3.0, a2, -(u4 - u1));
@@ -89,7 +106,7 @@ __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, doubl
   const double m3 = dabs(amax(amax(t0, t1), t2));
   const double m1 = dabs(amax(amax(amax(a0, a1), amax(a2, a3)), a4));
   d1_mid = a2;
-  return kappa_ratio(m3, m1, cv);
+  return kappa_q<GUARD>(m3, m1, cv, lo);
 }
 
 // M3 = max |D3| over the three interfaces around (u[2] | u[3]), M1 = max |D1| over the five (c-5), and the
@@ -128,6 +145,13 @@ __device__ __forceinline__ void kappa_batch(const double (&m3)[N], const double 
   }
 }
 
+#ifndef SMAUG_SPLIT_LATELOAD
+#define SMAUG_SPLIT_LATELOAD 0   // RK operands of the tail row: 0 loaded at the top of the step, 1 after barrier B,
+#endif                           // 2 after barrier B with an L2 prefetch at the top
+__device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+#ifndef SMAUG_SPLIT_SPEC
+#define SMAUG_SPLIT_SPEC 0
+#endif
 #ifndef SMAUG_SPLIT_KY
 #define SMAUG_SPLIT_KY 0      // 0: one kappa at a time (guarded division), 1: batched with a fast path
 #endif
@@ -231,7 +255,9 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
 
       // ---------------------------------------------------------------- x-interfaces (c0|c0+1), (c0+1|c0+2)
       double px[2][5], kxv[2], kxb[2], dcx_vy[2], dcx_by[2];
-      {
+      auto x_interfaces = [&](auto GUARD_) {
+        constexpr bool GUARD = decltype(GUARD_)::value;
+        int lo = 0x7fffffff;
         double u[7], k0, k1, d0, d1;
         auto gather = [&](int plane, double o0, double o1) {
           const double2 l = lds2(UPr + plane * PW + tp - 2), rgt = lds2(UPr + plane * PW + tp + 2);
@@ -239,28 +265,36 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           u[6] = UPr[plane * PW + tp + 4];
         };
         gather(0, rho[0], rho[1]);
-        kappa7(u, cv_rho, k0, k1, d0, d1);
+        kappa7<GUARD>(u, cv_rho, k0, k1, d0, d1, lo);
         const double rbar0 = 0.5 * (u[2] + u[3]), rbar1 = 0.5 * (u[3] + u[4]);
         px[0][C_RHO] = k0 * d0; px[1][C_RHO] = k1 * d1;
         gather(1, vx[0], vx[1]);
-        kappa7(u, cv_mom, k0, k1, d0, d1);
+        kappa7<GUARD>(u, cv_mom, k0, k1, d0, d1, lo);
         px[0][C_MX] = (rbar0 * k0) * d0; px[1][C_MX] = (rbar1 * k1) * d1;
         const double vxbar0 = 0.5 * (u[2] + u[3]), vxbar1 = 0.5 * (u[3] + u[4]);
         gather(2, vy[0], vy[1]);
-        kappa7(u, cv_mom, kxv[0], kxv[1], d0, d1);
+        kappa7<GUARD>(u, cv_mom, kxv[0], kxv[1], d0, d1, lo);
         px[0][C_MY] = ((0.5 * rbar0) * kxv[0]) * d0; px[1][C_MY] = ((0.5 * rbar1) * kxv[1]) * d1;
         const double vybar0 = 0.5 * (u[2] + u[3]), vybar1 = 0.5 * (u[3] + u[4]);
         dcx_vy[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_vy[1] = cd12v(u[1], u[2], u[4], u[5]);
         gather(3, eps[0], eps[1]);
-        kappa7(u, cv_e, k0, k1, d0, d1);
+        kappa7<GUARD>(u, cv_e, k0, k1, d0, d1, lo);
         const double p_eps0 = k0 * d0, p_eps1 = k1 * d1;
         gather(4, by[0], by[1]);
-        kappa7(u, cv_b, kxb[0], kxb[1], d0, d1);
+        kappa7<GUARD>(u, cv_b, kxb[0], kxb[1], d0, d1, lo);
         px[0][C_B] = kxb[0] * d0; px[1][C_B] = kxb[1] * d1;
         dcx_by[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_by[1] = cd12v(u[1], u[2], u[4], u[5]);
         px[0][C_E] = fma(0.5 * (u[2] + u[3]), px[0][C_B], fma(vybar0, px[0][C_MY], fma(vxbar0, px[0][C_MX], p_eps0)));
         px[1][C_E] = fma(0.5 * (u[3] + u[4]), px[1][C_B], fma(vybar1, px[1][C_MY], fma(vxbar1, px[1][C_MX], p_eps1)));
-      }
+        return lo;
+      };
+      // SMAUG_SPLIT_SPEC: speculate that every M1 of this warp's row step is an ordinary number and redo the
+      // section otherwise (measured slower on B200: 3.87 vs 3.57 ms per stage at 8000^2 -- larger loop bodies)
+#if SMAUG_SPLIT_SPEC
+      if (__any_sync(0xffffffffu, x_interfaces(std::false_type{}) < ORDINARY_HI)) x_interfaces(std::true_type{});
+#else
+      x_interfaces(std::true_type{});
+#endif
 #pragma unroll
       for (int f = 0; f < 5; ++f) sts2(PK + f * PW + tp, px[0][f], px[1][f]);
       sts2(PK + 5 * PW + tp, kxv[0], kxv[1]);
@@ -304,7 +338,10 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
                       sqrt(__longlong_as_double((long long)a.sc->red[a.red_in][3]));
     const double cv_rho = a.prm.c_rho * vt, cv_mom = a.prm.c_mom * vt, cv_e = a.prm.c_e * vt, cv_b = a.prm.c_b * vt;
     const double cdt = a.c * a.sc->dt;
-    const long long colbase = (long long)NG * g.pitch + (cl + XOFF);
+    // element offset of (cl, row j) inside a plane, advanced by one row per step (a plane has fewer than
+    // 2^31 elements: smaug_create checks); rows above the chunk are never dereferenced
+    unsigned gj = (unsigned)(ystart + NG) * (unsigned)g.pitch + (unsigned)(cl + XOFF);
+    const unsigned upitch = (unsigned)g.pitch;
     // six-row histories (index 0 = row r-5 ... 5 = row r)
     double hr[6], hvx[6], hvy[6], he[6], hbx[6];
 #pragma unroll
@@ -315,14 +352,14 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
     int par = 0;                                           // UP buffer of row r
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
-#pragma unroll 2
+#pragma unroll SPLIT_YUNROLL
     for (int r = ystart - NG; r < yend + NG; ++r) {
       const int j = r - NG;
       const bool tail_on = j >= ystart;
       const bool ky_on = r >= ystart + NG - 1;
-      const long long gj = colbase + (long long)max(j, -NG) * g.pitch;
       // operands of the RK combine for row j: issued here, consumed at the end of the step
       double jbase[NF], jacc[NF], jin[NF];
+#if SMAUG_SPLIT_LATELOAD == 0
       if (tail_on) {
         if (COMBINE == COMBINE_FINAL) {
 #pragma unroll
@@ -336,6 +373,21 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           }
         }
       }
+#elif SMAUG_SPLIT_LATELOAD == 2
+      if (tail_on) {     // bring the lines into L2; the loads themselves are issued after barrier B
+        if (COMBINE == COMBINE_FINAL) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) { prefetch_l2(a.in.p[f] + gj); prefetch_l2(a.acc_in.p[f] + gj); }
+        } else {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) prefetch_l2(a.base.p[f] + gj);
+          if (COMBINE == COMBINE_ACC) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) prefetch_l2(a.in.p[f] + gj);
+          }
+        }
+      }
+#endif
       cta_barrier<NTH>();                                             // ---- A (both roles)
       const double* const UPr = UP + par * 6 * PW;
 #pragma unroll
@@ -346,13 +398,15 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       // ---------------------------------------------------------------- y-interface (j | j+1)
       double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       double kyv = 0.0, kyb = 0.0;
-      if (ky_on) {
+      auto y_interface = [&](auto GUARD_) {
+        constexpr bool GUARD = decltype(GUARD_)::value;
+        int lo = 0x7fffffff;
         double d_rho, d_vx, d_vy, d_e, d_bx;
-        const double k_rho = kappa6m(hr[0], hr[1], hr[2], hr[3], hr[4], hr[5], cv_rho, d_rho);
-        kyv = kappa6m(hvx[0], hvx[1], hvx[2], hvx[3], hvx[4], hvx[5], cv_mom, d_vx);
-        const double k_vy = kappa6m(hvy[0], hvy[1], hvy[2], hvy[3], hvy[4], hvy[5], cv_mom, d_vy);
-        const double k_e = kappa6m(he[0], he[1], he[2], he[3], he[4], he[5], cv_e, d_e);
-        kyb = kappa6m(hbx[0], hbx[1], hbx[2], hbx[3], hbx[4], hbx[5], cv_b, d_bx);
+        const double k_rho = kappa6m<GUARD>(hr[0], hr[1], hr[2], hr[3], hr[4], hr[5], cv_rho, d_rho, lo);
+        kyv = kappa6m<GUARD>(hvx[0], hvx[1], hvx[2], hvx[3], hvx[4], hvx[5], cv_mom, d_vx, lo);
+        const double k_vy = kappa6m<GUARD>(hvy[0], hvy[1], hvy[2], hvy[3], hvy[4], hvy[5], cv_mom, d_vy, lo);
+        const double k_e = kappa6m<GUARD>(he[0], he[1], he[2], he[3], he[4], he[5], cv_e, d_e, lo);
+        kyb = kappa6m<GUARD>(hbx[0], hbx[1], hbx[2], hbx[3], hbx[4], hbx[5], cv_b, d_bx, lo);
         const double rbar = 0.5 * (hr[2] + hr[3]);
         const double p_rho = k_rho * d_rho;
         const double p_mx = ((0.5 * rbar) * kyv) * d_vx;
@@ -362,6 +416,14 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         py[C_RHO] = p_rho; py[C_MX] = p_mx; py[C_MY] = p_my; py[C_B] = p_b;
         py[C_E] = fma(0.5 * (hbx[2] + hbx[3]), p_b,
                       fma(0.5 * (hvy[2] + hvy[3]), p_my, fma(0.5 * (hvx[2] + hvx[3]), p_mx, p_eps)));
+        return lo;
+      };
+      if (ky_on) {
+#if SMAUG_SPLIT_SPEC
+        if (__any_sync(0xffffffffu, y_interface(std::false_type{}) < ORDINARY_HI)) y_interface(std::true_type{});
+#else
+        y_interface(std::true_type{});
+#endif
       }
       if (tail_on) {
         // G(my ; x), G(by ; x) and their energy companion at row j (histories index 2); C_x = F_x - G
@@ -379,6 +441,19 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
 
       // ---------------------------------------------------------------- assemble R(j), combine, write
       if (tail_on) {
+#if SMAUG_SPLIT_LATELOAD != 0
+        if (COMBINE == COMBINE_FINAL) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
+        } else {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
+          if (COMBINE == COMBINE_ACC) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
+          }
+        }
+#endif
         const double* cx = CXR + s5 * 5 * PW + tp;
         double R[NF];
         {
@@ -421,7 +496,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           for (int f = 0; f < NF; ++f) o[f] = fma(cdt, R[f], jbase[f]);
         }
         if (col_out && j < yend) {
-          const long long go = (long long)(j + NG) * g.pitch + (ci + XOFF);
+          const unsigned go = gj;      // an output column has cl == ci
 #pragma unroll
           for (int f = 0; f < NF; ++f) a.out.p[f][go] = o[f];
           if (COMBINE == COMBINE_ACC) {
@@ -439,6 +514,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
 #pragma unroll
       for (int f = 0; f < 5; ++f) py_prev[f] = py[f];
       kyv_prev = kyv; kyb_prev = kyb;
+      if (tail_on) gj += upitch;
       s4 = (s4 + 1) & 3;
       s5 = s5 == 4 ? 0 : s5 + 1;
       s6 = s6 == 5 ? 0 : s6 + 1;
