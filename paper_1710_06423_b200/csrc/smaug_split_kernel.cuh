@@ -25,19 +25,29 @@
 
 #include "smaug_march_kernel.cuh"
 
+#ifndef SMAUG_SPLIT_DECOUPLE
+#define SMAUG_SPLIT_DECOUPLE 1
+#endif
+
 namespace smaug {
 
 template <int NC>
 struct SplitSmem {
   static constexpr int PW = NC + 8;                     // padded plane width (index c + 4)
-  static constexpr int OFF_UP = 0;                      // 2 x 6 planes: rho, vx, vy, eps, by, bx of the head row
-                                                        // (double-buffered by row parity)
-  static constexpr int OFF_PK = OFF_UP + 12 * PW;       // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
+  // DEC (SMAUG_SPLIT_DECOUPLE): the X warps may run one row ahead of the Y warps (producer / consumer
+  // barriers instead of the CTA-wide barrier A); the rings X writes after barrier B are one row deeper then,
+  // and UP is single-buffered (X waits until Y has read it).
+  static constexpr bool DEC = SMAUG_SPLIT_DECOUPLE != 0;
+  static constexpr int NUP = DEC ? 1 : 2;               // UP buffers
+  static constexpr int ND = DEC ? 5 : 4;                // rows in DXR
+  static constexpr int NY = DEC ? 7 : 6;                // rows in CYR
+  static constexpr int OFF_UP = 0;                      // NUP x 6 planes: rho, vx, vy, eps, by, bx of the head row
+  static constexpr int OFF_PK = OFF_UP + NUP * 6 * PW;  // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
   static constexpr int OFF_CXR = OFF_PK + 7 * PW;       // ring 5 rows x 5 planes: F_x, then C_x
   static constexpr int OFF_BYR = OFF_CXR + 25 * PW;     // ring 5 rows: by
-  static constexpr int OFF_DXR = OFF_BYR + 5 * NC;      // ring 4 rows x 5: Phi_x differences
-  static constexpr int OFF_CYR = OFF_DXR + 20 * NC;     // ring 6 rows x 5: C_y
-  static constexpr int OFF_INR = OFF_CYR + 30 * NC;     // cp.async landing zone of the next input row (6 fields)
+  static constexpr int OFF_DXR = OFF_BYR + 5 * NC;      // ring ND rows x 5: Phi_x differences
+  static constexpr int OFF_CYR = OFF_DXR + ND * 5 * NC; // ring NY rows x 5: C_y
+  static constexpr int OFF_INR = OFF_CYR + NY * 5 * NC; // cp.async landing zone of the next input row (6 fields)
   static constexpr int OFF_RED = OFF_INR;               // block reduction scratch (after the march: INR is dead)
   static constexpr int TOTAL = OFF_INR + (6 * NC > 4 * 32 ? 6 * NC : 4 * 32);
   static constexpr int CTAS_PER_SM = NC <= 64 ? 4 : (NC <= 128 ? 2 : 1);
@@ -52,6 +62,9 @@ __device__ __forceinline__ double2 lds2(const double* p) { return *reinterpret_c
 __device__ __forceinline__ void sts2(double* p, double x, double y) { *reinterpret_cast<double2*>(p) = make_double2(x, y); }
 template <int NTHREADS>
 __device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 0, %0;" ::"n"(NTHREADS) : "memory"); }
+// producer / consumer halves of a named barrier over NTHREADS threads: the arriving threads do not wait
+template <int ID, int NTHREADS>
+__device__ __forceinline__ void bar_arrive() { asm volatile("bar.arrive %0, %1;" ::"n"(ID), "n"(NTHREADS) : "memory"); }
 // barrier among the NTHREADS threads of one role (named barrier ID > 0)
 template <int ID, int NTHREADS>
 __device__ __forceinline__ void role_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NTHREADS) : "memory"); }
@@ -207,8 +220,10 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       cp_async_commit();
     };
     fetch_row(ystart - NG);
-    int s4 = 0, s5 = 0, s6 = 0;     // ring slots of row r (mod 4, 5, 6)
+    int s4 = 0, s5 = 0, s6 = 0;     // ring slots of row r (mod ND, 5, NY)
     int par = 0;                    // UP buffer of row r
+    constexpr bool DEC = S::DEC;
+    constexpr int ND = S::ND, NY = S::NY;
 
 #pragma unroll 1
     for (int r = ystart - NG; r < yend + NG; ++r) {
@@ -244,6 +259,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         fx[q][C_E] = fma(vx[q], h, -(bx[q] * btv));
         fx[q][C_B] = fma(vx[q], by[q], -(bx[q] * vy[q]));
       }
+      if (DEC) role_barrier<4, NTH>();      // ---- E: every warp is done with UP of the previous row
       sts2(UPr + 0 * PW + tp, rho[0], rho[1]); sts2(UPr + 1 * PW + tp, vx[0], vx[1]);
       sts2(UPr + 2 * PW + tp, vy[0], vy[1]);   sts2(UPr + 3 * PW + tp, eps[0], eps[1]);
       sts2(UPr + 4 * PW + tp, by[0], by[1]);   sts2(UPr + 5 * PW + tp, bx[0], bx[1]);
@@ -251,7 +267,12 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       for (int f = 0; f < 5; ++f) sts2(CXR + (s5 * 5 + f) * PW + tp, fx[0][f], fx[1][f]);
       sts2(BYR + s5 * NC + c0, by[0], by[1]);
       fetch_row(r + 1);     // the stores above depend on every value read from the landing zone
-      cta_barrier<NTH>();                                             // ---- A (both roles)
+      if (DEC) {
+        bar_arrive<3, NTH>();                                         // ---- F: head row published for Y
+        role_barrier<5, NXT>();                                       // ---- A among the X warps
+      } else {
+        cta_barrier<NTH>();                                           // ---- A (both roles)
+      }
 
       // ---------------------------------------------------------------- x-interfaces (c0|c0+1), (c0+1|c0+2)
       double px[2][5], kxv[2], kxb[2], dcx_vy[2], dcx_by[2];
@@ -320,10 +341,10 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         sts2(cy + C_E * NC, cyn[0][C_E] - fma(vx[0], gm0, bx[0] * gb0), cyn[1][C_E] - fma(vx[1], gm1_, bx[1] * gb1));
         sts2(cy + C_B * NC, cyn[0][C_B] - gb0, cyn[1][C_B] - gb1);
       }
-      s4 = (s4 + 1) & 3;
+      s4 = s4 == ND - 1 ? 0 : s4 + 1;
       s5 = s5 == 4 ? 0 : s5 + 1;
-      s6 = s6 == 5 ? 0 : s6 + 1;
-      par ^= 1;
+      s6 = s6 == NY - 1 ? 0 : s6 + 1;
+      if (!DEC) par ^= 1;
     }
     cp_async_wait<0>();
   } else {
@@ -348,8 +369,11 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
     for (int k = 0; k < 6; ++k) { hr[k] = 1.0; hvx[k] = 0.0; hvy[k] = 0.0; he[k] = 0.0; hbx[k] = 0.0; }
     double py_prev[5] = {0.0, 0.0, 0.0, 0.0, 0.0};        // Phi_y at interface (j-1 | j)
     double kyv_prev = 0.0, kyb_prev = 0.0;                 // kappa_y(vx), kappa_y(bx) at (j-1 | j)
-    int s4 = 1, s5 = 2, s6 = 0;                            // slots of row j in DXR, CXR; of row r in CYR
+    constexpr bool DEC = S::DEC;
+    constexpr int ND = S::ND, NY = S::NY;
+    int s4 = ND - 3, s5 = 2, s6 = 0;                       // slots of row j in DXR, CXR; of row r in CYR
     int par = 0;                                           // UP buffer of row r
+    if (DEC) bar_arrive<4, NTH>();                         // E for the first row: nothing to wait for
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
 #pragma unroll SPLIT_YUNROLL
@@ -388,12 +412,18 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         }
       }
 #endif
-      cta_barrier<NTH>();                                             // ---- A (both roles)
+      if (DEC) role_barrier<3, NTH>();                                // ---- F: head row r is published
+      else cta_barrier<NTH>();                                        // ---- A (both roles)
       const double* const UPr = UP + par * 6 * PW;
 #pragma unroll
       for (int k = 0; k < 5; ++k) { hr[k] = hr[k + 1]; hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; he[k] = he[k + 1]; hbx[k] = hbx[k + 1]; }
       hr[5] = UPr[0 * PW + tp]; hvx[5] = UPr[1 * PW + tp]; hvy[5] = UPr[2 * PW + tp]; he[5] = UPr[3 * PW + tp];
       hbx[5] = UPr[5 * PW + tp];
+      if (DEC) {
+        // E: UP may be overwritten (the loads above must have landed: consume them first)
+        asm volatile("" ::"d"(hr[5]), "d"(hvx[5]), "d"(hvy[5]), "d"(he[5]), "d"(hbx[5]) : "memory");
+        if (r + 1 < yend + NG) bar_arrive<4, NTH>();
+      }
 
       // ---------------------------------------------------------------- y-interface (j | j+1)
       double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -460,9 +490,9 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           double cdx[5];
 #pragma unroll
           for (int f = 0; f < 5; ++f) cdx[f] = cd12v(cx[f * PW - 2], cx[f * PW - 1], cx[f * PW + 1], cx[f * PW + 2]);
-          // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-6 ring
-          const int jm2 = s6 + 1 >= 6 ? s6 - 5 : s6 + 1, jm1 = s6 + 2 >= 6 ? s6 - 4 : s6 + 2;
-          const int jp1 = s6 + 4 >= 6 ? s6 - 2 : s6 + 4, jp2 = s6 + 5 >= 6 ? s6 - 1 : s6 + 5;
+          // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-NY ring
+          auto back = [&](int k) { const int q = s6 + (NY - k); return q >= NY ? q - NY : q; };   // slot of row r - k
+          const int jm2 = back(5), jm1 = back(4), jp1 = back(2), jp2 = back(1);
           double cdy[5];
 #pragma unroll
           for (int f = 0; f < 5; ++f)
@@ -515,10 +545,10 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       for (int f = 0; f < 5; ++f) py_prev[f] = py[f];
       kyv_prev = kyv; kyb_prev = kyb;
       if (tail_on) gj += upitch;
-      s4 = (s4 + 1) & 3;
+      s4 = s4 == ND - 1 ? 0 : s4 + 1;
       s5 = s5 == 4 ? 0 : s5 + 1;
-      s6 = s6 == 5 ? 0 : s6 + 1;
-      par ^= 1;
+      s6 = s6 == NY - 1 ? 0 : s6 + 1;
+      if (!DEC) par ^= 1;
     }
   }
   if (WS != WS_NONE) {
