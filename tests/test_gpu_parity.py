@@ -183,3 +183,42 @@ def test_full_config2_properties_after_200_steps(gpu):
     assert np.abs(out - sign * out[:, ::-1, ::-1]).max() <= 1e-11 * np.abs(out).max()
     drift = np.abs(out.reshape(6, -1).sum(1) - w.reshape(6, -1).sum(1)) / np.abs(w).reshape(6, -1).sum(1)
     assert (drift < 1e-12).all(), drift
+
+
+@pytest.mark.parametrize("n,steps", [(2044, 3), (4000, 2)])
+def test_full_size_configs_3_4_sampled_steps(gpu, oracle_mod, n, steps):
+    """Orszag-Tang 2044^2 and 4000^2 (BASELINE.json configs 3 and 4; 2044 = 17 strips of 120 columns + a
+    ragged 4-column tail): a few full steps against the oracle on every cell."""
+    w, bc, gamma = si.orszag_tang(n)
+    a = gpu_run(gpu, w, bc, gamma, steps)
+    b = cpu_run(oracle_mod, w, bc, gamma, steps, threads=16)
+    check(*a, *b)
+
+
+def test_bench_config_8000_two_kernels_and_properties(gpu):
+    """Orszag-Tang 8000 x 8000 (config 5, the workload and launch configuration bench.py times).  The oracle
+    needs ~11 GB and minutes for it, so the full-size check is (i) bit-equality of the role-split streaming
+    kernel (the one bench.py times) with the tiled kernel -- an independently written implementation of the
+    same contract that the tests above pin to the oracle cell by cell -- and (ii) the properties that hold at
+    any size: P3 (180-degree point symmetry of a symmetrised initial state) and P2 (conservation)."""
+    import torch
+    n, steps = 8000, 2
+    w, bc, gamma = si.orszag_tang(n, symmetrise=True)
+    wt = torch.from_numpy(w)
+    outs = []
+    for kernel in (2, 0):
+        s = gpu.Smaug(n, n, gamma, bc, kernel=kernel)
+        s.set_state(wt)
+        s.step(steps, 0.3)
+        if kernel == 2:
+            assert s.kernel_name().startswith("split_kernel") and s.kernel_info()["ctas"] >= 2 * 148
+        outs.append((s.get_state(), s.time(), s.wavespeeds()))
+        s.close()
+    (a, ta, wsa), (b, tb, wsb) = outs
+    assert torch.equal(a, b) and ta == tb and list(wsa) == list(wsb)
+    assert bool(torch.isfinite(a).all())
+    sign = torch.tensor([1, -1, -1, 1, -1, -1.0], dtype=torch.float64, device=a.device)[:, None, None]
+    assert float((a - sign * torch.flip(a, (1, 2))).abs().max()) <= 1e-11 * float(a.abs().max())
+    w_dev = wt.to(a.device)
+    drift = (a.reshape(6, -1).sum(1) - w_dev.reshape(6, -1).sum(1)).abs() / w_dev.abs().reshape(6, -1).sum(1)
+    assert bool((drift < 1e-12).all()), drift
