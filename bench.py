@@ -201,7 +201,7 @@ def run_ours(args):
     w_host = torch.from_numpy(w_np).pin_memory()
     out_host = torch.empty_like(w_host).pin_memory()
     del w_np
-    sim = pkg.Smaug(nx, ny, gamma, bc, device=dev)
+    sim = pkg.Smaug(nx, ny, gamma, bc, device=dev, hd_on=0 if args.no_hd else 1)
     sim.set_state(w_host)
 
     K, W = args.steps, args.warmup
@@ -249,7 +249,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": True, "rk_order": 4,
+            "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": 4,
                        "background": "zero", "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "working set >> L2, no flush needed" if cells * 48 > 4e8 else
                              "working set comparable to L2 (126 MB): DRAM traffic is below algorithmic"},
@@ -264,7 +264,7 @@ def run_ours(args):
                            "peak": N_SM * FP64_LANES_PER_SM * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12,
                            "unit": "T fp64-instr/s", "instr_per_cell_stage": FP64_INSTR_PER_CELL_STAGE,
                            "note": "secondary ceiling; only meaningful for split_kernel<128>"}
-                          if stage_n else None),
+                          if stage_n and not args.no_hd else None),
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
                     "d2h_bytes_per_step": state_bytes / K,
                     "note": "smaug_set_state(host) + smaug_step(K) + smaug_get_state(host), pinned host memory"},
@@ -295,6 +295,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="orszag_tang_8000", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-hd", action="store_true",
+                    help="hyperdiffusion off (the 'Without HD' column of the paper's Table 1); extra row, not the default")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -12,7 +12,7 @@
 #include <string>
 #include <vector>
 
-#include "smaug_split_kernel.cuh"
+#include "smaug_flux_kernel.cuh"
 
 using namespace smaug;
 
@@ -209,7 +209,7 @@ constexpr int SPLIT_NC = SMAUG_SPLIT_NC;
 
 // Chunk height of a streaming kernel: every CTA costs (rows + 6) row steps and CTAs run in waves of n_sm,
 // so pick the chunk count that minimises waves * (rows + 6).
-int pick_rows_per_cta(int ny, int strips, int n_sm) {
+int pick_rows_per_cta(int ny, int strips, int n_sm, int warm_rows = 2 * NG) {
   int best_rows = ny;
   long long best_cost = -1;
   for (int k = 1; k <= 64; ++k) {
@@ -217,7 +217,7 @@ int pick_rows_per_cta(int ny, int strips, int n_sm) {
     int rows = std::max(std::min(ny, 16), (ny + nch - 1) / nch);
     nch = (ny + rows - 1) / rows;
     const long long waves = ((long long)strips * nch + n_sm - 1) / n_sm;
-    const long long cost = waves * (rows + 2 * NG);
+    const long long cost = waves * (rows + warm_rows);
     if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_rows = rows; }
   }
   return best_rows;
@@ -261,7 +261,44 @@ int launch_split(smaug_ctx* c, const StageArgs& a) {
   return fail(SMAUG_EINVAL, "split kernel: unsupported combine / wave-speed mode");
 }
 
+#ifndef SMAUG_FLUX_NT
+#define SMAUG_FLUX_NT 128
+#endif
+constexpr int FLUX_NT = SMAUG_FLUX_NT;
+
+// Streaming form without hyperdiffusion (smaug_flux_kernel.cuh): no background, HD off.
+int launch_flux(smaug_ctx* c, const StageArgs& a) {
+  static bool configured = false;
+  constexpr size_t smem = FluxSmem<FLUX_NT>::BYTES;
+  auto kern = flux_kernel<FLUX_NT>;
+  if (!configured) {
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  const int W = FLUX_NT - 4;
+  const int strips = (c->g.nx + W - 1) / W;
+  MarchGeom mg;
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * FluxSmem<FLUX_NT>::CTAS_PER_SM, 4);
+  const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
+  dim3 grid(strips, nchunks);
+  c->last_ctas = strips * nchunks;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing && c->ev_used + 2 <= c->ev.size()) {
+    e0 = c->ev[c->ev_used++];
+    e1 = c->ev[c->ev_used++];
+    CU(cudaEventRecord(e0, c->stream));
+  }
+  kern<<<grid, FLUX_NT, smem, c->stream>>>(a, mg);
+  if (e1) CU(cudaEventRecord(e1, c->stream));
+  c->launches++;
+  CU(cudaGetLastError());
+  return SMAUG_OK;
+}
+
+bool uses_flux(const smaug_ctx* c) { return !c->has_bg && !c->hd_on && c->kernel_mode != 0; }
+
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
+  if (uses_flux(c)) return launch_flux(c, a);
   if (!c->has_bg && c->hd_on && c->kernel_mode == 2) return launch_split(c, a);
   if (!c->has_bg && c->hd_on && c->kernel_mode == 1) return launch_march(c, a);
   if (c->has_bg) return c->hd_on ? launch_stage_t<true, true>(c, a) : launch_stage_t<true, false>(c, a);
@@ -558,7 +595,10 @@ int smaug_get_launch_count(smaug_ctx* c, long long* n) {
 int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (int rc = check_ctx(c)) return rc;
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
-  if (!c->has_bg && c->hd_on && c->kernel_mode == 2) {   // role-split streaming kernel: a strip of NC-8 columns
+  if (uses_flux(c)) {                                      // streaming kernel without HD: a strip of NT-4 columns
+    out[0] = FLUX_NT - 4; out[1] = 1; out[2] = FLUX_NT;
+    out[3] = (int)FluxSmem<FLUX_NT>::BYTES;
+  } else if (!c->has_bg && c->hd_on && c->kernel_mode == 2) {   // role-split streaming kernel: a strip of NC-8 columns
     out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
     out[3] = (int)SplitSmem<SPLIT_NC>::BYTES;
   } else if (!c->has_bg && c->hd_on && c->kernel_mode == 1) {   // streaming kernel: a strip of NT-6 columns
@@ -574,6 +614,7 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
 
 const char* smaug_get_kernel_name(smaug_ctx* c) {
   if (!c) return "?";
+  if (uses_flux(c)) return FLUX_NT == 128 ? "flux_kernel<128>" : "flux_kernel";
   if (!c->has_bg && c->hd_on && c->kernel_mode == 2) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
   if (!c->has_bg && c->hd_on && c->kernel_mode == 1) return "march_kernel<256>";
   return "stage_kernel<32,16,512>";

@@ -1,0 +1,180 @@
+// smaug_flux_kernel.cuh -- streaming fused stage kernel for the case WITHOUT hyperdiffusion and without a
+// background ("Without HD" column of the paper's Table 1): R = -(d^c_x F_x + d^c_y F_y),
+// RK combine, wave-speed maxima.  About 90 fp64 operations against 144 bytes per cell and stage: this case
+// sits on the memory side of the B200 ridge, so the kernel is built around bytes in flight, not arithmetic.
+// Same arithmetic contract as every other stage kernel: bit-identical to the oracle.
+//
+// One CTA owns a strip of NT - 4 output columns (thread t <-> column x0 - 2 + t) and marches down a chunk of
+// rows, newest ("head") row r, output ("tail") row j = r - 2:
+//   head: derived quantities of row r; F_x(r) -> shared-memory ring (4 rows); F_y(r) -> five-row register history
+//   -- one __syncthreads per row --
+//   tail: central x-difference of F_x(j) from the ring (neighbour columns), central y-difference of F_y from
+//         the history, R, RK combine, coalesced store, wave-speed maxima.
+// Input rows arrive DEPTH - 1 rows ahead through cp.async into a thread-private ring (no registers held, about
+// 3 x 48 bytes per thread in flight); the RK operands of the tail row are plain loads issued at the top of the
+// step.  Nothing is read twice from HBM: the 4 halo columns of a strip and the 4 warm-up rows of a chunk hit L2.
+#pragma once
+#include "smaug_split_kernel.cuh"
+
+namespace smaug {
+
+template <int NT>
+struct FluxSmem {
+  static constexpr int DEPTH = 4;                         // input rows in the landing ring
+  static constexpr int OFF_FXR = 0;                       // ring 4 rows x 5 planes: F_x
+  static constexpr int OFF_INR = OFF_FXR + 4 * 5 * NT;    // ring DEPTH rows x 6 fields: cp.async landing zone
+  static constexpr int OFF_RED = OFF_INR + DEPTH * NF * NT;
+  static constexpr int TOTAL = OFF_RED + 4 * 32;
+  static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
+  static constexpr int CTAS_PER_SM = NT <= 128 ? 4 : 2;
+};
+
+template <int NT>
+__global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(const StageArgs a, const MarchGeom mg) {
+  using S = FluxSmem<NT>;
+  constexpr int DEPTH = S::DEPTH;
+  extern __shared__ __align__(16) double smem[];
+  double* const FXR = smem + S::OFF_FXR;
+  double* const INR = smem + S::OFF_INR;
+  double* const red_sh = smem + S::OFF_RED;
+  const Grid& g = a.g;
+  const int tid = threadIdx.x;
+  constexpr int W = NT - 4;
+  const int x0 = blockIdx.x * W;
+  const int ci = x0 - 2 + tid;                            // interior column of this thread (>= -2: a ghost)
+  const int cl = min(ci, g.nx + NG - 1);                  // clamped for loads
+  const bool col_out = tid >= 2 && tid < NT - 2 && ci < g.nx;
+  const int ystart = blockIdx.y * mg.rows_per_cta;
+  const int yend = min(ystart + mg.rows_per_cta, g.ny);
+  const double gm1 = a.prm.gamma - 1.0, gamma = a.prm.gamma;
+  const double idx_ = a.prm.inv_dx, idy_ = a.prm.inv_dy;
+  const double cdt = a.c * a.sc->dt;
+  const int combine = a.combine, ws_mode = a.ws_mode;
+  const unsigned upitch = (unsigned)g.pitch;
+  // element offsets inside a plane (fewer than 2^31 elements: smaug_create checks)
+  unsigned gin = (unsigned)(ystart - 2 + NG) * upitch + (unsigned)(cl + XOFF);     // (cl, next row to fetch)
+  unsigned gj = (unsigned)(ystart + NG) * upitch + (unsigned)(cl + XOFF);           // (cl, tail row j)
+  int fetched = ystart - 2;                               // next row to fetch
+  const int last_row = g.ny + NG - 1;
+  int slot_f = 0;                                         // landing slot of the next row to fetch
+  auto fetch_row = [&]() {
+    double* dst = INR + slot_f * NF * NT + tid;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) cp_async8(dst + f * NT, a.in.p[f] + gin);
+    cp_async_commit();
+    if (fetched < last_row) gin += upitch;                // rows below the padded plane are never dereferenced
+    ++fetched;
+    slot_f = slot_f == DEPTH - 1 ? 0 : slot_f + 1;
+  };
+#pragma unroll
+  for (int k = 0; k < DEPTH - 1; ++k) fetch_row();
+  int slot_r = 0;                                         // landing slot of row r
+  int s4 = 0;                                             // FXR slot of row r (mod 4)
+
+  double fy[5][5];                                        // F_y of rows r-4 .. r (index 4 = row r)
+#pragma unroll
+  for (int k = 0; k < 5; ++k)
+#pragma unroll
+    for (int f = 0; f < 5; ++f) fy[k][f] = 0.0;
+  double wsmax[4] = {0.0, 0.0, 0.0, 0.0};
+
+#pragma unroll 1
+  for (int r = ystart - 2; r < yend + 2; ++r) {
+    const bool tail_on = r >= ystart + 2;                 // uniform over the CTA
+    // operands of the RK combine for row j: issued here, consumed at the end of the step
+    double jbase[NF], jacc[NF], jin[NF];
+    if (tail_on) {
+      if (combine == COMBINE_FINAL) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
+      } else {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
+        if (combine == COMBINE_ACC) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
+        }
+      }
+    }
+    cp_async_wait<DEPTH - 2>();                           // row r has landed (later rows may be in flight)
+    const double* src = INR + slot_r * NF * NT + tid;
+    const double rho = src[F_RHO * NT], mx = src[F_MX * NT], my = src[F_MY * NT];
+    const double et = src[F_E * NT], bx = src[F_BX * NT], by = src[F_BY * NT];
+    fetch_row();                                          // into the slot read one step ago
+    slot_r = slot_r == DEPTH - 1 ? 0 : slot_r + 1;
+
+    // ------------------------------------------------------------------ head: derived quantities, F_x, F_y of row r
+    const double rr = drcp(rho);
+    const double vx = mx * rr, vy = my * rr;
+    const double b2h = 0.5 * fma(by, by, bx * bx);
+    const double ke = 0.5 * fma(my, vy, mx * vx);
+    const double eps = (et - ke) - b2h;
+    const double ptt = fma(gm1, eps, b2h);
+    const double btv = fma(by, vy, bx * vx);
+    const double h = et + ptt;
+    double* fxw = FXR + s4 * 5 * NT + tid;
+    fxw[C_RHO * NT] = rho * vx;
+    fxw[C_MX * NT] = fma(mx, vx, -(bx * bx)) + ptt;
+    fxw[C_MY * NT] = fma(my, vx, -(by * bx));
+    fxw[C_E * NT] = fma(vx, h, -(bx * btv));
+    fxw[C_B * NT] = fma(vx, by, -(bx * vy));
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+      for (int f = 0; f < 5; ++f) fy[k][f] = fy[k + 1][f];
+    fy[4][C_RHO] = rho * vy;
+    fy[4][C_MX] = fma(mx, vy, -(bx * by));
+    fy[4][C_MY] = fma(my, vy, -(by * by)) + ptt;
+    fy[4][C_E] = fma(vy, h, -(by * btv));
+    fy[4][C_B] = fma(vy, bx, -(by * vx));
+    __syncthreads();
+
+    // ------------------------------------------------------------------ tail: R(j), combine, write
+    if (tail_on) {
+      const int sj = (s4 + 2) & 3;                        // FXR slot of row j = r - 2
+      const int tl = min(max(tid, 2), NT - 3);            // halo threads read in range; their result is unused
+      const double* fxr = FXR + sj * 5 * NT + tl;
+      double R[NF];
+      double cdx[5], cdy[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        cdx[f] = cd12v(fxr[f * NT - 2], fxr[f * NT - 1], fxr[f * NT + 1], fxr[f * NT + 2]);
+        cdy[f] = cd12v(fy[0][f], fy[1][f], fy[3][f], fy[4][f]);
+      }
+      R[F_RHO] = fma(cdx[C_RHO], idx_, cdy[C_RHO] * idy_) * (-1.0 / 12.0);
+      R[F_MX] = fma(cdx[C_MX], idx_, cdy[C_MX] * idy_) * (-1.0 / 12.0);
+      R[F_MY] = fma(cdx[C_MY], idx_, cdy[C_MY] * idy_) * (-1.0 / 12.0);
+      R[F_E] = fma(cdx[C_E], idx_, cdy[C_E] * idy_) * (-1.0 / 12.0);
+      R[F_BX] = (cdy[C_B] * idy_) * (-1.0 / 12.0);        // F_x(bx) == 0
+      R[F_BY] = fma(cdx[C_B], idx_, 0.0) * (-1.0 / 12.0); // F_y(by) == 0
+      double o[NF];
+      if (combine == COMBINE_FINAL) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) o[f] = fma(cdt, R[f], fma(fma(-2.0, jin[f], jacc[f]), 1.0 / 3.0, jin[f]));
+      } else {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) o[f] = fma(cdt, R[f], jbase[f]);
+      }
+      if (col_out) {            // then cl == ci: gj is the address of the output cell as well
+#pragma unroll
+        for (int f = 0; f < NF; ++f) a.out.p[f][gj] = o[f];
+        if (combine == COMBINE_ACC) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) a.acc_out.p[f][gj] = fma(2.0, o[f], jin[f] - jbase[f]);
+        }
+        if (ws_mode != WS_NONE) {
+          double w4[4];
+          cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, ws_mode == WS_FULL, w4);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) wsmax[k] = dmax(wsmax[k], w4[k]);
+        }
+      }
+      gj += upitch;
+    }
+    s4 = (s4 + 1) & 3;
+  }
+  cp_async_wait<0>();
+  if (ws_mode != WS_NONE) block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], ws_mode == WS_FULL ? 0 : 2);
+}
+
+}  // namespace smaug

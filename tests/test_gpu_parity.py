@@ -127,6 +127,29 @@ def test_parameters(gpu, oracle_mod, params):
     check(*a, *b)
 
 
+@pytest.mark.parametrize("nx,ny,steps,params", [(300, 130, 12, dict(hd_on=0)), (125, 9, 8, dict(hd_on=0, rk_order=2)),
+                                                (3, 40, 5, dict(hd_on=0, rk_order=1)),
+                                                (130, 300, 6, dict(hd_on=0, kernel=0))])
+def test_no_hyperdiffusion_streaming_kernel(gpu, oracle_mod, nx, ny, steps, params):
+    """HD off, no background: flux_kernel (strips of 124 columns + ragged tails, several row chunks)."""
+    w, bc, gamma = si.orszag_tang(nx, ny)
+    a = gpu_run(gpu, w, bc, gamma, steps, **params)
+    b = cpu_run(oracle_mod, w, bc, gamma, steps, **params)
+    check(*a, *b)
+
+
+def test_no_hyperdiffusion_open_and_fixed_boundaries(gpu, oracle_mod):
+    w, bc, gamma = si.brio_wu(200, 12)
+    a = gpu_run(gpu, w, bc, gamma, 40, hd_on=0, cfl=0.2)
+    b = cpu_run(oracle_mod, w, bc, gamma, 40, hd_on=0, cfl=0.2)
+    check(*a, *b)
+    w, _, gamma = si.smooth_random(90, 70, seed=11, amp=2e-2)
+    for bc in [(2, 2, 1, 1), (1, 2, 0, 0)]:
+        a = gpu_run(gpu, w, bc, gamma, 10, hd_on=0)
+        b = cpu_run(oracle_mod, w, bc, gamma, 10, hd_on=0)
+        check(*a, *b)
+
+
 def test_uniform_state_preserved_bitwise_on_gpu(gpu):
     nx, ny, gamma = 40, 20, 5.0 / 3.0
     w = si.prim_to_cons(0.3, 0.7, -0.4, 0.2, 0.5, -0.25, gamma)[:, None, None] * np.ones((1, ny, nx))
