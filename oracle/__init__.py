@@ -19,6 +19,7 @@ _LIB = os.path.join(_HERE, "liboracle_smaug.so")
 
 BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2
 (P_LX, P_LY, P_HD_ON, P_C_RHO, P_C_MOM, P_C_E, P_C_B, P_RK_ORDER, P_FIXED_DT) = range(9)
+P_GX, P_GY = 10, 11
 ENONFINITE = -4
 
 _lib = None
@@ -103,7 +104,7 @@ class Oracle:
             self.set_param(k, v)
 
     _KEYS = dict(lx=P_LX, ly=P_LY, hd_on=P_HD_ON, c_rho=P_C_RHO, c_mom=P_C_MOM, c_e=P_C_E, c_b=P_C_B,
-                 rk_order=P_RK_ORDER, fixed_dt=P_FIXED_DT)
+                 rk_order=P_RK_ORDER, fixed_dt=P_FIXED_DT, gx=P_GX, gy=P_GY)
 
     def set_param(self, key, value):
         k = self._KEYS[key] if isinstance(key, str) else int(key)

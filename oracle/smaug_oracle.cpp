@@ -15,6 +15,8 @@
 //   hyper_div              P1, P2 (conservation incl. energy couplings), P3, P5 (x<->y transposition)
 //   wavespeeds / dt        P11 (closed-form Brio-Wu and Orszag-Tang maxima and dt0)
 //   rk4_step               P6 (temporal order 4), P4 (RK4 amplification factor), P12 (restart)
+//   gravity (c-10)         G1 (hydrostatic background stays exactly static), G2 (free fall: closed form),
+//                          G3 (hydrostatic balance of PAPER.md:35 to 4th order), G4 (split == unsplit, 4th order)
 // "Parity unpinned" against the SAC/SMAUG codes themselves: the paper prints no field values and its
 // figures are not in the container.
 //
@@ -40,7 +42,7 @@ enum { BC_PERIODIC = 0, BC_OPEN = 1, BC_FIXED = 2 };
 enum { SIDE_XLO = 0, SIDE_XHI = 1, SIDE_YLO = 2, SIDE_YHI = 3 };
 enum {
   P_LX = 0, P_LY = 1, P_HD_ON = 2, P_C_RHO = 3, P_C_MOM = 4, P_C_E = 5, P_C_B = 6, P_RK_ORDER = 7,
-  P_FIXED_DT = 8
+  P_FIXED_DT = 8, P_GX = 10, P_GY = 11   // (9 is the CUDA library's kernel selector; unused here)
 };
 enum { OK = 0, EINVAL_ = -1, ENOMEM_ = -2, ECUDA_ = -3, ENONFINITE_ = -4 };
 
@@ -55,6 +57,7 @@ struct Ctx {
   double c_rho = 0.02, c_mom = 0.4, c_e = 0.02, c_b = 0.02;
   int rk_order = 4;
   double fixed_dt = 0.0;
+  double gx = 0.0, gy = 0.0;     // uniform gravitational acceleration g, c-10
   Plane bg[NBG];
   Plane w[NF];
   double t = 0.0, last_dt = 0.0;
@@ -376,7 +379,7 @@ void rhs(const Ctx& c, const Plane* w, Plane* R) {
         R[f][q] = fma(cd12(Cx, q, 1), inv_dx, cd12(Cy, q, (size_t)c.NX) * inv_dy) * (-1.0 / 12.0);
       }
   }
-  // c-2 energy source (zero when the background is zero; gravity absent):
+  // c-2 energy source (zero when the background is zero; gravity: c-10 below):
   //   S_e = -p_tb (dvx/dx + dvy/dy) + sum_{k,l} B_b,k B_b,l d_k v_l,  p_tb = (gamma-1)(e_b - B_b^2/2) + B_b^2/2
   const double gm1 = c.gamma - 1.0;
 #pragma omp parallel for num_threads(c.nthreads) schedule(static)
@@ -394,6 +397,24 @@ void rhs(const Ctx& c, const Plane* w, Plane* R) {
                            fma(bby * bby, dyvy, fma(bbx * bby, dxvy + dyvx, (bbx * bbx) * dxvx)));
       R[F_E][q] = R[F_E][q] + S;
     }
+  // c-10 gravity ("rho g" in the momentum equation, "rho g.v" in the energy equation), in the
+  // split form: the background is taken to be in magneto-hydrostatic balance,
+  //   grad p_tb - (B_b.grad) B_b = rho_b g,
+  // so the background part of "rho g" cancels the background pressure gradient and the background part of
+  // "rho g.v" cancels v.grad p_tb (which is how S_e above arises); what is left acts on the PERTURBED density:
+  //   S(m) = rho~ g,   S(e~) = rho~ (g.v)        [g uniform; with a zero background rho~ = rho: PAPER.md:35 as printed]
+  // Applied only when g != 0 (fma(x, 0, -0.0) would turn a -0 into +0).
+  if (c.gx != 0.0 || c.gy != 0.0) {
+#pragma omp parallel for num_threads(c.nthreads) schedule(static)
+    for (int j = 0; j < c.ny; ++j)
+      for (int i = 0; i < c.nx; ++i) {
+        const size_t q = c.at(i, j);
+        const double rt = w[F_RHO][q];
+        R[F_MX][q] = fma(rt, c.gx, R[F_MX][q]);
+        R[F_MY][q] = fma(rt, c.gy, R[F_MY][q]);
+        R[F_E][q] = fma(rt, fma(c.gy, d.vy[q], c.gx * d.vx[q]), R[F_E][q]);
+      }
+  }
   // c-5 interface fluxes, x then y
   if (c.hd_on) {
 #pragma omp parallel for num_threads(c.nthreads) schedule(static)
@@ -543,6 +564,8 @@ int oracle_set_param(oracle_ctx* p, int key, double v) {
     case P_C_B: if (!(v >= 0)) break; c.c_b = v; return OK;
     case P_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c.rk_order = (int)v; return OK;
     case P_FIXED_DT: if (!(v >= 0)) break; c.fixed_dt = v; return OK;
+    case P_GX: if (!std::isfinite(v)) break; c.gx = v; return OK;
+    case P_GY: if (!std::isfinite(v)) break; c.gy = v; return OK;
     default: g_err = "unknown parameter key"; return EINVAL_;
   }
   g_err = "parameter value out of range";

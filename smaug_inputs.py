@@ -106,6 +106,39 @@ def uniform_background(nx: int, ny: int, rho_b: float, e_b: float, bx_b: float, 
     return bg
 
 
+def stratified_atmosphere(nx: int, ny: int, gamma: float = 5.0 / 3.0, g: float = 1.0, scale_height: float = 0.25,
+                          rho0: float = 1.0, by0: float = 0.3, pulse: float = 1e-2, split: bool = True):
+    """A gravitationally stratified, magnetised atmosphere with a wave-driving pulse (the use the paper
+    states for the code): isothermal hydrostatic column rho_b = rho0 exp(-y/H),
+    p_b = rho_b g H under g = (0, -g), uniform vertical field B_b = (0, by0) (force-free, so the balance
+    grad p_tb - (B_b.grad)B_b = rho_b g holds analytically), e_b = p_b/(gamma-1) + by0^2/2; on top a
+    Gaussian velocity/pressure pulse of relative amplitude `pulse` centred at (0.5, 0.3).  Periodic in x,
+    open in y.  split=True: returns the perturbation w on the background bg; split=False: the same total
+    state as a perturbation on a zero background (bg = None).
+    Returns (w, bc, gamma, bg, (gx, gy))."""
+    x = centres(nx)[None, :] * np.ones((ny, 1))
+    y = centres(ny)[:, None] * np.ones((1, nx))
+    H = scale_height
+    rho_b = rho0 * np.exp(-y / H)
+    p_b = rho_b * g * H
+    e_b = p_b / (gamma - 1.0) + 0.5 * by0 * by0
+    bump = np.exp(-((x - 0.5) ** 2 + (y - 0.3) ** 2) / (2 * 0.05 ** 2))
+    vy = pulse * bump
+    vx = 0.5 * pulse * bump * np.sin(2 * np.pi * x)
+    p = p_b * (1.0 + pulse * bump)
+    rho = rho_b * (1.0 + 0.5 * pulse * bump)
+    tot = prim_to_cons(rho, vx, vy, p, np.zeros_like(x), by0 * np.ones_like(x), gamma)
+    bc = (BC_PERIODIC, BC_PERIODIC, BC_OPEN, BC_OPEN)
+    if not split:
+        return tot, bc, gamma, None, (0.0, -g)
+    bg = np.ascontiguousarray(np.stack([rho_b, e_b, np.zeros_like(x), by0 * np.ones_like(x)]))
+    w = tot.copy()
+    w[0] -= rho_b
+    w[3] -= e_b
+    w[5] -= by0
+    return np.ascontiguousarray(w), bc, gamma, bg, (0.0, -g)
+
+
 def rel_l2(a: np.ndarray, ref: np.ndarray) -> np.ndarray:
     """c-9 error metric per field: ||a_f - ref_f||_2 / ||ref_f||_2; where the denominator is 0 the
     numerator is divided by max_f ||ref_f||_2 instead."""
