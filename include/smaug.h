@@ -10,6 +10,7 @@
  *   - the Runge-Kutta stage updates (classical RK4; 2 = midpoint, 1 = Euler)              PAPER.md:45,    c-6
  *   - ghost-cell (halo) fill, periodic / open / fixed, in device memory                   PAPER.md:59,101, c-8
  *   - the max-wavespeed reduction and the CFL time step                                   PAPER.md:45,    c-4, c-7
+ *   - uniform gravity acting on the perturbed density (stratified backgrounds)           PAPER.md:35,    c-10
  * Every step of that path runs in hand-written fp64 CUDA kernels for sm_100a; there is no CPU fallback
  * (every entry point fails with SMAUG_ECUDA when no CUDA device is usable).
  *
@@ -58,9 +59,14 @@ enum { /* keys of smaug_set_param */
   SMAUG_PARAM_C_B = 6,      /*   0.02 */
   SMAUG_PARAM_RK_ORDER = 7, /* 4 (default), 2 (midpoint) or 1 (forward Euler) */
   SMAUG_PARAM_FIXED_DT = 8, /* > 0: use this dt instead of the CFL step; 0 (default): CFL */
-  SMAUG_PARAM_KERNEL = 9    /* 2 (default): role-split streaming stage kernel where applicable (no background,
+  SMAUG_PARAM_KERNEL = 9,   /* 2 (default): role-split streaming stage kernel where applicable (no background,
                                hyperdiffusion on); 1: single-role streaming kernel where applicable; 0: always the
                                tile kernel.  All are bit-identical; the switch exists for tests and profiling. */
+  SMAUG_PARAM_GX = 10,      /* uniform gravitational acceleration g = (GX, GY) of PAPER.md:35 ("rho g", "rho g.v"); */
+  SMAUG_PARAM_GY = 11       /*   default 0.  Split form (c-10): the background is taken to be in magneto-hydrostatic
+                               balance  grad p_tb - (B_b.grad)B_b = rho_b g,  so gravity acts on the perturbed
+                               density: S(m) = rho~ g, S(e~) = rho~ g.v.  With a zero background rho~ is the total
+                               density and these are the printed source terms.  Any finite value. */
 };
 
 /* Bytes of device memory a context for an nx-by-ny grid needs (has_bg != 0: a background is given).

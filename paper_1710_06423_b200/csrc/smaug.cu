@@ -79,6 +79,7 @@ struct smaug_ctx {
   double c_rho = 0.02, c_mom = 0.4, c_e = 0.02, c_b = 0.02;
   int rk_order = 4;
   double fixed_dt = 0;
+  double gx = 0, gy = 0;    // uniform gravity (c-10)
   bool has_bg = false;
   Layout L;
   char* base = nullptr;     // device workspace
@@ -117,6 +118,8 @@ Params make_params(const smaug_ctx* c) {
   p.inv_dy = c->g.ny / c->Ly;
   p.c_rho = c->c_rho; p.c_mom = c->c_mom; p.c_e = c->c_e; p.c_b = c->c_b;
   p.hd_on = c->hd_on;
+  p.gx = c->gx; p.gy = c->gy;
+  p.grav_on = (c->gx != 0.0 || c->gy != 0.0) ? 1 : 0;
   return p;
 }
 
@@ -295,12 +298,17 @@ int launch_flux(smaug_ctx* c, const StageArgs& a) {
   return SMAUG_OK;
 }
 
-bool uses_flux(const smaug_ctx* c) { return !c->has_bg && !c->hd_on && c->kernel_mode != 0; }
+// The streaming kernels cover the benchmark configurations (zero background, no gravity); everything else
+// runs in the tiled kernel.
+bool plain(const smaug_ctx* c) { return !c->has_bg && c->gx == 0.0 && c->gy == 0.0; }
+bool uses_flux(const smaug_ctx* c) { return plain(c) && !c->hd_on && c->kernel_mode != 0; }
+bool uses_split(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 2; }
+bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 1; }
 
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
   if (uses_flux(c)) return launch_flux(c, a);
-  if (!c->has_bg && c->hd_on && c->kernel_mode == 2) return launch_split(c, a);
-  if (!c->has_bg && c->hd_on && c->kernel_mode == 1) return launch_march(c, a);
+  if (uses_split(c)) return launch_split(c, a);
+  if (uses_march(c)) return launch_march(c, a);
   if (c->has_bg) return c->hd_on ? launch_stage_t<true, true>(c, a) : launch_stage_t<true, false>(c, a);
   return c->hd_on ? launch_stage_t<false, true>(c, a) : launch_stage_t<false, false>(c, a);
 }
@@ -509,6 +517,8 @@ int smaug_set_param(smaug_ctx* c, int key, double v) {
     case SMAUG_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c->rk_order = (int)v; return SMAUG_OK;
     case SMAUG_PARAM_FIXED_DT: if (!(v >= 0)) break; c->fixed_dt = v; return SMAUG_OK;
     case SMAUG_PARAM_KERNEL: if (v != 0 && v != 1 && v != 2) break; c->kernel_mode = (int)v; return SMAUG_OK;
+    case SMAUG_PARAM_GX: if (!std::isfinite(v)) break; c->gx = v; return SMAUG_OK;
+    case SMAUG_PARAM_GY: if (!std::isfinite(v)) break; c->gy = v; return SMAUG_OK;
     default: return fail(SMAUG_EINVAL, "unknown parameter key");
   }
   return fail(SMAUG_EINVAL, "parameter value out of range");
@@ -598,10 +608,10 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (uses_flux(c)) {                                      // streaming kernel without HD: a strip of NT-4 columns
     out[0] = FLUX_NT - 4; out[1] = 1; out[2] = FLUX_NT;
     out[3] = (int)FluxSmem<FLUX_NT>::BYTES;
-  } else if (!c->has_bg && c->hd_on && c->kernel_mode == 2) {   // role-split streaming kernel: a strip of NC-8 columns
+  } else if (uses_split(c)) {   // role-split streaming kernel: a strip of NC-8 columns
     out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
     out[3] = (int)SplitSmem<SPLIT_NC>::BYTES;
-  } else if (!c->has_bg && c->hd_on && c->kernel_mode == 1) {   // streaming kernel: a strip of NT-6 columns
+  } else if (uses_march(c)) {   // streaming kernel: a strip of NT-6 columns
     out[0] = MARCH_NT - 2 * NG; out[1] = 1; out[2] = MARCH_NT;
     out[3] = (int)MarchSmem<MARCH_NT>::BYTES;
   } else {
@@ -615,8 +625,8 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
 const char* smaug_get_kernel_name(smaug_ctx* c) {
   if (!c) return "?";
   if (uses_flux(c)) return FLUX_NT == 128 ? "flux_kernel<128>" : "flux_kernel";
-  if (!c->has_bg && c->hd_on && c->kernel_mode == 2) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
-  if (!c->has_bg && c->hd_on && c->kernel_mode == 1) return "march_kernel<256>";
+  if (uses_split(c)) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
+  if (uses_march(c)) return "march_kernel<256>";
   return "stage_kernel<32,16,512>";
 }
 

@@ -367,6 +367,15 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
                            fma(Bby * Bby, dyvy, fma(Bbx * Bby, dxvy + dyvx, (Bbx * Bbx) * dxvx)));
       R[F_E] = R[F_E] + S;
     }
+    if (a.prm.grav_on) {
+      // gravity in the split form (c-10): S(m) = rho~ g, S(e) = rho~ (g.v), on the PERTURBED density
+      const int s = T::u(r, c);
+      const double rt = U[URT * T::U_PLANE + s];
+      const double gv = fma(a.prm.gy, U[U_VY * T::U_PLANE + s], a.prm.gx * U[U_VX * T::U_PLANE + s]);
+      R[F_MX] = fma(rt, a.prm.gx, R[F_MX]);
+      R[F_MY] = fma(rt, a.prm.gy, R[F_MY]);
+      R[F_E] = fma(rt, gv, R[F_E]);
+    }
 
     if (HD) {
       const double* px = KX + T::kx(r, c);      // interface (c | c+1); (c-1 | c) is at px[-1]

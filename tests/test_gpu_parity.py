@@ -245,3 +245,29 @@ def test_bench_config_8000_two_kernels_and_properties(gpu):
     w_dev = wt.to(a.device)
     drift = (a.reshape(6, -1).sum(1) - w_dev.reshape(6, -1).sum(1)).abs() / w_dev.abs().reshape(6, -1).sum(1)
     assert bool((drift < 1e-12).all()), drift
+
+
+# ----------------------------------------------------------------------------- gravity (c-10)
+@pytest.mark.parametrize("nx,ny,steps,hd_on", [(70, 90, 30, 1), (33, 50, 20, 0), (200, 160, 40, 1)])
+def test_stratified_atmosphere_parity(gpu, oracle_mod, nx, ny, steps, hd_on):
+    """Hydrostatic, magnetised background + gravity + a pulse (the code's stated use), periodic in
+    x, open in y: background loads, energy source, gravity sources and open ghosts together."""
+    w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(nx, ny)
+    a = gpu_run(gpu, w, bc, gamma, steps, bg=bg, gx=gx, gy=gy, hd_on=hd_on)
+    b = cpu_run(oracle_mod, w, bc, gamma, steps, bg=bg, gx=gx, gy=gy, hd_on=hd_on)
+    check(*a, *b)
+    assert np.abs(a[0][2]).max() > 1e-4           # the pulse moved something
+
+
+def test_gravity_without_background_and_static_atmosphere(gpu, oracle_mod):
+    # zero background: rho~ is the total density (the printed equations); both components of g
+    w, bc, gamma = si.orszag_tang(64, 48)
+    a = gpu_run(gpu, w, bc, gamma, 15, gx=0.4, gy=-0.9)
+    b = cpu_run(oracle_mod, w, bc, gamma, 15, gx=0.4, gy=-0.9)
+    check(*a, *b)
+    a0 = gpu_run(gpu, w, bc, gamma, 15)
+    assert not np.array_equal(a[0], a0[0])        # gravity is really applied
+    # G1 on the GPU: a hydrostatic background with zero perturbation stays exactly static
+    w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(40, 60, pulse=0.0)
+    out, t, ws = gpu_run(gpu, w, bc, gamma, 10, bg=bg, gx=gx, gy=gy)
+    assert not out.any() and t[0] > 0
