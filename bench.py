@@ -37,6 +37,9 @@ WORKLOADS = {
     "orszag_tang_2044": (2044, 2044, "ot"),
     "orszag_tang_1000": (1000, 1000, "ot"),
     "brio_wu_800": (800, 1, "bw"),
+    # SURVEY 8(f) NEXT-2 (not a BASELINE config): stratified magnetised atmosphere with a pulse, non-uniform
+    # background + gravity, periodic in x, open in y -- runs in the tiled kernel
+    "stratified_4000": (4000, 4000, "strat"),
 }
 # Algorithmic HBM bytes per cell-update of the fused step as built: per stage the
 # kernel reads the 6 input planes once and writes 6; stages 2-3 also read w^n; stage 2 also writes the
@@ -55,10 +58,17 @@ UNIT = "cell-updates/s"
 
 
 def make_state(name):
+    """(w, bc, gamma, bg, (gx, gy)) of a workload."""
     nx, ny, kind = WORKLOADS[name]
-    if kind == "ot":
-        return si.orszag_tang(nx, ny)
-    return si.brio_wu(nx, ny)
+    if kind == "strat":
+        return si.stratified_atmosphere(nx, ny)
+    w, bc, gamma = si.orszag_tang(nx, ny) if kind == "ot" else si.brio_wu(nx, ny)
+    return w, bc, gamma, None, (0.0, 0.0)
+
+
+def bytes_per_cell_update(has_bg):
+    """Algorithmic HBM bytes per cell-update: 576 (see above) + the four background planes read once per stage."""
+    return BYTES_PER_CELL_UPDATE + (STAGES_PER_STEP * 4 * 8 if has_bg else 0)
 
 
 def peaks():
@@ -138,11 +148,15 @@ def replica_value(cells, steps, world, ms):
     return world * float(cells) * steps / (ms * 1e-3)
 
 
-def oracle_rate(sample_n, steps, warmup=0, threads=1):
-    """cell-updates/s of the oracle (as it stands) on an Orszag-Tang sample_n^2 grid."""
+def oracle_rate(sample_n, steps, warmup=0, threads=1, kind="ot"):
+    """cell-updates/s of the oracle (as it stands) on a sample_n^2 grid of the workload's kind."""
     import oracle
-    w, bc, gamma = si.orszag_tang(sample_n)
-    o = oracle.Oracle(sample_n, sample_n, gamma, bc, threads=threads)
+    if kind == "strat":
+        w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(sample_n, sample_n)
+        o = oracle.Oracle(sample_n, sample_n, gamma, bc, bg=bg, threads=threads, gx=gx, gy=gy)
+    else:
+        w, bc, gamma = si.orszag_tang(sample_n)
+        o = oracle.Oracle(sample_n, sample_n, gamma, bc, threads=threads)
     o.set_state(w)
     if warmup:
         o.step(warmup, 0.3)
@@ -197,11 +211,14 @@ def run_ours(args):
 
     name = args.workload
     nx, ny, _ = WORKLOADS[name]
-    w_np, bc, gamma = make_state(name)
+    w_np, bc, gamma, bg_np, (gx, gy) = make_state(name)
     w_host = torch.from_numpy(w_np).pin_memory()
     out_host = torch.empty_like(w_host).pin_memory()
-    del w_np
-    sim = pkg.Smaug(nx, ny, gamma, bc, device=dev, hd_on=0 if args.no_hd else 1)
+    bg_dev = None if bg_np is None else torch.from_numpy(bg_np).to(dev)
+    has_bg = bg_np is not None
+    del w_np, bg_np
+    sim = pkg.Smaug(nx, ny, gamma, bc, bg=bg_dev, device=dev, hd_on=0 if args.no_hd else 1, gx=gx, gy=gy)
+    del bg_dev
     sim.set_state(w_host)
 
     K, W = args.steps, args.warmup
@@ -241,7 +258,8 @@ def run_ours(args):
         e2e = replica_value(cells, K, world, e2e_ms)
         peak, peak_src = peaks()
         info = sim.kernel_info()
-        per_launch_bytes = BYTES_PER_CELL_UPDATE / STAGES_PER_STEP * cells
+        bpcu = bytes_per_cell_update(has_bg)
+        per_launch_bytes = bpcu / STAGES_PER_STEP * cells
         avg_launch_ms = stage_ms / max(stage_n, 1)
         achieved = per_launch_bytes / (avg_launch_ms * 1e-3) / 1e9 if stage_n else None
         state_bytes = 6 * 8 * cells
@@ -250,10 +268,10 @@ def run_ours(args):
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": 4,
-                       "background": "zero", "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "background": "stratified, g = (%g, %g)" % (gx, gy) if has_bg else "zero", "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "working set >> L2, no flush needed" if cells * 48 > 4e8 else
                              "working set comparable to L2 (126 MB): DRAM traffic is below algorithmic"},
-            "hbm_gbs_algorithmic": value / world * BYTES_PER_CELL_UPDATE / 1e9,
+            "hbm_gbs_algorithmic": value / world * bpcu / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": (achieved / peak) if achieved else None, "traffic": ncu_traffic(name),
                          "peak_source": peak_src, "kernel": f"smaug::{sim.kernel_name()} (fused RK stage)",
@@ -264,7 +282,7 @@ def run_ours(args):
                            "peak": N_SM * FP64_LANES_PER_SM * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12,
                            "unit": "T fp64-instr/s", "instr_per_cell_stage": FP64_INSTR_PER_CELL_STAGE,
                            "note": "secondary ceiling; only meaningful for split_kernel<128>"}
-                          if stage_n and not args.no_hd else None),
+                          if stage_n and not args.no_hd and not has_bg else None),
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
                     "d2h_bytes_per_step": state_bytes / K,
                     "note": "smaug_set_state(host) + smaug_step(K) + smaug_get_state(host), pinned host memory"},
@@ -276,10 +294,12 @@ def run_ours(args):
             line["fp64_pipe"]["frac"] = line["fp64_pipe"]["achieved"] / line["fp64_pipe"]["peak"]
         if not args.no_cpu_baseline and world == 1:
             n_s, steps_s = 1000, 6
-            rate, el = oracle_rate(n_s, steps_s, threads=1)
+            kind = "strat" if has_bg else "ot"
+            rate, el = oracle_rate(n_s, steps_s, threads=1, kind=kind)
             line["cpu_baseline"] = {
                 "value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                "sample": f"Orszag-Tang {n_s}x{n_s} (same IC and parameters), {steps_s} steps, {el:.1f} s, "
+                "sample": f"{'stratified atmosphere' if has_bg else 'Orszag-Tang'} {n_s}x{n_s} (same IC and "
+                          f"parameters), {steps_s} steps, {el:.1f} s, "
                           f"1 of {os.cpu_count()} host cores"}
         print(json.dumps(line), flush=True)
     sim.close()

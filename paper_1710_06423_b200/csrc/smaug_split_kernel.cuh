@@ -173,6 +173,50 @@ __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("pre
 #endif
 constexpr int SPLIT_YUNROLL = SMAUG_SPLIT_YUNROLL;   // row steps of the Y role per loop trip
 
+#ifndef SMAUG_SPLIT_WSFILTER
+#define SMAUG_SPLIT_WSFILTER 1
+#endif
+// Wave-speed maxima of one written cell folded into the running maxima m[4] (c-4): the same operation sequence
+// as cell_wavespeeds, with two changes that leave every reduced value unchanged:
+//  * a candidate enters with `c > m ? c : m` against a running maximum that is >= 0, which drops NaNs and
+//    negative values exactly like the clamp fmax(c, 0) followed by a max;
+//  * FULL: the two fast speeds (four square roots) are evaluated only where they can still raise a maximum.
+//    thr[d] is any lower bound of the final max(|v_d| + c_f,d) (the running maximum of this thread or the value
+//    other CTAs have already published).  With a^2 >= 0, b^2 >= 0:  c_f,d^2 <= s = a^2 + b^2, and in floating
+//    point |v_d| + sqrt(c_f,d^2) <= (|v_d| + sqrt(s) (1 + 2u)) (1 + u), u = 2^-53.  So with t = thr - |v_d|,
+//    t > thr 2^-10 and t^2 >= s (1 + 2^-40) prove the cell cannot exceed thr (the margin 2^-40 covers the
+//    rounding of t, t^2 and the bound by ten orders of magnitude; t > thr 2^-10 keeps the cancellation in t
+//    harmless).  Skipped cells therefore never held the maximum: the reduced values are bit-identical.
+template <int WS>
+__device__ __forceinline__ void split_wavespeeds(const double (&o)[NF], double gamma, double (&m)[4], double thr0,
+                                                 double thr1) {
+  const double rr = drcp(o[F_RHO]);
+  const double vx = o[F_MX] * rr, vy = o[F_MY] * rr;
+  const double B2 = fma(o[F_BY], o[F_BY], o[F_BX] * o[F_BX]);
+  const double pk = (gamma - 1.0) * ((o[F_E] - 0.5 * fma(o[F_MY], vy, o[F_MX] * vx)) - 0.5 * B2);
+  const double a2 = (gamma * pk) * rr;
+  const double b2 = B2 * rr;
+  m[2] = a2 > m[2] ? a2 : m[2];
+  m[3] = b2 > m[3] ? b2 : m[3];
+  if (WS == WS_FULL) {
+    const double s = a2 + b2;
+#if SMAUG_SPLIT_WSFILTER
+    const double t0 = thr0 - fabs(vx), t1 = thr1 - fabs(vy);
+    const double sm = s * (1.0 + 0x1p-40);
+    const bool skip = a2 >= 0.0 && b2 >= 0.0 && t0 > thr0 * 0x1p-10 && t1 > thr1 * 0x1p-10 && t0 * t0 >= sm &&
+                      t1 * t1 >= sm;
+    if (skip) return;
+#endif
+    const double fa = (4.0 * a2) * rr;
+    const double d0 = fma(s, s, -(fa * (o[F_BX] * o[F_BX]))), d1 = fma(s, s, -(fa * (o[F_BY] * o[F_BY])));
+    const double cfx2 = 0.5 * (s + sqrt(d0 > 0.0 ? d0 : 0.0));
+    const double cfy2 = 0.5 * (s + sqrt(d1 > 0.0 ? d1 : 0.0));
+    const double c0 = fabs(vx) + sqrt(cfx2), c1 = fabs(vy) + sqrt(cfy2);
+    m[0] = c0 > m[0] ? c0 : m[0];
+    m[1] = c1 > m[1] ? c1 : m[1];
+  }
+}
+
 template <int NC, int COMBINE, int WS>
 #ifdef SMAUG_SPLIT_MAXNREG
 __global__ void __maxnreg__(SMAUG_SPLIT_MAXNREG) split_kernel
@@ -383,6 +427,13 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       const bool ky_on = r >= ystart + NG - 1;
       // operands of the RK combine for row j: issued here, consumed at the end of the step
       double jbase[NF], jacc[NF], jin[NF];
+      // maxima other CTAs have already published for this launch: lower bounds of the final maxima (any stale
+      // value is one too), used by split_wavespeeds to skip cells that cannot raise them
+      double gthr0 = 0.0, gthr1 = 0.0;
+      if (WS == WS_FULL && tail_on) {
+        gthr0 = __longlong_as_double((long long)__ldcg(&a.sc->red[a.red_out][0]));
+        gthr1 = __longlong_as_double((long long)__ldcg(&a.sc->red[a.red_out][1]));
+      }
 #if SMAUG_SPLIT_LATELOAD == 0
       if (tail_on) {
         if (COMBINE == COMBINE_FINAL) {
@@ -534,10 +585,12 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
             for (int f = 0; f < NF; ++f) a.acc_out.p[f][go] = fma(2.0, o[f], jin[f] - jbase[f]);
           }
           if (WS != WS_NONE) {
-            double w4[4];
-            cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, WS == WS_FULL, w4);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) wsmax[k] = dmax(wsmax[k], w4[k]);
+            double thr0 = wsmax[0], thr1 = wsmax[1];
+            if (WS == WS_FULL) {
+              thr0 = gthr0 > thr0 ? gthr0 : thr0;
+              thr1 = gthr1 > thr1 ? gthr1 : thr1;
+            }
+            split_wavespeeds<WS>(o, gamma, wsmax, thr0, thr1);
           }
         }
       }
