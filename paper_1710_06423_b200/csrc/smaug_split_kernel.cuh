@@ -176,6 +176,9 @@ constexpr int SPLIT_YUNROLL = SMAUG_SPLIT_YUNROLL;   // row steps of the Y role 
 #ifndef SMAUG_SPLIT_WSFILTER
 #define SMAUG_SPLIT_WSFILTER 1
 #endif
+#ifndef SMAUG_SPLIT_JIN3
+#define SMAUG_SPLIT_JIN3 1
+#endif
 // Wave-speed maxima of one written cell folded into the running maxima m[4] (c-4): the same operation sequence
 // as cell_wavespeeds, with two changes that leave every reduced value unchanged:
 //  * a candidate enters with `c > m ? c : m` against a running maximum that is >= 0, which drops NaNs and
@@ -427,6 +430,16 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       const bool ky_on = r >= ystart + NG - 1;
       // operands of the RK combine for row j: issued here, consumed at the end of the step
       double jbase[NF], jacc[NF], jin[NF];
+      // the stage input at row j: rho~, bx~ are in the histories and by~ in the by ring (the same values X read
+      // from global memory), so only mx, my, e~ are loaded
+      auto load_jin = [&]() {
+#if SMAUG_SPLIT_JIN3
+        jin[F_MX] = a.in.p[F_MX][gj]; jin[F_MY] = a.in.p[F_MY][gj]; jin[F_E] = a.in.p[F_E][gj];
+#else
+#pragma unroll
+        for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
+#endif
+      };
       // maxima other CTAs have already published for this launch: lower bounds of the final maxima (any stale
       // value is one too), used by split_wavespeeds to skip cells that cannot raise them
       double gthr0 = 0.0, gthr1 = 0.0;
@@ -434,21 +447,20 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         gthr0 = __longlong_as_double((long long)__ldcg(&a.sc->red[a.red_out][0]));
         gthr1 = __longlong_as_double((long long)__ldcg(&a.sc->red[a.red_out][1]));
       }
-#if SMAUG_SPLIT_LATELOAD == 0
-      if (tail_on) {
+      auto load_operands = [&]() {
         if (COMBINE == COMBINE_FINAL) {
 #pragma unroll
-          for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
+          for (int f = 0; f < NF; ++f) jacc[f] = a.acc_in.p[f][gj];
+          load_jin();
         } else {
 #pragma unroll
           for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
-          if (COMBINE == COMBINE_ACC) {
-#pragma unroll
-            for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
-          }
+          if (COMBINE == COMBINE_ACC) load_jin();
         }
-      }
-#elif SMAUG_SPLIT_LATELOAD == 2
+      };
+#if SMAUG_SPLIT_LATELOAD == 0
+      if (tail_on) load_operands();
+#elif SMAUG_SPLIT_LATELOAD == 2 || SMAUG_SPLIT_LATELOAD == 3
       if (tail_on) {     // bring the lines into L2; the loads themselves are issued after barrier B
         if (COMBINE == COMBINE_FINAL) {
 #pragma unroll
@@ -506,6 +518,9 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         y_interface(std::true_type{});
 #endif
       }
+#if SMAUG_SPLIT_LATELOAD == 3 || SMAUG_SPLIT_LATELOAD == 4
+      if (tail_on) load_operands();     // after the register-hungry kappa phase, one barrier ahead of their use
+#endif
       if (tail_on) {
         // G(my ; x), G(by ; x) and their energy companion at row j (histories index 2); C_x = F_x - G
         const double kv = 0.5 * (kyv_prev + kyv);
@@ -514,6 +529,9 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         const double gb = -(kb * (cd12v(hbx[0], hbx[1], hbx[3], hbx[4]) * (1.0 / 12.0)));
         double* cx = CXR + s5 * 5 * PW + tp;
         const double jby = BYR[s5 * NC + c];
+#if SMAUG_SPLIT_JIN3
+        if (COMBINE != COMBINE_BASE) { jin[F_RHO] = hr[2]; jin[F_BX] = hbx[2]; jin[F_BY] = jby; }
+#endif
         cx[C_MY * PW] = cx[C_MY * PW] - gm;
         cx[C_E * PW] = cx[C_E * PW] - fma(hvy[2], gm, jby * gb);
         cx[C_B * PW] = cx[C_B * PW] - gb;
@@ -522,7 +540,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
 
       // ---------------------------------------------------------------- assemble R(j), combine, write
       if (tail_on) {
-#if SMAUG_SPLIT_LATELOAD != 0
+#if SMAUG_SPLIT_LATELOAD == 1 || SMAUG_SPLIT_LATELOAD == 2
         if (COMBINE == COMBINE_FINAL) {
 #pragma unroll
           for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
