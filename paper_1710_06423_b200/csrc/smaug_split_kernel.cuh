@@ -49,7 +49,8 @@ struct SplitSmem {
   static constexpr int OFF_CYR = OFF_DXR + ND * 5 * NC; // ring NY rows x 5: C_y
   static constexpr int OFF_INR = OFF_CYR + NY * 5 * NC; // cp.async landing zone of the next input row (6 fields)
   static constexpr int OFF_RED = OFF_INR;               // block reduction scratch (after the march: INR is dead)
-  static constexpr int TOTAL = OFF_INR + (6 * NC > 4 * 32 ? 6 * NC : 4 * 32);
+  static constexpr int OFF_MBAR = OFF_INR + (6 * NC > 4 * 32 ? 6 * NC : 4 * 32);   // one mbarrier (barrier B of Y)
+  static constexpr int TOTAL = OFF_MBAR + 2;
   static constexpr int CTAS_PER_SM = NC <= 64 ? 4 : (NC <= 128 ? 2 : 1);
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
 };
@@ -68,6 +69,29 @@ __device__ __forceinline__ void bar_arrive() { asm volatile("bar.arrive %0, %1;"
 // barrier among the NTHREADS threads of one role (named barrier ID > 0)
 template <int ID, int NTHREADS>
 __device__ __forceinline__ void role_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(NTHREADS) : "memory"); }
+
+// split-phase barrier (mbarrier): arrive when this thread's data is published, wait -- later -- for everyone's
+__device__ __forceinline__ void mbar_init(double* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(double* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(double* bar, int parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+#ifndef SMAUG_SPLIT_MBAR
+#define SMAUG_SPLIT_MBAR 0      // barrier B of the Y role: 0 bar.sync; 1 split-phase mbarrier (arrive after publishing
+                                // C_x, wait after the y-differences) -- measured: no gain (3.310 vs 3.302 ms per stage)
+#endif
 
 // the operand of larger magnitude (max and abs are exact, so |amax| chains equal max-of-abs chains bit for bit;
 // the comparisons take |.| as a free source modifier)
@@ -245,6 +269,11 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
   const int ystart = blockIdx.y * mg.rows_per_cta;
   const int yend = min(ystart + mg.rows_per_cta, g.ny);
   double wsmax[4] = {0.0, 0.0, 0.0, 0.0};
+  double* const MBAR = smem + S::OFF_MBAR;
+#if SMAUG_SPLIT_MBAR
+  if (tid == 0) mbar_init(MBAR, NC);
+  __syncthreads();
+#endif
 
   if (tid < NXT) {
     // =================================================================== X role: columns c0, c0 + 1
@@ -420,6 +449,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
     constexpr int ND = S::ND, NY = S::NY;
     int s4 = ND - 3, s5 = 2, s6 = 0;                       // slots of row j in DXR, CXR; of row r in CYR
     int par = 0;                                           // UP buffer of row r
+    [[maybe_unused]] int mph = 0;                          // phase parity of barrier B (mbarrier)
     if (DEC) bar_arrive<4, NTH>();                         // E for the first row: nothing to wait for
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
@@ -536,9 +566,28 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         cx[C_E * PW] = cx[C_E * PW] - fma(hvy[2], gm, jby * gb);
         cx[C_B * PW] = cx[C_B * PW] - gb;
       }
+#if SMAUG_SPLIT_MBAR
+      mbar_arrive(MBAR);                                              // ---- B (Y warps only): C_x(j) published
+#else
       role_barrier<2, NC>();                                          // ---- B (Y warps only)
+#endif
 
       // ---------------------------------------------------------------- assemble R(j), combine, write
+      // (everything that does not need the neighbours' C_x comes before the wait of barrier B)
+      double cdyi[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (tail_on) {
+        // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-NY ring
+        auto back = [&](int k) { const int q = s6 + (NY - k); return q >= NY ? q - NY : q; };   // slot of row r - k
+        const int jm2 = back(5), jm1 = back(4), jp1 = back(2), jp2 = back(1);
+#pragma unroll
+        for (int f = 0; f < 5; ++f)
+          cdyi[f] = cd12v(CYR[(jm2 * 5 + f) * NC + c], CYR[(jm1 * 5 + f) * NC + c], CYR[(jp1 * 5 + f) * NC + c],
+                          CYR[(jp2 * 5 + f) * NC + c]) * idy_;
+      }
+#if SMAUG_SPLIT_MBAR
+      mbar_wait(MBAR, mph);
+      mph ^= 1;
+#endif
       if (tail_on) {
 #if SMAUG_SPLIT_LATELOAD == 1 || SMAUG_SPLIT_LATELOAD == 2
         if (COMBINE == COMBINE_FINAL) {
@@ -559,19 +608,11 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           double cdx[5];
 #pragma unroll
           for (int f = 0; f < 5; ++f) cdx[f] = cd12v(cx[f * PW - 2], cx[f * PW - 1], cx[f * PW + 1], cx[f * PW + 2]);
-          // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-NY ring
-          auto back = [&](int k) { const int q = s6 + (NY - k); return q >= NY ? q - NY : q; };   // slot of row r - k
-          const int jm2 = back(5), jm1 = back(4), jp1 = back(2), jp2 = back(1);
-          double cdy[5];
-#pragma unroll
-          for (int f = 0; f < 5; ++f)
-            cdy[f] = cd12v(CYR[(jm2 * 5 + f) * NC + c], CYR[(jm1 * 5 + f) * NC + c], CYR[(jp1 * 5 + f) * NC + c],
-                           CYR[(jp2 * 5 + f) * NC + c]);
-          R[F_RHO] = fma(cdx[C_RHO], idx_, cdy[C_RHO] * idy_) * (-1.0 / 12.0);
-          R[F_MX] = fma(cdx[C_MX], idx_, cdy[C_MX] * idy_) * (-1.0 / 12.0);
-          R[F_MY] = fma(cdx[C_MY], idx_, cdy[C_MY] * idy_) * (-1.0 / 12.0);
-          R[F_E] = fma(cdx[C_E], idx_, cdy[C_E] * idy_) * (-1.0 / 12.0);
-          R[F_BX] = (cdy[C_B] * idy_) * (-1.0 / 12.0);
+          R[F_RHO] = fma(cdx[C_RHO], idx_, cdyi[C_RHO]) * (-1.0 / 12.0);
+          R[F_MX] = fma(cdx[C_MX], idx_, cdyi[C_MX]) * (-1.0 / 12.0);
+          R[F_MY] = fma(cdx[C_MY], idx_, cdyi[C_MY]) * (-1.0 / 12.0);
+          R[F_E] = fma(cdx[C_E], idx_, cdyi[C_E]) * (-1.0 / 12.0);
+          R[F_BX] = cdyi[C_B] * (-1.0 / 12.0);
           R[F_BY] = fma(cdx[C_B], idx_, 0.0) * (-1.0 / 12.0);
         }
         const double* dx = DXR + s4 * 5 * NC + c;
@@ -585,7 +626,6 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         R[F_MY] = fma(py[C_MY] - py_prev[C_MY], idy_, R[F_MY]);
         R[F_E] = fma(py[C_E] - py_prev[C_E], idy_, R[F_E]);
         R[F_BX] = fma(py[C_B] - py_prev[C_B], idy_, R[F_BX]);
-
         double o[NF];
         if (COMBINE == COMBINE_FINAL) {
 #pragma unroll
