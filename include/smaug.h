@@ -63,10 +63,13 @@ enum { /* keys of smaug_set_param */
                                hyperdiffusion on); 1: single-role streaming kernel where applicable; 0: always the
                                tile kernel.  All are bit-identical; the switch exists for tests and profiling. */
   SMAUG_PARAM_GX = 10,      /* uniform gravitational acceleration g = (GX, GY) of PAPER.md:35 ("rho g", "rho g.v"); */
-  SMAUG_PARAM_GY = 11       /*   default 0.  Split form (c-10): the background is taken to be in magneto-hydrostatic
+  SMAUG_PARAM_GY = 11,      /*   default 0.  Split form (c-10): the background is taken to be in magneto-hydrostatic
                                balance  grad p_tb - (B_b.grad)B_b = rho_b g,  so gravity acts on the perturbed
                                density: S(m) = rho~ g, S(e~) = rho~ g.v.  With a zero background rho~ is the total
                                density and these are the printed source terms.  Any finite value. */
+  SMAUG_PARAM_GRAPH = 12    /* 1 (default): smaug_step replays whole time steps as CUDA graphs (captured on first use for
+                               calls of >= 8 steps, re-captured when a parameter, the stream or cfl changes);
+                               0: plain kernel launches.  Same kernels, same results; only the launch path differs. */
 };
 
 /* Bytes of device memory a context for an nx-by-ny grid needs (has_bg != 0: a background is given).

@@ -18,7 +18,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, ENONFINITE = 0, -1, -2, -3, -4
-PARAMS = dict(lx=0, ly=1, hd_on=2, c_rho=3, c_mom=4, c_e=5, c_b=6, rk_order=7, fixed_dt=8, kernel=9, gx=10, gy=11)
+PARAMS = dict(lx=0, ly=1, hd_on=2, c_rho=3, c_mom=4, c_e=5, c_b=6, rk_order=7, fixed_dt=8, kernel=9, gx=10, gy=11, graph=12)
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-fmad=false", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -101,6 +101,18 @@ struct smaug_ctx {
   int kernel_mode = 2;      // SMAUG_PARAM_KERNEL: 2 role-split streaming kernel, 1 single-role streaming kernel
                             // (both only without background and with hyperdiffusion), 0 always the tile kernel
   int n_sm = 148;
+  // CUDA-graph replay of whole time steps (launch-bound small grids; SMAUG_PARAM_GRAPH).  One step is 9 launches
+  // whose arguments are fixed except for the reduction-set parity (state_set 0 <-> 4), so three executables cover
+  // every call: a step from set 0, a step from set 4, and the pair starting at set 0.  They are captured on a
+  // library-owned stream (the caller's may be the legacy default stream, which cannot be captured) that is
+  // chained to the caller's stream by events.
+  int use_graph = 1;
+  bool graph_valid = false;
+  double graph_cfl = 0;
+  cudaGraphExec_t gexec[3] = {nullptr, nullptr, nullptr};
+  cudaStream_t gstream = nullptr;
+  cudaEvent_t gev_in = nullptr, gev_out = nullptr;
+  int launches_per_step = 0;
 };
 
 namespace {
@@ -363,6 +375,81 @@ int enqueue_step(smaug_ctx* c, double cfl) {
   return rc;
 }
 
+void invalidate_graphs(smaug_ctx* c) {
+  for (auto& g : c->gexec) {
+    if (g) cudaGraphExecDestroy(g);
+    g = nullptr;
+  }
+  c->graph_valid = false;
+}
+
+// Capture the three step graphs for this cfl (parameters are baked into the kernel arguments: any
+// smaug_set_param / smaug_set_stream invalidates them).  Leaves the context's state untouched.
+int capture_graphs(smaug_ctx* c, double cfl) {
+  invalidate_graphs(c);
+  if (!c->gstream) {
+    CU(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&c->gev_in, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&c->gev_out, cudaEventDisableTiming));
+  }
+  const int saved_set = c->state_set;
+  const long long saved_launches = c->launches;
+  cudaStream_t user = c->stream;
+  c->stream = c->gstream;
+  int rc = SMAUG_OK;
+  for (int k = 0; k < 3 && !rc; ++k) {
+    c->state_set = k == 1 ? 4 : 0;
+    const long long l0 = c->launches;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      rc = fail(SMAUG_ECUDA, "cudaStreamBeginCapture failed");
+      break;
+    }
+    rc = enqueue_step(c, cfl);
+    if (!rc && k == 2) rc = enqueue_step(c, cfl);
+    const cudaError_t e = cudaStreamEndCapture(c->gstream, &graph);
+    if (!rc && e != cudaSuccess) rc = fail(SMAUG_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+    if (!rc && cudaGraphInstantiate(&c->gexec[k], graph, 0) != cudaSuccess)
+      rc = fail(SMAUG_ECUDA, "cudaGraphInstantiate failed");
+    if (graph) cudaGraphDestroy(graph);
+    if (k == 0) c->launches_per_step = (int)(c->launches - l0);
+  }
+  c->stream = user;
+  c->state_set = saved_set;
+  c->launches = saved_launches;
+  if (rc) {
+    cudaGetLastError();
+    invalidate_graphs(c);
+    return rc;
+  }
+  c->graph_valid = true;
+  c->graph_cfl = cfl;
+  return SMAUG_OK;
+}
+
+// n steps as graph replays on the library's stream, ordered after / before the caller's stream by events.
+int replay_steps(smaug_ctx* c, int n) {
+  CU(cudaEventRecord(c->gev_in, c->stream));
+  CU(cudaStreamWaitEvent(c->gstream, c->gev_in, 0));
+  int left = n;
+  if (left > 0 && c->state_set == 4) {
+    CU(cudaGraphLaunch(c->gexec[1], c->gstream));
+    c->state_set = 0;
+    --left;
+  }
+  for (; left >= 2; left -= 2) CU(cudaGraphLaunch(c->gexec[2], c->gstream));
+  if (left == 1) {
+    CU(cudaGraphLaunch(c->gexec[0], c->gstream));
+    c->state_set = 4;
+  }
+  c->launches += (long long)n * c->launches_per_step;
+  CU(cudaEventRecord(c->gev_out, c->gstream));
+  CU(cudaStreamWaitEvent(c->stream, c->gev_out, 0));
+  return SMAUG_OK;
+}
+
+constexpr int GRAPH_MIN_STEPS = 8;   // fewer steps than this do not pay for a capture
+
 int check_ctx(smaug_ctx* c) {
   if (!c) return fail(SMAUG_EINVAL, "NULL context");
   return SMAUG_OK;
@@ -491,6 +578,13 @@ int smaug_create(int nx, int ny, double gamma, const int bc[4], const double* bg
 void smaug_destroy(smaug_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
+  invalidate_graphs(c);
+  if (c->gstream) {
+    cudaStreamSynchronize(c->gstream);
+    cudaStreamDestroy(c->gstream);
+    cudaEventDestroy(c->gev_in);
+    cudaEventDestroy(c->gev_out);
+  }
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   if (c->owns && c->base) cudaFree(c->base);
   cudaGetLastError();
@@ -501,11 +595,13 @@ int smaug_set_stream(smaug_ctx* c, void* stream) {
   if (int rc = check_ctx(c)) return rc;
   CU(cudaStreamSynchronize(c->stream));
   c->stream = (cudaStream_t)stream;
+  invalidate_graphs(c);
   return SMAUG_OK;
 }
 
 int smaug_set_param(smaug_ctx* c, int key, double v) {
   if (int rc = check_ctx(c)) return rc;
+  invalidate_graphs(c);      // parameters are baked into captured kernel arguments
   switch (key) {
     case SMAUG_PARAM_LX: if (!(v > 0)) break; c->Lx = v; return SMAUG_OK;
     case SMAUG_PARAM_LY: if (!(v > 0)) break; c->Ly = v; return SMAUG_OK;
@@ -517,6 +613,7 @@ int smaug_set_param(smaug_ctx* c, int key, double v) {
     case SMAUG_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c->rk_order = (int)v; return SMAUG_OK;
     case SMAUG_PARAM_FIXED_DT: if (!(v >= 0)) break; c->fixed_dt = v; return SMAUG_OK;
     case SMAUG_PARAM_KERNEL: if (v != 0 && v != 1 && v != 2) break; c->kernel_mode = (int)v; return SMAUG_OK;
+    case SMAUG_PARAM_GRAPH: c->use_graph = v != 0.0; return SMAUG_OK;
     case SMAUG_PARAM_GX: if (!std::isfinite(v)) break; c->gx = v; return SMAUG_OK;
     case SMAUG_PARAM_GY: if (!std::isfinite(v)) break; c->gy = v; return SMAUG_OK;
     default: return fail(SMAUG_EINVAL, "unknown parameter key");
@@ -547,6 +644,20 @@ int smaug_step_async(smaug_ctx* c, int n_steps, double cfl) {
   if (int rc = check_ctx(c)) return rc;
   if (n_steps < 0) return fail(SMAUG_EINVAL, "n_steps must be >= 0");
   if (!(c->fixed_dt > 0.0) && !(cfl > 0.0)) return fail(SMAUG_EINVAL, "cfl must be > 0");
+  // Whole steps as CUDA-graph replays: worth it when launches are a visible share of the step (small grids);
+  // harmless otherwise.  Not while per-kernel timing events are wanted, and not for Euler (its buffers swap).
+  if (c->use_graph && !c->timing && c->rk_order != 1 && n_steps > 0 &&
+      ((c->graph_valid && c->graph_cfl == cfl) || n_steps >= GRAPH_MIN_STEPS)) {
+    int rc = SMAUG_OK;
+    if (!(c->graph_valid && c->graph_cfl == cfl)) rc = capture_graphs(c, cfl);
+    if (!rc) {
+      rc = replay_steps(c, n_steps);
+      if (rc) return rc;
+      c->pending_status = true;
+      return SMAUG_OK;
+    }
+    // capture unavailable (e.g. the stream is being captured by the caller): fall through to plain launches
+  }
   for (int s = 0; s < n_steps; ++s) {
     int rc = enqueue_step(c, cfl);
     if (rc) return rc;

@@ -40,7 +40,7 @@ def gpu_run(pkg, w, bc, gamma, steps, cfl=0.3, bg=None, host=True, chunks=1, **p
 
 def cpu_run(oracle_mod, w, bc, gamma, steps, cfl=0.3, bg=None, threads=8, **params):
     ny, nx = w.shape[1:]
-    params = {k: v for k, v in params.items() if k != "kernel"}     # kernel choice is a GPU-only switch
+    params = {k: v for k, v in params.items() if k not in ("kernel", "graph")}     # GPU-only switches
     o = oracle_mod.Oracle(nx, ny, gamma, bc, bg=bg, threads=threads, **params)
     o.set_state(w)
     o.step(steps, cfl)
@@ -271,3 +271,32 @@ def test_gravity_without_background_and_static_atmosphere(gpu, oracle_mod):
     w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(40, 60, pulse=0.0)
     out, t, ws = gpu_run(gpu, w, bc, gamma, 10, bg=bg, gx=gx, gy=gy)
     assert not out.any() and t[0] > 0
+
+
+# ----------------------------------------------------------------------------- CUDA-graph replay of steps
+def test_graph_replay_equals_plain_launches(gpu, oracle_mod):
+    """SMAUG_PARAM_GRAPH: whole steps replayed as CUDA graphs give the same bits as plain launches, for odd and
+    even step counts, repeated calls (both reduction-set parities), a cfl change (re-capture) and a restart."""
+    import torch
+    w, bc, gamma = si.orszag_tang(150, 40)
+    outs = {}
+    for graph in (0, 1):
+        s = gpu.Smaug(150, 40, gamma, bc, graph=graph)
+        s.set_state(torch.from_numpy(w))
+        for n, cfl in ((9, 0.3), (8, 0.3), (3, 0.3), (11, 0.25), (1, 0.25), (16, 0.3)):
+            s.step(n, cfl)
+        mid = s.get_state().cpu().numpy()
+        s.set_state(torch.from_numpy(w))
+        s.step(13, 0.3)
+        outs[graph] = (mid, s.get_state().cpu().numpy(), s.time(), s.launch_count())
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert outs[0][2] == outs[1][2]
+    assert outs[0][3] == outs[1][3]                     # the launch count claims the same kernels either way
+    b = cpu_run(oracle_mod, w, bc, gamma, 13)
+    assert np.array_equal(outs[1][1], b[0])
+    # Brio-Wu (800 x 1, the launch-bound config) through graphs, against plain launches
+    w, bc, gamma = si.brio_wu(800, 1)
+    a1 = gpu_run(gpu, w, bc, gamma, 101, graph=1)
+    a0 = gpu_run(gpu, w, bc, gamma, 101, graph=0)
+    assert np.array_equal(a1[0], a0[0]) and a1[1] == a0[1]
