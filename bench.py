@@ -40,6 +40,9 @@ WORKLOADS = {
     # SURVEY 8(f) NEXT-2 (not a BASELINE config): stratified magnetised atmosphere with a pulse, non-uniform
     # background + gravity, periodic in x, open in y -- runs in the tiled kernel
     "stratified_4000": (4000, 4000, "strat"),
+    # SURVEY 8(d) extra row: the 8000^2 Orszag-Tang state as a perturbation on a uniform non-zero background
+    # (exercises the background loads and the energy source) -- tiled kernel
+    "orszag_tang_8000_bg": (8000, 8000, "otbg"),
 }
 # Algorithmic HBM bytes per cell-update of the fused step as built: per stage the
 # kernel reads the 6 input planes once and writes 6; stages 2-3 also read w^n; stage 2 also writes the
@@ -62,6 +65,11 @@ def make_state(name):
     nx, ny, kind = WORKLOADS[name]
     if kind == "strat":
         return si.stratified_atmosphere(nx, ny)
+    if kind == "otbg":
+        w, bc, gamma = si.orszag_tang(nx, ny)
+        rho_b, e_b, bx_b, by_b = 0.1, 0.2, 0.05, 0.03
+        w[0] -= rho_b; w[3] -= e_b; w[4] -= bx_b; w[5] -= by_b
+        return w, bc, gamma, si.uniform_background(nx, ny, rho_b, e_b, bx_b, by_b), (0.0, 0.0)
     w, bc, gamma = si.orszag_tang(nx, ny) if kind == "ot" else si.brio_wu(nx, ny)
     return w, bc, gamma, None, (0.0, 0.0)
 
@@ -154,6 +162,11 @@ def oracle_rate(sample_n, steps, warmup=0, threads=1, kind="ot"):
     if kind == "strat":
         w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(sample_n, sample_n)
         o = oracle.Oracle(sample_n, sample_n, gamma, bc, bg=bg, threads=threads, gx=gx, gy=gy)
+    elif kind == "otbg":
+        w, bc, gamma = si.orszag_tang(sample_n)
+        w[0] -= 0.1; w[3] -= 0.2; w[4] -= 0.05; w[5] -= 0.03
+        o = oracle.Oracle(sample_n, sample_n, gamma, bc, bg=si.uniform_background(sample_n, sample_n, 0.1, 0.2, 0.05, 0.03),
+                          threads=threads)
     else:
         w, bc, gamma = si.orszag_tang(sample_n)
         o = oracle.Oracle(sample_n, sample_n, gamma, bc, threads=threads)
@@ -268,7 +281,7 @@ def run_ours(args):
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": 4,
-                       "background": "stratified, g = (%g, %g)" % (gx, gy) if has_bg else "zero", "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "background": ("stratified, g = (%g, %g)" % (gx, gy) if gy or gx else "uniform") if has_bg else "zero", "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "working set >> L2, no flush needed" if cells * 48 > 4e8 else
                              "working set comparable to L2 (126 MB): DRAM traffic is below algorithmic"},
             "hbm_gbs_algorithmic": value / world * bpcu / 1e9,
@@ -295,11 +308,11 @@ def run_ours(args):
             line["fp64_pipe"]["frac"] = line["fp64_pipe"]["achieved"] / line["fp64_pipe"]["peak"]
         if not args.no_cpu_baseline and world == 1:
             n_s, steps_s = 1000, 6
-            kind = "strat" if has_bg else "ot"
+            kind = WORKLOADS[name][2] if has_bg else "ot"
             rate, el = oracle_rate(n_s, steps_s, threads=1, kind=kind)
             line["cpu_baseline"] = {
                 "value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
-                "sample": f"{'stratified atmosphere' if has_bg else 'Orszag-Tang'} {n_s}x{n_s} (same IC and "
+                "sample": f"{ {'strat': 'stratified atmosphere', 'otbg': 'Orszag-Tang on a uniform background'}.get(kind, 'Orszag-Tang')} {n_s}x{n_s} (same IC and "
                           f"parameters), {steps_s} steps, {el:.1f} s, "
                           f"1 of {os.cpu_count()} host cores"}
         print(json.dumps(line), flush=True)
