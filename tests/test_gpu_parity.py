@@ -312,3 +312,46 @@ def test_graph_replay_equals_plain_launches(gpu, oracle_mod):
     a1 = gpu_run(gpu, w, bc, gamma, 101, graph=1)
     a0 = gpu_run(gpu, w, bc, gamma, 101, graph=0)
     assert np.array_equal(a1[0], a0[0]) and a1[1] == a0[1]
+
+
+# ----------------------------------------------------------------------------- seeded sweep over configurations
+def _random_case(rng):
+    nx, ny = int(rng.integers(1, 261)), int(rng.integers(1, 141))
+    per_x, per_y = rng.random() < 0.5, rng.random() < 0.5
+    bc = ((0, 0) if per_x else tuple(int(v) for v in rng.integers(1, 3, 2))) + \
+         ((0, 0) if per_y else tuple(int(v) for v in rng.integers(1, 3, 2)))
+    W, _, gamma = si.smooth_random(nx, ny, seed=int(rng.integers(1 << 30)), amp=2e-2)
+    W[1] += 0.2 * W[0]
+    bg = None
+    kind = int(rng.integers(0, 3))
+    if kind:
+        x = si.centres(nx)[None, :] * np.ones((ny, 1))
+        y = si.centres(ny)[:, None] * np.ones((1, nx))
+        mod = (0.0 if kind == 1 else 1.0)
+        bg = np.stack([0.05 + 0.02 * mod * np.cos(2 * np.pi * x), 0.1 + 0.03 * mod * np.sin(2 * np.pi * y),
+                       0.03 + 0.01 * mod * np.sin(2 * np.pi * y), 0.02 + 0.01 * mod * np.cos(2 * np.pi * x)])
+        W = W.copy()
+        W[0] -= bg[0]; W[3] -= bg[1]; W[4] -= bg[2]; W[5] -= bg[3]
+    params = dict(hd_on=int(rng.random() < 0.7), rk_order=int(rng.choice([4, 4, 2, 1])),
+                  kernel=int(rng.choice([2, 2, 1, 0])))
+    if rng.random() < 0.4:
+        params.update(gx=float(rng.normal(0, 0.5)), gy=float(rng.normal(0, 0.5)))
+    if rng.random() < 0.3:
+        params.update(lx=float(rng.uniform(0.5, 2.0)), ly=float(rng.uniform(0.5, 2.0)))
+    steps = int(rng.integers(2, 13))
+    return np.ascontiguousarray(W), bc, gamma, bg, params, steps
+
+
+def test_seeded_sweep_of_configurations(gpu, oracle_mod):
+    """40 seeded draws of (grid 1..260 x 1..140, boundary kinds, no / uniform / non-uniform background, gravity,
+    hyperdiffusion on/off, RK order, kernel form, domain lengths, step count): every one bit-identical to the
+    oracle -- ragged strips, n < ghost width, every kernel selection path."""
+    rng = np.random.default_rng(1710)
+    for case in range(40):
+        w, bc, gamma, bg, params, steps = _random_case(rng)
+        a = gpu_run(gpu, w, bc, gamma, steps, bg=bg, **params)
+        b = cpu_run(oracle_mod, w, bc, gamma, steps, bg=bg, threads=4, **params)
+        try:
+            check(*a, *b)
+        except AssertionError as e:
+            raise AssertionError(f"case {case}: {w.shape[1:]} bc={bc} bg={bg is not None} {params} steps={steps}: {e}")
