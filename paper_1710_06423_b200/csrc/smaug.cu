@@ -37,7 +37,7 @@ int fail(int code, const std::string& msg) {
 #define SMAUG_TW 32
 #endif
 #ifndef SMAUG_TH
-#define SMAUG_TH 16
+#define SMAUG_TH 8
 #endif
 #ifndef SMAUG_NT
 #define SMAUG_NT 512
@@ -738,7 +738,7 @@ const char* smaug_get_kernel_name(smaug_ctx* c) {
   if (uses_flux(c)) return FLUX_NT == 128 ? "flux_kernel<128>" : "flux_kernel";
   if (uses_split(c)) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
   if (uses_march(c)) return "march_kernel<256>";
-  return "stage_kernel<32,16,512>";
+  return TW == 32 && TH == 8 && NT == 512 ? "stage_kernel<32,8,512>" : "stage_kernel";
 }
 
 int smaug_set_kernel_timing(smaug_ctx* c, int on) {

@@ -65,7 +65,7 @@ def check(a, ta, wsa, b, tb, wsb, tol=TOL, exact=True):
     return err
 
 
-# sizes span several 32x16 tiles / 248-column strips plus ragged tails in both directions
+# sizes span several 32x8 tiles / 120-column strips plus ragged tails in both directions
 @pytest.mark.parametrize("nx,ny,steps", [(70, 45, 20), (32, 16, 10), (33, 17, 10), (200, 200, 40), (520, 70, 6)])
 def test_orszag_tang_parity(gpu, oracle_mod, nx, ny, steps):
     w, bc, gamma = si.orszag_tang(nx, ny)
