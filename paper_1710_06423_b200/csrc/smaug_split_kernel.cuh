@@ -28,6 +28,11 @@
 #ifndef SMAUG_SPLIT_DECOUPLE
 #define SMAUG_SPLIT_DECOUPLE 1
 #endif
+#ifndef SMAUG_SPLIT_TMEM
+#define SMAUG_SPLIT_TMEM 0      // 1: the C_y ring of the Y role lives in tensor memory (thread-private columns), shared
+#endif                          //    memory keeps a two-row staging buffer only (needs SMAUG_SPLIT_DECOUPLE): 25.6 KB
+                                //    less shared memory per CTA, bit-identical, 3.35 instead of 3.31 ms per stage at
+                                //    8000^2 -- a capacity lever (room for the background planes), not a speed-up
 
 namespace smaug {
 
@@ -40,7 +45,9 @@ struct SplitSmem {
   static constexpr bool DEC = SMAUG_SPLIT_DECOUPLE != 0;
   static constexpr int NUP = DEC ? 1 : 2;               // UP buffers
   static constexpr int ND = DEC ? 5 : 4;                // rows in DXR
-  static constexpr int NY = DEC ? 7 : 6;                // rows in CYR
+  static constexpr bool TM = SMAUG_SPLIT_TMEM != 0;
+  static_assert(!TM || DEC, "SMAUG_SPLIT_TMEM needs SMAUG_SPLIT_DECOUPLE");
+  static constexpr int NY = TM ? 2 : (DEC ? 7 : 6);     // rows in CYR (TM: a two-row staging buffer)
   static constexpr int OFF_UP = 0;                      // NUP x 6 planes: rho, vx, vy, eps, by, bx of the head row
   static constexpr int OFF_PK = OFF_UP + NUP * 6 * PW;  // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
   static constexpr int OFF_CXR = OFF_PK + 7 * PW;       // ring 5 rows x 5 planes: F_x, then C_x
@@ -88,6 +95,23 @@ __device__ __forceinline__ void mbar_wait(double* bar, int parity) {
       "MBAR_DONE:\n"
       "}" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
 }
+// Tensor memory as thread-private fp64 storage: a double is two 32-bit columns of the thread's own lane
+// (32x32b shape: lane = 32 * (warp % 4) + lane id).  .sync.aligned: whole warps execute these together.
+__device__ __forceinline__ void tm_st(unsigned taddr, double v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__double2loint(v)),
+               "r"(__double2hiint(v)) : "memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_ld4(unsigned taddr, double (&v)[4]) {     // four consecutive doubles
+  unsigned r0, r1, r2, r3, r4, r5, r6, r7;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3), "=r"(r4), "=r"(r5), "=r"(r6), "=r"(r7) : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  v[0] = __hiloint2double(r1, r0); v[1] = __hiloint2double(r3, r2);
+  v[2] = __hiloint2double(r5, r4); v[3] = __hiloint2double(r7, r6);
+}
+constexpr int SPLIT_TMEM_COLS = 128;     // 5 components x 10 slots x 2 columns = 100 -> next power of two
+
 #ifndef SMAUG_SPLIT_MBAR
 #define SMAUG_SPLIT_MBAR 0      // barrier B of the Y role: 0 bar.sync; 1 split-phase mbarrier (arrive after publishing
                                 // C_x, wait after the y-differences) -- measured: no gain (3.310 vs 3.302 ms per stage)
@@ -274,6 +298,18 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
   if (tid == 0) mbar_init(MBAR, NC);
   __syncthreads();
 #endif
+#if SMAUG_SPLIT_TMEM
+  unsigned* const tm_base_sh = reinterpret_cast<unsigned*>(MBAR + 1);
+  if (tid < 32) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(tm_base_sh)), "n"(SPLIT_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const unsigned tm_base = *tm_base_sh;
+#endif
 
   if (tid < NXT) {
     // =================================================================== X role: columns c0, c0 + 1
@@ -450,6 +486,14 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
     int s4 = ND - 3, s5 = 2, s6 = 0;                       // slots of row j in DXR, CXR; of row r in CYR
     int par = 0;                                           // UP buffer of row r
     [[maybe_unused]] int mph = 0;                          // phase parity of barrier B (mbarrier)
+#if SMAUG_SPLIT_TMEM
+    // C_y ring in tensor memory: component f at columns 20 f .. 20 f + 19 = ten slots of one double; row k is
+    // written to slots (k mod 5) and (k mod 5) + 5, so that any four consecutive rows are four consecutive slots
+    const unsigned tm_y = tm_base + ((unsigned)(((tid >> 5) & 3) * 32) << 16);
+    int p5 = 4;                                            // slot class of row r - 1
+    int yst = 1;                                           // staging buffer holding C_y(r - 1)
+    double cyv[5] = {0.0, 0.0, 0.0, 0.0, 0.0};             // C_y(r - 1) of this column
+#endif
     if (DEC) bar_arrive<4, NTH>();                         // E for the first row: nothing to wait for
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
@@ -512,11 +556,25 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       for (int k = 0; k < 5; ++k) { hr[k] = hr[k + 1]; hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; he[k] = he[k + 1]; hbx[k] = hbx[k + 1]; }
       hr[5] = UPr[0 * PW + tp]; hvx[5] = UPr[1 * PW + tp]; hvy[5] = UPr[2 * PW + tp]; he[5] = UPr[3 * PW + tp];
       hbx[5] = UPr[5 * PW + tp];
+#if SMAUG_SPLIT_TMEM
+      // C_y(r - 1), which X wrote at the end of its step r - 1, from the staging buffer into the ring
+#pragma unroll
+      for (int f = 0; f < 5; ++f) cyv[f] = CYR[(yst * 5 + f) * NC + c];
+      asm volatile("" ::"d"(cyv[0]), "d"(cyv[1]), "d"(cyv[2]), "d"(cyv[3]), "d"(cyv[4]) : "memory");
+#endif
       if (DEC) {
         // E: UP may be overwritten (the loads above must have landed: consume them first)
         asm volatile("" ::"d"(hr[5]), "d"(hvx[5]), "d"(hvy[5]), "d"(he[5]), "d"(hbx[5]) : "memory");
         if (r + 1 < yend + NG) bar_arrive<4, NTH>();
       }
+#if SMAUG_SPLIT_TMEM
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        tm_st(tm_y + 20 * f + 2 * p5, cyv[f]);
+        tm_st(tm_y + 20 * f + 2 * p5 + 10, cyv[f]);
+      }
+      tm_wait_st();
+#endif
 
       // ---------------------------------------------------------------- y-interface (j | j+1)
       double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -579,10 +637,21 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-NY ring
         auto back = [&](int k) { const int q = s6 + (NY - k); return q >= NY ? q - NY : q; };   // slot of row r - k
         const int jm2 = back(5), jm1 = back(4), jp1 = back(2), jp2 = back(1);
+#if SMAUG_SPLIT_TMEM
+        (void)jm2; (void)jm1; (void)jp1; (void)jp2;
+        const int q5 = p5 == 4 ? 0 : p5 + 1;              // slot of row r - 5; rows r-5 .. r-2 follow each other
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          double v[4];
+          tm_ld4(tm_y + 20 * f + 2 * q5, v);
+          cdyi[f] = cd12v(v[0], v[1], v[3], cyv[f]) * idy_;
+        }
+#else
 #pragma unroll
         for (int f = 0; f < 5; ++f)
           cdyi[f] = cd12v(CYR[(jm2 * 5 + f) * NC + c], CYR[(jm1 * 5 + f) * NC + c], CYR[(jp1 * 5 + f) * NC + c],
                           CYR[(jp2 * 5 + f) * NC + c]) * idy_;
+#endif
       }
 #if SMAUG_SPLIT_MBAR
       mbar_wait(MBAR, mph);
@@ -660,12 +729,22 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       s5 = s5 == 4 ? 0 : s5 + 1;
       s6 = s6 == NY - 1 ? 0 : s6 + 1;
       if (!DEC) par ^= 1;
+#if SMAUG_SPLIT_TMEM
+      p5 = p5 == 4 ? 0 : p5 + 1;
+      yst ^= 1;
+#endif
     }
   }
   if (WS != WS_NONE) {
     __syncthreads();      // red_sh aliases the landing zone of the X warps
     block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], WS == WS_FULL ? 0 : 2);
   }
+#if SMAUG_SPLIT_TMEM
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (tid < 32)
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base), "n"(SPLIT_TMEM_COLS) : "memory");
+#endif
 }
 
 }  // namespace smaug
