@@ -238,11 +238,11 @@ int pick_rows_per_cta(int ny, int strips, int n_sm, int warm_rows = 2 * NG) {
   return best_rows;
 }
 
-template <int COMBINE, int WS>
+template <int COMBINE, int WS, bool BG = false>
 int launch_split_t(smaug_ctx* c, const StageArgs& a) {
   static bool configured = false;
-  constexpr size_t smem = SplitSmem<SPLIT_NC>::BYTES;
-  auto kern = split_kernel<SPLIT_NC, COMBINE, WS>;
+  constexpr size_t smem = SplitSmem<SPLIT_NC, BG>::BYTES;
+  auto kern = split_kernel<SPLIT_NC, COMBINE, WS, BG>;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
@@ -250,7 +250,7 @@ int launch_split_t(smaug_ctx* c, const StageArgs& a) {
   const int W = SPLIT_NC - 8;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
-  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * SplitSmem<SPLIT_NC>::CTAS_PER_SM);
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * SplitSmem<SPLIT_NC, BG>::CTAS_PER_SM);
   const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
   dim3 grid(strips, nchunks);
   c->last_ctas = strips * nchunks;
@@ -267,8 +267,16 @@ int launch_split_t(smaug_ctx* c, const StageArgs& a) {
   return SMAUG_OK;
 }
 
-// Role-split streaming form (smaug_split_kernel.cuh): no background, hyperdiffusion on.
+// Role-split streaming form (smaug_split_kernel.cuh): hyperdiffusion on; BG instantiations for a background
+// (with or without gravity).
 int launch_split(smaug_ctx* c, const StageArgs& a) {
+  if (c->has_bg) {
+    if (a.combine == COMBINE_BASE && a.ws_mode == WS_VT) return launch_split_t<COMBINE_BASE, WS_VT, true>(c, a);
+    if (a.combine == COMBINE_ACC && a.ws_mode == WS_VT) return launch_split_t<COMBINE_ACC, WS_VT, true>(c, a);
+    if (a.combine == COMBINE_FINAL && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_FINAL, WS_FULL, true>(c, a);
+    if (a.combine == COMBINE_BASE && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_BASE, WS_FULL, true>(c, a);
+    return fail(SMAUG_EINVAL, "split kernel: unsupported combine / wave-speed mode");
+  }
   if (a.combine == COMBINE_BASE && a.ws_mode == WS_VT) return launch_split_t<COMBINE_BASE, WS_VT>(c, a);
   if (a.combine == COMBINE_ACC && a.ws_mode == WS_VT) return launch_split_t<COMBINE_ACC, WS_VT>(c, a);
   if (a.combine == COMBINE_FINAL && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_FINAL, WS_FULL>(c, a);
@@ -314,7 +322,8 @@ int launch_flux(smaug_ctx* c, const StageArgs& a) {
 // runs in the tiled kernel.
 bool plain(const smaug_ctx* c) { return !c->has_bg && c->gx == 0.0 && c->gy == 0.0; }
 bool uses_flux(const smaug_ctx* c) { return plain(c) && !c->hd_on && c->kernel_mode != 0; }
-bool uses_split(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 2; }
+// (gravity without a background stays in the tiled kernel: the BG form of the split kernel reads background planes)
+bool uses_split(const smaug_ctx* c) { return (plain(c) || c->has_bg) && c->hd_on && c->kernel_mode == 2; }
 bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 1; }
 
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
@@ -721,7 +730,7 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
     out[3] = (int)FluxSmem<FLUX_NT>::BYTES;
   } else if (uses_split(c)) {   // role-split streaming kernel: a strip of NC-8 columns
     out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
-    out[3] = (int)SplitSmem<SPLIT_NC>::BYTES;
+    out[3] = (int)(c->has_bg ? SplitSmem<SPLIT_NC, true>::BYTES : SplitSmem<SPLIT_NC>::BYTES);
   } else if (uses_march(c)) {   // streaming kernel: a strip of NT-6 columns
     out[0] = MARCH_NT - 2 * NG; out[1] = 1; out[2] = MARCH_NT;
     out[3] = (int)MarchSmem<MARCH_NT>::BYTES;

@@ -36,7 +36,7 @@
 
 namespace smaug {
 
-template <int NC>
+template <int NC, bool BG = false>
 struct SplitSmem {
   static constexpr int PW = NC + 8;                     // padded plane width (index c + 4)
   // DEC (SMAUG_SPLIT_DECOUPLE): the X warps may run one row ahead of the Y warps (producer / consumer
@@ -45,18 +45,22 @@ struct SplitSmem {
   static constexpr bool DEC = SMAUG_SPLIT_DECOUPLE != 0;
   static constexpr int NUP = DEC ? 1 : 2;               // UP buffers
   static constexpr int ND = DEC ? 5 : 4;                // rows in DXR
-  static constexpr bool TM = SMAUG_SPLIT_TMEM != 0;
+  static constexpr bool TM = BG || SMAUG_SPLIT_TMEM != 0;     // the background form needs the room
   static_assert(!TM || DEC, "SMAUG_SPLIT_TMEM needs SMAUG_SPLIT_DECOUPLE");
   static constexpr int NY = TM ? 2 : (DEC ? 7 : 6);     // rows in CYR (TM: a two-row staging buffer)
-  static constexpr int OFF_UP = 0;                      // NUP x 6 planes: rho, vx, vy, eps, by, bx of the head row
-  static constexpr int OFF_PK = OFF_UP + NUP * 6 * PW;  // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
+  static constexpr int NUPP = BG ? 8 : 6;               // planes of one UP buffer
+  static constexpr int NIN = BG ? NF + NBG : NF;        // fields in the landing zone
+  static constexpr int OFF_UP = 0;                      // NUP x NUPP planes: rho, vx, vy, eps, by~, bx~ of the head row
+                                                        // (BG: rho is the total density; + rho~, total By)
+  static constexpr int OFF_PK = OFF_UP + NUP * NUPP * PW;  // 7 planes: Phi_x[5], kappa_x(vy), kappa_x(by)
   static constexpr int OFF_CXR = OFF_PK + 7 * PW;       // ring 5 rows x 5 planes: F_x, then C_x
-  static constexpr int OFF_BYR = OFF_CXR + 25 * PW;     // ring 5 rows: by
+  static constexpr int OFF_BYR = OFF_CXR + 25 * PW;     // ring 5 rows: by~
   static constexpr int OFF_DXR = OFF_BYR + 5 * NC;      // ring ND rows x 5: Phi_x differences
   static constexpr int OFF_CYR = OFF_DXR + ND * 5 * NC; // ring NY rows x 5: C_y
-  static constexpr int OFF_INR = OFF_CYR + NY * 5 * NC; // cp.async landing zone of the next input row (6 fields)
+  static constexpr int OFF_VJ = OFF_CYR + NY * 5 * NC;  // BG: 2 buffers x 2 planes: vx, vy of the tail row (for S_e)
+  static constexpr int OFF_INR = OFF_VJ + (BG ? 4 * PW : 0);  // cp.async landing zone of the next input row
   static constexpr int OFF_RED = OFF_INR;               // block reduction scratch (after the march: INR is dead)
-  static constexpr int OFF_MBAR = OFF_INR + (6 * NC > 4 * 32 ? 6 * NC : 4 * 32);   // one mbarrier (barrier B of Y)
+  static constexpr int OFF_MBAR = OFF_INR + (NIN * NC > 4 * 32 ? NIN * NC : 4 * 32);   // one mbarrier (barrier B of Y)
   static constexpr int TOTAL = OFF_MBAR + 2;
   static constexpr int CTAS_PER_SM = NC <= 64 ? 4 : (NC <= 128 ? 2 : 1);
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
@@ -268,14 +272,15 @@ __device__ __forceinline__ void split_wavespeeds(const double (&o)[NF], double g
   }
 }
 
-template <int NC, int COMBINE, int WS>
+template <int NC, int COMBINE, int WS, bool BG = false>
 #ifdef SMAUG_SPLIT_MAXNREG
 __global__ void __maxnreg__(SMAUG_SPLIT_MAXNREG) split_kernel
 #else
-__global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split_kernel
+__global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) split_kernel
 #endif
 (const StageArgs a, const MarchGeom mg) {
-  using S = SplitSmem<NC>;
+  using S = SplitSmem<NC, BG>;
+  constexpr bool TM = S::TM;
   constexpr int PW = S::PW, NXT = NC / 2, NTH = NC + NC / 2;
   extern __shared__ __align__(16) double smem[];
   double* const UP = smem + S::OFF_UP;
@@ -298,7 +303,8 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
   if (tid == 0) mbar_init(MBAR, NC);
   __syncthreads();
 #endif
-#if SMAUG_SPLIT_TMEM
+  unsigned tm_base = 0;
+  if constexpr (TM) {
   unsigned* const tm_base_sh = reinterpret_cast<unsigned*>(MBAR + 1);
   if (tid < 32) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
@@ -308,8 +314,8 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const unsigned tm_base = *tm_base_sh;
-#endif
+  tm_base = *tm_base_sh;
+  }
 
   if (tid < NXT) {
     // =================================================================== X role: columns c0, c0 + 1
@@ -329,6 +335,10 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       const long long ga = colbase + (long long)min(row, g.ny + NG - 1) * g.pitch;
 #pragma unroll
       for (int f = 0; f < NF; ++f) cp_async16(inr + f * NC, a.in.p[f] + ga);
+      if constexpr (BG) {
+#pragma unroll
+        for (int k = 0; k < NBG; ++k) cp_async16(inr + (NF + k) * NC, a.bg.p[k] + ga);
+      }
       cp_async_commit();
     };
     fetch_row(ystart - NG);
@@ -347,9 +357,42 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         rho[0] = q0.x; rho[1] = q0.y; mx[0] = q1.x; mx[1] = q1.y; my[0] = q2.x; my[1] = q2.y;
         et[0] = q3.x; et[1] = q3.y; bx[0] = q4.x; bx[1] = q4.y; by[0] = q5.x; by[1] = q5.y;
       }
-      double* const UPr = UP + par * 6 * PW;
+      double* const UPr = UP + par * S::NUPP * PW;
       // ---------------------------------------------------------------- derived quantities, F_x, F_y of row r
+      // (BG: c-2 with the background terms; rho[] becomes the total density, rhot[] keeps the perturbation,
+      //  Bxt / Byt are the total field; without a background these coincide and the extra terms are exact zeros)
       double vx[2], vy[2], eps[2], cyn[2][5], fx[2][5];
+      [[maybe_unused]] double rhot[2] = {rho[0], rho[1]}, Bxt[2] = {bx[0], bx[1]}, Byt[2] = {by[0], by[1]};
+      if constexpr (BG) {
+        const double2 g0 = lds2(inr + (NF + BG_RHO) * NC), g1 = lds2(inr + (NF + BG_E) * NC);
+        const double2 g2 = lds2(inr + (NF + BG_BX) * NC), g3 = lds2(inr + (NF + BG_BY) * NC);
+        const double rb[2] = {g0.x, g0.y}, eb[2] = {g1.x, g1.y}, Bbx[2] = {g2.x, g2.y}, Bby[2] = {g3.x, g3.y};
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+          rho[q] = rb[q] + rhot[q];
+          const double rr = drcp(rho[q]);
+          vx[q] = mx[q] * rr; vy[q] = my[q] * rr;
+          const double b2h = 0.5 * fma(by[q], by[q], bx[q] * bx[q]);
+          const double cross = fma(Bby[q], by[q], Bbx[q] * bx[q]);
+          const double ke = 0.5 * fma(my[q], vy[q], mx[q] * vx[q]);
+          eps[q] = ((et[q] - ke) - cross) - b2h;
+          const double ptt = fma(gm1, eps[q], cross + b2h);
+          Bxt[q] = Bbx[q] + bx[q]; Byt[q] = Bby[q] + by[q];
+          const double btv = fma(by[q], vy[q], bx[q] * vx[q]);
+          const double Bbv = fma(Bby[q], vy[q], Bbx[q] * vx[q]);
+          const double h = (et[q] + eb[q]) + ptt;
+          cyn[q][C_RHO] = rho[q] * vy[q];
+          cyn[q][C_MX] = (fma(mx[q], vy[q], -(bx[q] * by[q])) - bx[q] * Bby[q]) - Bbx[q] * by[q];
+          cyn[q][C_MY] = ((fma(my[q], vy[q], -(by[q] * by[q])) - by[q] * Bby[q]) - Bby[q] * by[q]) + ptt;
+          cyn[q][C_E] = (fma(vy[q], h, -(by[q] * btv)) - by[q] * Bbv) - Bby[q] * btv;
+          cyn[q][C_B] = fma(vy[q], Bxt[q], -(Byt[q] * vx[q]));
+          fx[q][C_RHO] = rho[q] * vx[q];
+          fx[q][C_MX] = ((fma(mx[q], vx[q], -(bx[q] * bx[q])) - bx[q] * Bbx[q]) - Bbx[q] * bx[q]) + ptt;
+          fx[q][C_MY] = (fma(my[q], vx[q], -(by[q] * bx[q])) - by[q] * Bbx[q]) - Bby[q] * bx[q];
+          fx[q][C_E] = (fma(vx[q], h, -(bx[q] * btv)) - bx[q] * Bbv) - Bbx[q] * btv;
+          fx[q][C_B] = fma(vx[q], Byt[q], -(Bxt[q] * vy[q]));
+        }
+      } else {
 #pragma unroll
       for (int q = 0; q < 2; ++q) {
         const double rr = drcp(rho[q]);
@@ -371,10 +414,12 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         fx[q][C_E] = fma(vx[q], h, -(bx[q] * btv));
         fx[q][C_B] = fma(vx[q], by[q], -(bx[q] * vy[q]));
       }
+      }
       if (DEC) role_barrier<4, NTH>();      // ---- E: every warp is done with UP of the previous row
       sts2(UPr + 0 * PW + tp, rho[0], rho[1]); sts2(UPr + 1 * PW + tp, vx[0], vx[1]);
       sts2(UPr + 2 * PW + tp, vy[0], vy[1]);   sts2(UPr + 3 * PW + tp, eps[0], eps[1]);
       sts2(UPr + 4 * PW + tp, by[0], by[1]);   sts2(UPr + 5 * PW + tp, bx[0], bx[1]);
+      if constexpr (BG) { sts2(UPr + 6 * PW + tp, rhot[0], rhot[1]); sts2(UPr + 7 * PW + tp, Byt[0], Byt[1]); }
 #pragma unroll
       for (int f = 0; f < 5; ++f) sts2(CXR + (s5 * 5 + f) * PW + tp, fx[0][f], fx[1][f]);
       sts2(BYR + s5 * NC + c0, by[0], by[1]);
@@ -397,9 +442,11 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           u[0] = l.x; u[1] = l.y; u[2] = o0; u[3] = o1; u[4] = rgt.x; u[5] = rgt.y;
           u[6] = UPr[plane * PW + tp + 4];
         };
-        gather(0, rho[0], rho[1]);
+        // kappa_x(rho~) on the perturbed density; the interface weights rho-bar use the total density
+        if constexpr (BG) gather(6, rhot[0], rhot[1]); else gather(0, rho[0], rho[1]);
         kappa7<GUARD>(u, cv_rho, k0, k1, d0, d1, lo);
-        const double rbar0 = 0.5 * (u[2] + u[3]), rbar1 = 0.5 * (u[3] + u[4]);
+        const double rho_r = BG ? UPr[0 * PW + tp + 2] : u[4];           // total density of the cell right of the pair
+        const double rbar0 = 0.5 * (rho[0] + rho[1]), rbar1 = 0.5 * (rho[1] + rho_r);
         px[0][C_RHO] = k0 * d0; px[1][C_RHO] = k1 * d1;
         gather(1, vx[0], vx[1]);
         kappa7<GUARD>(u, cv_mom, k0, k1, d0, d1, lo);
@@ -417,8 +464,10 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         kappa7<GUARD>(u, cv_b, kxb[0], kxb[1], d0, d1, lo);
         px[0][C_B] = kxb[0] * d0; px[1][C_B] = kxb[1] * d1;
         dcx_by[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_by[1] = cd12v(u[1], u[2], u[4], u[5]);
-        px[0][C_E] = fma(0.5 * (u[2] + u[3]), px[0][C_B], fma(vybar0, px[0][C_MY], fma(vxbar0, px[0][C_MX], p_eps0)));
-        px[1][C_E] = fma(0.5 * (u[3] + u[4]), px[1][C_B], fma(vybar1, px[1][C_MY], fma(vxbar1, px[1][C_MX], p_eps1)));
+        // ohmic coupling with the TOTAL transverse field (u[] holds by~ here)
+        const double By_r = BG ? UPr[7 * PW + tp + 2] : u[4];
+        px[0][C_E] = fma(0.5 * (Byt[0] + Byt[1]), px[0][C_B], fma(vybar0, px[0][C_MY], fma(vxbar0, px[0][C_MX], p_eps0)));
+        px[1][C_E] = fma(0.5 * (Byt[1] + By_r), px[1][C_B], fma(vybar1, px[1][C_MY], fma(vxbar1, px[1][C_MX], p_eps1)));
         return lo;
       };
       // SMAUG_SPLIT_SPEC: speculate that every M1 of this warp's row step is an ordinary number and redo the
@@ -450,7 +499,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         sts2(cy + C_RHO * NC, cyn[0][C_RHO], cyn[1][C_RHO]);
         sts2(cy + C_MX * NC, cyn[0][C_MX] - gm0, cyn[1][C_MX] - gm1_);
         sts2(cy + C_MY * NC, cyn[0][C_MY], cyn[1][C_MY]);
-        sts2(cy + C_E * NC, cyn[0][C_E] - fma(vx[0], gm0, bx[0] * gb0), cyn[1][C_E] - fma(vx[1], gm1_, bx[1] * gb1));
+        sts2(cy + C_E * NC, cyn[0][C_E] - fma(vx[0], gm0, Bxt[0] * gb0), cyn[1][C_E] - fma(vx[1], gm1_, Bxt[1] * gb1));
         sts2(cy + C_B * NC, cyn[0][C_B] - gb0, cyn[1][C_B] - gb1);
       }
       s4 = s4 == ND - 1 ? 0 : s4 + 1;
@@ -486,14 +535,15 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
     int s4 = ND - 3, s5 = 2, s6 = 0;                       // slots of row j in DXR, CXR; of row r in CYR
     int par = 0;                                           // UP buffer of row r
     [[maybe_unused]] int mph = 0;                          // phase parity of barrier B (mbarrier)
-#if SMAUG_SPLIT_TMEM
-    // C_y ring in tensor memory: component f at columns 20 f .. 20 f + 19 = ten slots of one double; row k is
+    // (TM) C_y ring in tensor memory: component f at columns 20 f .. 20 f + 19 = ten slots of one double; row k is
     // written to slots (k mod 5) and (k mod 5) + 5, so that any four consecutive rows are four consecutive slots
-    const unsigned tm_y = tm_base + ((unsigned)(((tid >> 5) & 3) * 32) << 16);
-    int p5 = 4;                                            // slot class of row r - 1
-    int yst = 1;                                           // staging buffer holding C_y(r - 1)
-    double cyv[5] = {0.0, 0.0, 0.0, 0.0, 0.0};             // C_y(r - 1) of this column
-#endif
+    [[maybe_unused]] const unsigned tm_y = tm_base + ((unsigned)(((tid >> 5) & 3) * 32) << 16);
+    [[maybe_unused]] int p5 = 4;                           // slot class of row r - 1
+    [[maybe_unused]] int yst = 1;                          // staging buffer holding C_y(r - 1)
+    [[maybe_unused]] double cyv[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // C_y(r - 1) of this column
+    [[maybe_unused]] double* const VJ = smem + S::OFF_VJ;  // BG: vx, vy of the tail row, two buffers
+    [[maybe_unused]] int vjb = 0;
+    [[maybe_unused]] const double gm1y = a.prm.gamma - 1.0;
     if (DEC) bar_arrive<4, NTH>();                         // E for the first row: nothing to wait for
     // (row r starts in slot 0 of every ring; row j = r - 3 is then at -3 mod 4 = 1 and -3 mod 5 = 2)
 
@@ -551,31 +601,42 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
 #endif
       if (DEC) role_barrier<3, NTH>();                                // ---- F: head row r is published
       else cta_barrier<NTH>();                                        // ---- A (both roles)
-      const double* const UPr = UP + par * 6 * PW;
+      const double* const UPr = UP + par * S::NUPP * PW;
 #pragma unroll
       for (int k = 0; k < 5; ++k) { hr[k] = hr[k + 1]; hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; he[k] = he[k + 1]; hbx[k] = hbx[k + 1]; }
-      hr[5] = UPr[0 * PW + tp]; hvx[5] = UPr[1 * PW + tp]; hvy[5] = UPr[2 * PW + tp]; he[5] = UPr[3 * PW + tp];
+      hr[5] = UPr[(BG ? 6 : 0) * PW + tp]; hvx[5] = UPr[1 * PW + tp]; hvy[5] = UPr[2 * PW + tp]; he[5] = UPr[3 * PW + tp];
       hbx[5] = UPr[5 * PW + tp];
-#if SMAUG_SPLIT_TMEM
-      // C_y(r - 1), which X wrote at the end of its step r - 1, from the staging buffer into the ring
+      if constexpr (TM) {
+        // C_y(r - 1), which X wrote at the end of its step r - 1, from the staging buffer into the ring
 #pragma unroll
-      for (int f = 0; f < 5; ++f) cyv[f] = CYR[(yst * 5 + f) * NC + c];
-      asm volatile("" ::"d"(cyv[0]), "d"(cyv[1]), "d"(cyv[2]), "d"(cyv[3]), "d"(cyv[4]) : "memory");
-#endif
+        for (int f = 0; f < 5; ++f) cyv[f] = CYR[(yst * 5 + f) * NC + c];
+        asm volatile("" ::"d"(cyv[0]), "d"(cyv[1]), "d"(cyv[2]), "d"(cyv[3]), "d"(cyv[4]) : "memory");
+      }
       if (DEC) {
         // E: UP may be overwritten (the loads above must have landed: consume them first)
         asm volatile("" ::"d"(hr[5]), "d"(hvx[5]), "d"(hvy[5]), "d"(he[5]), "d"(hbx[5]) : "memory");
         if (r + 1 < yend + NG) bar_arrive<4, NTH>();
       }
-#if SMAUG_SPLIT_TMEM
+      if constexpr (TM) {
 #pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        tm_st(tm_y + 20 * f + 2 * p5, cyv[f]);
-        tm_st(tm_y + 20 * f + 2 * p5 + 10, cyv[f]);
+        for (int f = 0; f < 5; ++f) {
+          tm_st(tm_y + 20 * f + 2 * p5, cyv[f]);
+          tm_st(tm_y + 20 * f + 2 * p5 + 10, cyv[f]);
+        }
+        tm_wait_st();
       }
-      tm_wait_st();
-#endif
 
+      // BG: background of rows j and j + 1 at this column (L2 hits: X fetched these rows three steps ago); the
+      // totals are rebuilt with the oracle's own operations (rho = rho_b + rho~, B = B_b + b~)
+      [[maybe_unused]] double rb0 = 0.0, rb1 = 0.0, Bbx0 = 0.0, Bbx1 = 0.0, eb0 = 0.0, Bby0 = 0.0;
+      if constexpr (BG) {
+        if (ky_on) {
+          const unsigned gq = tail_on ? gj : gj - upitch;            // (cl, row j)
+          rb0 = a.bg.p[BG_RHO][gq]; rb1 = a.bg.p[BG_RHO][gq + upitch];
+          Bbx0 = a.bg.p[BG_BX][gq]; Bbx1 = a.bg.p[BG_BX][gq + upitch];
+          if (tail_on) { eb0 = a.bg.p[BG_E][gq]; Bby0 = a.bg.p[BG_BY][gq]; }
+        }
+      }
       // ---------------------------------------------------------------- y-interface (j | j+1)
       double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       double kyv = 0.0, kyb = 0.0;
@@ -588,14 +649,15 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         const double k_vy = kappa6m<GUARD>(hvy[0], hvy[1], hvy[2], hvy[3], hvy[4], hvy[5], cv_mom, d_vy, lo);
         const double k_e = kappa6m<GUARD>(he[0], he[1], he[2], he[3], he[4], he[5], cv_e, d_e, lo);
         kyb = kappa6m<GUARD>(hbx[0], hbx[1], hbx[2], hbx[3], hbx[4], hbx[5], cv_b, d_bx, lo);
-        const double rbar = 0.5 * (hr[2] + hr[3]);
+        const double rbar = BG ? 0.5 * ((rb0 + hr[2]) + (rb1 + hr[3])) : 0.5 * (hr[2] + hr[3]);
         const double p_rho = k_rho * d_rho;
         const double p_mx = ((0.5 * rbar) * kyv) * d_vx;
         const double p_my = (rbar * k_vy) * d_vy;
         const double p_eps = k_e * d_e;
         const double p_b = kyb * d_bx;
         py[C_RHO] = p_rho; py[C_MX] = p_mx; py[C_MY] = p_my; py[C_B] = p_b;
-        py[C_E] = fma(0.5 * (hbx[2] + hbx[3]), p_b,
+        const double Bbar = BG ? 0.5 * ((Bbx0 + hbx[2]) + (Bbx1 + hbx[3])) : 0.5 * (hbx[2] + hbx[3]);
+        py[C_E] = fma(Bbar, p_b,
                       fma(0.5 * (hvy[2] + hvy[3]), p_my, fma(0.5 * (hvx[2] + hvx[3]), p_mx, p_eps)));
         return lo;
       };
@@ -613,7 +675,8 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         // G(my ; x), G(by ; x) and their energy companion at row j (histories index 2); C_x = F_x - G
         const double kv = 0.5 * (kyv_prev + kyv);
         const double kb = 0.5 * (kyb_prev + kyb);
-        const double gm = ((0.5 * hr[2]) * kv) * (cd12v(hvx[0], hvx[1], hvx[3], hvx[4]) * (1.0 / 12.0));
+        const double rho_j = BG ? rb0 + hr[2] : hr[2];               // total density of the tail cell
+        const double gm = ((0.5 * rho_j) * kv) * (cd12v(hvx[0], hvx[1], hvx[3], hvx[4]) * (1.0 / 12.0));
         const double gb = -(kb * (cd12v(hbx[0], hbx[1], hbx[3], hbx[4]) * (1.0 / 12.0)));
         double* cx = CXR + s5 * 5 * PW + tp;
         const double jby = BYR[s5 * NC + c];
@@ -621,8 +684,12 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         if (COMBINE != COMBINE_BASE) { jin[F_RHO] = hr[2]; jin[F_BX] = hbx[2]; jin[F_BY] = jby; }
 #endif
         cx[C_MY * PW] = cx[C_MY * PW] - gm;
-        cx[C_E * PW] = cx[C_E * PW] - fma(hvy[2], gm, jby * gb);
+        cx[C_E * PW] = cx[C_E * PW] - fma(hvy[2], gm, (BG ? Bby0 + jby : jby) * gb);
         cx[C_B * PW] = cx[C_B * PW] - gb;
+        if constexpr (BG) {       // vx, vy of the tail row for the x-derivatives of S_e (read after barrier B)
+          VJ[(vjb * 2 + 0) * PW + tp] = hvx[2];
+          VJ[(vjb * 2 + 1) * PW + tp] = hvy[2];
+        }
       }
 #if SMAUG_SPLIT_MBAR
       mbar_arrive(MBAR);                                              // ---- B (Y warps only): C_x(j) published
@@ -637,21 +704,20 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
         // rows j-2, j-1, j+1, j+2 = r-5, r-4, r-2, r-1 in the mod-NY ring
         auto back = [&](int k) { const int q = s6 + (NY - k); return q >= NY ? q - NY : q; };   // slot of row r - k
         const int jm2 = back(5), jm1 = back(4), jp1 = back(2), jp2 = back(1);
-#if SMAUG_SPLIT_TMEM
-        (void)jm2; (void)jm1; (void)jp1; (void)jp2;
-        const int q5 = p5 == 4 ? 0 : p5 + 1;              // slot of row r - 5; rows r-5 .. r-2 follow each other
+        if constexpr (TM) {
+          const int q5 = p5 == 4 ? 0 : p5 + 1;            // slot of row r - 5; rows r-5 .. r-2 follow each other
 #pragma unroll
-        for (int f = 0; f < 5; ++f) {
-          double v[4];
-          tm_ld4(tm_y + 20 * f + 2 * q5, v);
-          cdyi[f] = cd12v(v[0], v[1], v[3], cyv[f]) * idy_;
+          for (int f = 0; f < 5; ++f) {
+            double v[4];
+            tm_ld4(tm_y + 20 * f + 2 * q5, v);
+            cdyi[f] = cd12v(v[0], v[1], v[3], cyv[f]) * idy_;
+          }
+        } else {
+#pragma unroll
+          for (int f = 0; f < 5; ++f)
+            cdyi[f] = cd12v(CYR[(jm2 * 5 + f) * NC + c], CYR[(jm1 * 5 + f) * NC + c], CYR[(jp1 * 5 + f) * NC + c],
+                            CYR[(jp2 * 5 + f) * NC + c]) * idy_;
         }
-#else
-#pragma unroll
-        for (int f = 0; f < 5; ++f)
-          cdyi[f] = cd12v(CYR[(jm2 * 5 + f) * NC + c], CYR[(jm1 * 5 + f) * NC + c], CYR[(jp1 * 5 + f) * NC + c],
-                          CYR[(jp2 * 5 + f) * NC + c]) * idy_;
-#endif
       }
 #if SMAUG_SPLIT_MBAR
       mbar_wait(MBAR, mph);
@@ -683,6 +749,26 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
           R[F_E] = fma(cdx[C_E], idx_, cdyi[C_E]) * (-1.0 / 12.0);
           R[F_BX] = cdyi[C_B] * (-1.0 / 12.0);
           R[F_BY] = fma(cdx[C_B], idx_, 0.0) * (-1.0 / 12.0);
+        }
+        if constexpr (BG) {
+          // energy source S_e = -p_tb div v + B_b B_b : grad v (c-2) at the tail cell; then gravity (c-10)
+          const double* vxj = VJ + (vjb * 2 + 0) * PW + tp;
+          const double* vyj = VJ + (vjb * 2 + 1) * PW + tp;
+          const double dxvx = (cd12v(vxj[-2], vxj[-1], vxj[1], vxj[2]) * idx_) * (1.0 / 12.0);
+          const double dxvy = (cd12v(vyj[-2], vyj[-1], vyj[1], vyj[2]) * idx_) * (1.0 / 12.0);
+          const double dyvx = (cd12v(hvx[0], hvx[1], hvx[3], hvx[4]) * idy_) * (1.0 / 12.0);
+          const double dyvy = (cd12v(hvy[0], hvy[1], hvy[3], hvy[4]) * idy_) * (1.0 / 12.0);
+          const double bb2h = 0.5 * fma(Bby0, Bby0, Bbx0 * Bbx0);
+          const double ptb = fma(gm1y, eb0 - bb2h, bb2h);
+          const double S = fma(-ptb, dxvx + dyvy,
+                               fma(Bby0 * Bby0, dyvy, fma(Bbx0 * Bby0, dxvy + dyvx, (Bbx0 * Bbx0) * dxvx)));
+          R[F_E] = R[F_E] + S;
+          if (a.prm.grav_on) {
+            const double rt = hr[2];
+            R[F_MX] = fma(rt, a.prm.gx, R[F_MX]);
+            R[F_MY] = fma(rt, a.prm.gy, R[F_MY]);
+            R[F_E] = fma(rt, fma(a.prm.gy, hvy[2], a.prm.gx * hvx[2]), R[F_E]);
+          }
         }
         const double* dx = DXR + s4 * 5 * NC + c;
         R[F_RHO] = fma(dx[C_RHO * NC], idx_, R[F_RHO]);
@@ -717,7 +803,12 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
               thr0 = gthr0 > thr0 ? gthr0 : thr0;
               thr1 = gthr1 > thr1 ? gthr1 : thr1;
             }
-            split_wavespeeds<WS>(o, gamma, wsmax, thr0, thr1);
+            if constexpr (BG) {
+              const double ot[NF] = {rb0 + o[F_RHO], o[F_MX], o[F_MY], eb0 + o[F_E], Bbx0 + o[F_BX], Bby0 + o[F_BY]};
+              split_wavespeeds<WS>(ot, gamma, wsmax, thr0, thr1);
+            } else {
+              split_wavespeeds<WS>(o, gamma, wsmax, thr0, thr1);
+            }
           }
         }
       }
@@ -729,22 +820,23 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC>::CTAS_PER_SM) split
       s5 = s5 == 4 ? 0 : s5 + 1;
       s6 = s6 == NY - 1 ? 0 : s6 + 1;
       if (!DEC) par ^= 1;
-#if SMAUG_SPLIT_TMEM
-      p5 = p5 == 4 ? 0 : p5 + 1;
-      yst ^= 1;
-#endif
+      if constexpr (TM) {
+        p5 = p5 == 4 ? 0 : p5 + 1;
+        yst ^= 1;
+      }
+      if constexpr (BG) vjb ^= 1;
     }
   }
   if (WS != WS_NONE) {
     __syncthreads();      // red_sh aliases the landing zone of the X warps
     block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], WS == WS_FULL ? 0 : 2);
   }
-#if SMAUG_SPLIT_TMEM
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
-  if (tid < 32)
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base), "n"(SPLIT_TMEM_COLS) : "memory");
-#endif
+  if constexpr (TM) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (tid < 32)
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tm_base), "n"(SPLIT_TMEM_COLS) : "memory");
+  }
 }
 
 }  // namespace smaug
