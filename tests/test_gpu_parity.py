@@ -355,3 +355,27 @@ def test_seeded_sweep_of_configurations(gpu, oracle_mod):
             check(*a, *b)
         except AssertionError as e:
             raise AssertionError(f"case {case}: {w.shape[1:]} bc={bc} bg={bg is not None} {params} steps={steps}: {e}")
+
+
+def test_background_streaming_kernel_against_oracle_and_tile_kernel(gpu, oracle_mod):
+    """The BG form of the role-split streaming kernel (background planes, total fields, S_e, gravity, tensor-memory
+    C_y ring) over several strips and row chunks: against the oracle on every cell, and bit-equal to the tiled
+    kernel (an independently written implementation of the same contract)."""
+    import torch
+    w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(1100, 900)
+    s = gpu.Smaug(1100, 900, gamma, bc, bg=torch.from_numpy(bg), gx=gx, gy=gy)
+    assert s.kernel_name().startswith("split_kernel")
+    s.close()
+    a = gpu_run(gpu, w, bc, gamma, 9, bg=bg, gx=gx, gy=gy)
+    t = gpu_run(gpu, w, bc, gamma, 9, bg=bg, gx=gx, gy=gy, kernel=0)
+    b = cpu_run(oracle_mod, w, bc, gamma, 9, bg=bg, gx=gx, gy=gy, threads=16)
+    check(*a, *b)
+    assert np.array_equal(a[0], t[0]) and a[1] == t[1] and list(a[2]) == list(t[2])
+    # uniform background, periodic, RK2 and fixed boundaries as well
+    W, bcp, gamma = si.orszag_tang(520, 300)
+    bgu = si.uniform_background(520, 300, 0.1, 0.2, 0.05, 0.03)
+    W[0] -= 0.1; W[3] -= 0.2; W[4] -= 0.05; W[5] -= 0.03
+    for bcs, params in ((bcp, {}), (bcp, dict(rk_order=2)), ((2, 1, 0, 0), dict(c_mom=0.2))):
+        a = gpu_run(gpu, W, bcs, gamma, 8, bg=bgu, **params)
+        b = cpu_run(oracle_mod, W, bcs, gamma, 8, bg=bgu, threads=16, **params)
+        check(*a, *b)
