@@ -59,9 +59,9 @@ enum { /* keys of smaug_set_param */
   SMAUG_PARAM_C_B = 6,      /*   0.02 */
   SMAUG_PARAM_RK_ORDER = 7, /* 4 (default), 2 (midpoint) or 1 (forward Euler) */
   SMAUG_PARAM_FIXED_DT = 8, /* > 0: use this dt instead of the CFL step; 0 (default): CFL */
-  SMAUG_PARAM_KERNEL = 9,   /* 2 (default): role-split streaming stage kernel where applicable (no background,
-                               hyperdiffusion on); 1: single-role streaming kernel where applicable; 0: always the
-                               tile kernel.  All are bit-identical; the switch exists for tests and profiling. */
+  SMAUG_PARAM_KERNEL = 9,   /* 2 (default): role-split streaming stage kernel where applicable (hyperdiffusion on;
+                               with or without a background); 1: single-role streaming kernel where applicable
+                               (no background); 0: always the tile kernel.  All are bit-identical; the switch exists for tests and profiling. */
   SMAUG_PARAM_GX = 10,      /* uniform gravitational acceleration g = (GX, GY) of PAPER.md:35 ("rho g", "rho g.v"); */
   SMAUG_PARAM_GY = 11,      /*   default 0.  Split form (c-10): the background is taken to be in magneto-hydrostatic
                                balance  grad p_tb - (B_b.grad)B_b = rho_b g,  so gravity acts on the perturbed
@@ -125,7 +125,8 @@ int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
 /* Name of the fused stage kernel the context's current parameters select (static string, never NULL;
  * "?" for a NULL context): "split_kernel<128>" (role-split streaming form), "march_kernel<256>"
  * (single-role streaming form), "flux_kernel<128>" (streaming form without hyperdiffusion) or
- * "stage_kernel<32,8,512>" (tiled form: with a background, or forced by SMAUG_PARAM_KERNEL = 0). */
+ * "stage_kernel<32,8,512>" (tiled form: gravity without a background, a background without hyperdiffusion, or
+ * forced by SMAUG_PARAM_KERNEL = 0). */
 const char* smaug_get_kernel_name(smaug_ctx* ctx);
 
 /* Device time, in milliseconds, spent in the fused stage kernels (summed over launches) and the number of

@@ -1,6 +1,6 @@
-// smaug_split_kernel.cuh -- the role-split streaming form of the fused stage kernel (no background,
-// hyperdiffusion on: the benchmark configurations).  Same arithmetic contract as every other stage kernel
-// (DESIGN.md section 4): bit-identical to the oracle.
+// smaug_split_kernel.cuh -- the role-split streaming form of the fused stage kernel (hyperdiffusion on; BG = false:
+// zero background, the benchmark configurations; BG = true: a background, with or without gravity).  Same
+// arithmetic contract as every other stage kernel: bit-identical to the oracle.
 //
 // One CTA owns a strip of NC columns (NC - 8 of them produce output, 4 halo columns on each side so that
 // column pairs are 16-byte aligned) and marches down a chunk of rows, newest ("head") row r, output ("tail")
@@ -20,6 +20,12 @@
 // 4 rows), CYR (C_y; 6 rows).  Two CTA-wide barriers per row (A: UP/CXR published, B: PK/C_x published) order
 // every write against every read (ring depths chosen so that a slot is never rewritten in the barrier
 // interval in which it is read).  12 warps per SM at <= 168 registers instead of 8 at 240.
+//
+// BG = true adds: the four background planes of the head row in the landing zone; total density / total By planes
+// beside the perturbed ones in UP; the totals of the tail rows rebuilt in the Y role from background values it
+// loads itself; the energy source S_e from a two-buffer exchange of the tail row's vx, vy; gravity; and -- to make
+// room for all that -- the C_y ring in TENSOR MEMORY (thread-private columns, tcgen05.st / tcgen05.ld) with a
+// two-row staging buffer in shared memory.
 #pragma once
 #include <type_traits>
 
