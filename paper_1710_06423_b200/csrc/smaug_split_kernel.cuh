@@ -605,6 +605,17 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) s
         }
       }
 #endif
+      // BG: background of rows j and j + 1 at this column (L2 hits: X fetched these rows three steps ago); the
+      // totals are rebuilt with the oracle's own operations (rho = rho_b + rho~, B = B_b + b~)
+      [[maybe_unused]] double rb0 = 0.0, rb1 = 0.0, Bbx0 = 0.0, Bbx1 = 0.0, eb0 = 0.0, Bby0 = 0.0;
+      if constexpr (BG) {
+        if (ky_on) {
+          const unsigned gq = tail_on ? gj : gj - upitch;            // (cl, row j)
+          rb0 = a.bg.p[BG_RHO][gq]; rb1 = a.bg.p[BG_RHO][gq + upitch];
+          Bbx0 = a.bg.p[BG_BX][gq]; Bbx1 = a.bg.p[BG_BX][gq + upitch];
+          if (tail_on) { eb0 = a.bg.p[BG_E][gq]; Bby0 = a.bg.p[BG_BY][gq]; }
+        }
+      }
       if (DEC) role_barrier<3, NTH>();                                // ---- F: head row r is published
       else cta_barrier<NTH>();                                        // ---- A (both roles)
       const double* const UPr = UP + par * S::NUPP * PW;
@@ -632,17 +643,6 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) s
         tm_wait_st();
       }
 
-      // BG: background of rows j and j + 1 at this column (L2 hits: X fetched these rows three steps ago); the
-      // totals are rebuilt with the oracle's own operations (rho = rho_b + rho~, B = B_b + b~)
-      [[maybe_unused]] double rb0 = 0.0, rb1 = 0.0, Bbx0 = 0.0, Bbx1 = 0.0, eb0 = 0.0, Bby0 = 0.0;
-      if constexpr (BG) {
-        if (ky_on) {
-          const unsigned gq = tail_on ? gj : gj - upitch;            // (cl, row j)
-          rb0 = a.bg.p[BG_RHO][gq]; rb1 = a.bg.p[BG_RHO][gq + upitch];
-          Bbx0 = a.bg.p[BG_BX][gq]; Bbx1 = a.bg.p[BG_BX][gq + upitch];
-          if (tail_on) { eb0 = a.bg.p[BG_E][gq]; Bby0 = a.bg.p[BG_BY][gq]; }
-        }
-      }
       // ---------------------------------------------------------------- y-interface (j | j+1)
       double py[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       double kyv = 0.0, kyb = 0.0;
