@@ -238,11 +238,11 @@ int pick_rows_per_cta(int ny, int strips, int n_sm, int warm_rows = 2 * NG) {
   return best_rows;
 }
 
-template <int COMBINE, int WS, bool BG = false>
+template <int COMBINE, int WS, bool BG = false, bool GRAV = false>
 int launch_split_t(smaug_ctx* c, const StageArgs& a) {
   static bool configured = false;
   constexpr size_t smem = SplitSmem<SPLIT_NC, BG>::BYTES;
-  auto kern = split_kernel<SPLIT_NC, COMBINE, WS, BG>;
+  auto kern = split_kernel<SPLIT_NC, COMBINE, WS, BG, GRAV>;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
@@ -275,6 +275,13 @@ int launch_split(smaug_ctx* c, const StageArgs& a) {
     if (a.combine == COMBINE_ACC && a.ws_mode == WS_VT) return launch_split_t<COMBINE_ACC, WS_VT, true>(c, a);
     if (a.combine == COMBINE_FINAL && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_FINAL, WS_FULL, true>(c, a);
     if (a.combine == COMBINE_BASE && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_BASE, WS_FULL, true>(c, a);
+    return fail(SMAUG_EINVAL, "split kernel: unsupported combine / wave-speed mode");
+  }
+  if (a.prm.grav_on) {       // gravity on a zero background
+    if (a.combine == COMBINE_BASE && a.ws_mode == WS_VT) return launch_split_t<COMBINE_BASE, WS_VT, false, true>(c, a);
+    if (a.combine == COMBINE_ACC && a.ws_mode == WS_VT) return launch_split_t<COMBINE_ACC, WS_VT, false, true>(c, a);
+    if (a.combine == COMBINE_FINAL && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_FINAL, WS_FULL, false, true>(c, a);
+    if (a.combine == COMBINE_BASE && a.ws_mode == WS_FULL) return launch_split_t<COMBINE_BASE, WS_FULL, false, true>(c, a);
     return fail(SMAUG_EINVAL, "split kernel: unsupported combine / wave-speed mode");
   }
   if (a.combine == COMBINE_BASE && a.ws_mode == WS_VT) return launch_split_t<COMBINE_BASE, WS_VT>(c, a);
@@ -322,8 +329,7 @@ int launch_flux(smaug_ctx* c, const StageArgs& a) {
 // runs in the tiled kernel.
 bool plain(const smaug_ctx* c) { return !c->has_bg && c->gx == 0.0 && c->gy == 0.0; }
 bool uses_flux(const smaug_ctx* c) { return plain(c) && !c->hd_on && c->kernel_mode != 0; }
-// (gravity without a background stays in the tiled kernel: the BG form of the split kernel reads background planes)
-bool uses_split(const smaug_ctx* c) { return (plain(c) || c->has_bg) && c->hd_on && c->kernel_mode == 2; }
+bool uses_split(const smaug_ctx* c) { return c->hd_on && c->kernel_mode == 2; }
 bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 1; }
 
 int launch_stage(smaug_ctx* c, const StageArgs& a) {

@@ -278,7 +278,7 @@ __device__ __forceinline__ void split_wavespeeds(const double (&o)[NF], double g
   }
 }
 
-template <int NC, int COMBINE, int WS, bool BG = false>
+template <int NC, int COMBINE, int WS, bool BG = false, bool GRAV = false>   // GRAV: gravity without a background
 #ifdef SMAUG_SPLIT_MAXNREG
 __global__ void __maxnreg__(SMAUG_SPLIT_MAXNREG) split_kernel
 #else
@@ -775,6 +775,12 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) s
             R[F_MY] = fma(rt, a.prm.gy, R[F_MY]);
             R[F_E] = fma(rt, fma(a.prm.gy, hvy[2], a.prm.gx * hvx[2]), R[F_E]);
           }
+        }
+        if constexpr (!BG && GRAV) {      // gravity on a zero background (c-10: rho~ is the total density)
+          const double rt = hr[2];
+          R[F_MX] = fma(rt, a.prm.gx, R[F_MX]);
+          R[F_MY] = fma(rt, a.prm.gy, R[F_MY]);
+          R[F_E] = fma(rt, fma(a.prm.gy, hvy[2], a.prm.gx * hvx[2]), R[F_E]);
         }
         const double* dx = DXR + s4 * 5 * NC + c;
         R[F_RHO] = fma(dx[C_RHO * NC], idx_, R[F_RHO]);
