@@ -404,3 +404,27 @@ def test_configs_3_4_5_full_step_count(gpu, oracle_mod, n, steps):
     b = cpu_run(oracle_mod, w, bc, gamma, steps, threads=16)
     err = check(*a, *b)
     print(f"config {n}^2 x {steps} steps: rel L2 per field = {err}, t = {a[1]}")
+
+
+def test_two_contexts_on_two_streams(gpu, oracle_mod):
+    """Two contexts stepping concurrently on two streams (a background run, whose kernel allocates tensor memory, next
+    to a zero-background run): same bits as the oracle for both -- no shared global state, TMEM allocation per CTA."""
+    import torch
+    w1, bc1, g1, bg1, (gx, gy) = si.stratified_atmosphere(300, 260)
+    w2, bc2, g2 = si.orszag_tang(280, 300)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s1):
+        a = gpu.Smaug(300, 260, g1, bc1, bg=torch.from_numpy(bg1), gx=gx, gy=gy)
+        a.set_state(torch.from_numpy(w1))
+    with torch.cuda.stream(s2):
+        b = gpu.Smaug(280, 300, g2, bc2)
+        b.set_state(torch.from_numpy(w2))
+    L = gpu.lib()
+    for _ in range(3):                       # interleaved asynchronous enqueues: both streams busy at once
+        assert L.smaug_step_async(a._h, 10, 0.3) == 0
+        assert L.smaug_step_async(b._h, 10, 0.3) == 0
+    oa, ob = a.get_state().cpu().numpy(), b.get_state().cpu().numpy()
+    a.close(); b.close()
+    ra = cpu_run(oracle_mod, w1, bc1, g1, 30, bg=bg1, gx=gx, gy=gy, threads=8)[0]
+    rb = cpu_run(oracle_mod, w2, bc2, g2, 30, threads=8)[0]
+    assert np.array_equal(oa, ra) and np.array_equal(ob, rb)
