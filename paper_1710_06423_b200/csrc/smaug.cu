@@ -296,11 +296,12 @@ int launch_split(smaug_ctx* c, const StageArgs& a) {
 #endif
 constexpr int FLUX_NT = SMAUG_FLUX_NT;
 
-// Streaming form without hyperdiffusion (smaug_flux_kernel.cuh): no background, HD off.
-int launch_flux(smaug_ctx* c, const StageArgs& a) {
+// Streaming form without hyperdiffusion (smaug_flux_kernel.cuh): HD off, with (BG) or without a background.
+template <bool BG>
+int launch_flux_t(smaug_ctx* c, const StageArgs& a) {
   static bool configured = false;
-  constexpr size_t smem = FluxSmem<FLUX_NT>::BYTES;
-  auto kern = flux_kernel<FLUX_NT>;
+  constexpr size_t smem = FluxSmem<FLUX_NT, BG>::BYTES;
+  auto kern = flux_kernel<FLUX_NT, BG>;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
@@ -308,7 +309,7 @@ int launch_flux(smaug_ctx* c, const StageArgs& a) {
   const int W = FLUX_NT - 4;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
-  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * FluxSmem<FLUX_NT>::CTAS_PER_SM, 4);
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * FluxSmem<FLUX_NT, BG>::CTAS_PER_SM, 4);
   const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
   dim3 grid(strips, nchunks);
   c->last_ctas = strips * nchunks;
@@ -325,10 +326,14 @@ int launch_flux(smaug_ctx* c, const StageArgs& a) {
   return SMAUG_OK;
 }
 
-// The streaming kernels cover the benchmark configurations (zero background, no gravity); everything else
-// runs in the tiled kernel.
+int launch_flux(smaug_ctx* c, const StageArgs& a) {
+  return c->has_bg ? launch_flux_t<true>(c, a) : launch_flux_t<false>(c, a);
+}
+
+// The streaming kernels cover everything except gravity on a zero background without hyperdiffusion, which
+// runs in the tiled kernel (as does everything when SMAUG_PARAM_KERNEL = 0).
 bool plain(const smaug_ctx* c) { return !c->has_bg && c->gx == 0.0 && c->gy == 0.0; }
-bool uses_flux(const smaug_ctx* c) { return plain(c) && !c->hd_on && c->kernel_mode != 0; }
+bool uses_flux(const smaug_ctx* c) { return (plain(c) || c->has_bg) && !c->hd_on && c->kernel_mode != 0; }
 bool uses_split(const smaug_ctx* c) { return c->hd_on && c->kernel_mode == 2; }
 bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 1; }
 
@@ -733,7 +738,7 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
   if (uses_flux(c)) {                                      // streaming kernel without HD: a strip of NT-4 columns
     out[0] = FLUX_NT - 4; out[1] = 1; out[2] = FLUX_NT;
-    out[3] = (int)FluxSmem<FLUX_NT>::BYTES;
+    out[3] = (int)(c->has_bg ? FluxSmem<FLUX_NT, true>::BYTES : FluxSmem<FLUX_NT>::BYTES);
   } else if (uses_split(c)) {   // role-split streaming kernel: a strip of NC-8 columns
     out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
     out[3] = (int)(c->has_bg ? SplitSmem<SPLIT_NC, true>::BYTES : SplitSmem<SPLIT_NC>::BYTES);

@@ -18,23 +18,29 @@
 
 namespace smaug {
 
-template <int NT>
+// BG = true: a background (with or without gravity): the four background planes ride in the landing ring, the
+// fluxes take their background terms (c-2), vx / vy of the head row go into a second ring for the x-derivatives of
+// the energy source S_e (their y-derivatives come from a five-row register history), gravity is three fmas (c-10).
+template <int NT, bool BG = false>
 struct FluxSmem {
   static constexpr int DEPTH = 4;                         // input rows in the landing ring
+  static constexpr int NIN = BG ? NF + NBG : NF;          // fields per landing row
   static constexpr int OFF_FXR = 0;                       // ring 4 rows x 5 planes: F_x
-  static constexpr int OFF_INR = OFF_FXR + 4 * 5 * NT;    // ring DEPTH rows x 6 fields: cp.async landing zone
-  static constexpr int OFF_RED = OFF_INR + DEPTH * NF * NT;
+  static constexpr int OFF_VXR = OFF_FXR + 4 * 5 * NT;    // BG: ring 4 rows x 2 planes: vx, vy
+  static constexpr int OFF_INR = OFF_VXR + (BG ? 4 * 2 * NT : 0);   // ring DEPTH rows x NIN fields: cp.async landing zone
+  static constexpr int OFF_RED = OFF_INR + DEPTH * NIN * NT;
   static constexpr int TOTAL = OFF_RED + 4 * 32;
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
-  static constexpr int CTAS_PER_SM = NT <= 128 ? 4 : 2;
+  static constexpr int CTAS_PER_SM = NT <= 128 ? (BG ? 3 : 4) : 2;
 };
 
-template <int NT>
-__global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(const StageArgs a, const MarchGeom mg) {
-  using S = FluxSmem<NT>;
-  constexpr int DEPTH = S::DEPTH;
+template <int NT, bool BG = false>
+__global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel(const StageArgs a, const MarchGeom mg) {
+  using S = FluxSmem<NT, BG>;
+  constexpr int DEPTH = S::DEPTH, NIN = S::NIN;
   extern __shared__ __align__(16) double smem[];
   double* const FXR = smem + S::OFF_FXR;
+  [[maybe_unused]] double* const VXR = smem + S::OFF_VXR;
   double* const INR = smem + S::OFF_INR;
   double* const red_sh = smem + S::OFF_RED;
   const Grid& g = a.g;
@@ -58,9 +64,13 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(con
   const int last_row = g.ny + NG - 1;
   int slot_f = 0;                                         // landing slot of the next row to fetch
   auto fetch_row = [&]() {
-    double* dst = INR + slot_f * NF * NT + tid;
+    double* dst = INR + slot_f * NIN * NT + tid;
 #pragma unroll
     for (int f = 0; f < NF; ++f) cp_async8(dst + f * NT, a.in.p[f] + gin);
+    if constexpr (BG) {
+#pragma unroll
+      for (int k = 0; k < NBG; ++k) cp_async8(dst + (NF + k) * NT, a.bg.p[k] + gin);
+    }
     cp_async_commit();
     if (fetched < last_row) gin += upitch;                // rows below the padded plane are never dereferenced
     ++fetched;
@@ -77,6 +87,7 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(con
 #pragma unroll
     for (int f = 0; f < 5; ++f) fy[k][f] = 0.0;
   double wsmax[4] = {0.0, 0.0, 0.0, 0.0};
+  [[maybe_unused]] double hvx[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, hvy[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // BG: rows r-4 .. r
 
 #pragma unroll 1
   for (int r = ystart - 2; r < yend + 2; ++r) {
@@ -97,36 +108,66 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(con
       }
     }
     cp_async_wait<DEPTH - 2>();                           // row r has landed (later rows may be in flight)
-    const double* src = INR + slot_r * NF * NT + tid;
-    const double rho = src[F_RHO * NT], mx = src[F_MX * NT], my = src[F_MY * NT];
+    const double* src = INR + slot_r * NIN * NT + tid;
+    const double rhot = src[F_RHO * NT], mx = src[F_MX * NT], my = src[F_MY * NT];
     const double et = src[F_E * NT], bx = src[F_BX * NT], by = src[F_BY * NT];
+    double rb = 0.0, eb = 0.0, Bbx = 0.0, Bby = 0.0;
+    if constexpr (BG) {
+      rb = src[(NF + BG_RHO) * NT]; eb = src[(NF + BG_E) * NT];
+      Bbx = src[(NF + BG_BX) * NT]; Bby = src[(NF + BG_BY) * NT];
+    }
     fetch_row();                                          // into the slot read one step ago
     slot_r = slot_r == DEPTH - 1 ? 0 : slot_r + 1;
 
     // ------------------------------------------------------------------ head: derived quantities, F_x, F_y of row r
+    const double rho = BG ? rb + rhot : rhot;
     const double rr = drcp(rho);
     const double vx = mx * rr, vy = my * rr;
     const double b2h = 0.5 * fma(by, by, bx * bx);
     const double ke = 0.5 * fma(my, vy, mx * vx);
-    const double eps = (et - ke) - b2h;
-    const double ptt = fma(gm1, eps, b2h);
     const double btv = fma(by, vy, bx * vx);
-    const double h = et + ptt;
     double* fxw = FXR + s4 * 5 * NT + tid;
-    fxw[C_RHO * NT] = rho * vx;
-    fxw[C_MX * NT] = fma(mx, vx, -(bx * bx)) + ptt;
-    fxw[C_MY * NT] = fma(my, vx, -(by * bx));
-    fxw[C_E * NT] = fma(vx, h, -(bx * btv));
-    fxw[C_B * NT] = fma(vx, by, -(bx * vy));
 #pragma unroll
     for (int k = 0; k < 4; ++k)
 #pragma unroll
       for (int f = 0; f < 5; ++f) fy[k][f] = fy[k + 1][f];
-    fy[4][C_RHO] = rho * vy;
-    fy[4][C_MX] = fma(mx, vy, -(bx * by));
-    fy[4][C_MY] = fma(my, vy, -(by * by)) + ptt;
-    fy[4][C_E] = fma(vy, h, -(by * btv));
-    fy[4][C_B] = fma(vy, bx, -(by * vx));
+    if constexpr (BG) {
+      const double cross = fma(Bby, by, Bbx * bx);
+      const double eps = ((et - ke) - cross) - b2h;
+      const double ptt = fma(gm1, eps, cross + b2h);
+      const double Bx = Bbx + bx, By = Bby + by;
+      const double Bbv = fma(Bby, vy, Bbx * vx);
+      const double h = (et + eb) + ptt;
+      fxw[C_RHO * NT] = rho * vx;
+      fxw[C_MX * NT] = ((fma(mx, vx, -(bx * bx)) - bx * Bbx) - Bbx * bx) + ptt;
+      fxw[C_MY * NT] = (fma(my, vx, -(by * bx)) - by * Bbx) - Bby * bx;
+      fxw[C_E * NT] = (fma(vx, h, -(bx * btv)) - bx * Bbv) - Bbx * btv;
+      fxw[C_B * NT] = fma(vx, By, -(Bx * vy));
+      fy[4][C_RHO] = rho * vy;
+      fy[4][C_MX] = (fma(mx, vy, -(bx * by)) - bx * Bby) - Bbx * by;
+      fy[4][C_MY] = ((fma(my, vy, -(by * by)) - by * Bby) - Bby * by) + ptt;
+      fy[4][C_E] = (fma(vy, h, -(by * btv)) - by * Bbv) - Bby * btv;
+      fy[4][C_B] = fma(vy, Bx, -(By * vx));
+      VXR[(s4 * 2 + 0) * NT + tid] = vx;
+      VXR[(s4 * 2 + 1) * NT + tid] = vy;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; }
+      hvx[4] = vx; hvy[4] = vy;
+    } else {
+      const double eps = (et - ke) - b2h;
+      const double ptt = fma(gm1, eps, b2h);
+      const double h = et + ptt;
+      fxw[C_RHO * NT] = rho * vx;
+      fxw[C_MX * NT] = fma(mx, vx, -(bx * bx)) + ptt;
+      fxw[C_MY * NT] = fma(my, vx, -(by * bx));
+      fxw[C_E * NT] = fma(vx, h, -(bx * btv));
+      fxw[C_B * NT] = fma(vx, by, -(bx * vy));
+      fy[4][C_RHO] = rho * vy;
+      fy[4][C_MX] = fma(mx, vy, -(bx * by));
+      fy[4][C_MY] = fma(my, vy, -(by * by)) + ptt;
+      fy[4][C_E] = fma(vy, h, -(by * btv));
+      fy[4][C_B] = fma(vy, bx, -(by * vx));
+    }
     __syncthreads();
 
     // ------------------------------------------------------------------ tail: R(j), combine, write
@@ -147,6 +188,28 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(con
       R[F_E] = fma(cdx[C_E], idx_, cdy[C_E] * idy_) * (-1.0 / 12.0);
       R[F_BX] = (cdy[C_B] * idy_) * (-1.0 / 12.0);        // F_x(bx) == 0
       R[F_BY] = fma(cdx[C_B], idx_, 0.0) * (-1.0 / 12.0); // F_y(by) == 0
+      [[maybe_unused]] double jrb = 0.0, jeb = 0.0, jBbx = 0.0, jBby = 0.0;
+      if constexpr (BG) {
+        // energy source S_e (c-2) and gravity (c-10) at the tail cell (row j = r - 2: histories index 2)
+        jrb = a.bg.p[BG_RHO][gj]; jeb = a.bg.p[BG_E][gj]; jBbx = a.bg.p[BG_BX][gj]; jBby = a.bg.p[BG_BY][gj];
+        const double* vxr = VXR + (sj * 2 + 0) * NT + tl;
+        const double* vyr = VXR + (sj * 2 + 1) * NT + tl;
+        const double dxvx = (cd12v(vxr[-2], vxr[-1], vxr[1], vxr[2]) * idx_) * (1.0 / 12.0);
+        const double dxvy = (cd12v(vyr[-2], vyr[-1], vyr[1], vyr[2]) * idx_) * (1.0 / 12.0);
+        const double dyvx = (cd12v(hvx[0], hvx[1], hvx[3], hvx[4]) * idy_) * (1.0 / 12.0);
+        const double dyvy = (cd12v(hvy[0], hvy[1], hvy[3], hvy[4]) * idy_) * (1.0 / 12.0);
+        const double bb2h = 0.5 * fma(jBby, jBby, jBbx * jBbx);
+        const double ptb = fma(gm1, jeb - bb2h, bb2h);
+        const double S = fma(-ptb, dxvx + dyvy,
+                             fma(jBby * jBby, dyvy, fma(jBbx * jBby, dxvy + dyvx, (jBbx * jBbx) * dxvx)));
+        R[F_E] = R[F_E] + S;
+        if (a.prm.grav_on) {
+          const double rt = a.in.p[F_RHO][gj];             // rho~ of the tail cell
+          R[F_MX] = fma(rt, a.prm.gx, R[F_MX]);
+          R[F_MY] = fma(rt, a.prm.gy, R[F_MY]);
+          R[F_E] = fma(rt, fma(a.prm.gy, hvy[2], a.prm.gx * hvx[2]), R[F_E]);
+        }
+      }
       double o[NF];
       if (combine == COMBINE_FINAL) {
 #pragma unroll
@@ -164,7 +227,11 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT>::CTAS_PER_SM) flux_kernel(con
         }
         if (ws_mode != WS_NONE) {
           double w4[4];
-          cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, ws_mode == WS_FULL, w4);
+          if constexpr (BG)
+            cell_wavespeeds(jrb + o[F_RHO], o[F_MX], o[F_MY], jeb + o[F_E], jBbx + o[F_BX], jBby + o[F_BY], gamma,
+                            ws_mode == WS_FULL, w4);
+          else
+            cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, ws_mode == WS_FULL, w4);
 #pragma unroll
           for (int k = 0; k < 4; ++k) wsmax[k] = dmax(wsmax[k], w4[k]);
         }

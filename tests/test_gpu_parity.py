@@ -428,3 +428,25 @@ def test_two_contexts_on_two_streams(gpu, oracle_mod):
     ra = cpu_run(oracle_mod, w1, bc1, g1, 30, bg=bg1, gx=gx, gy=gy, threads=8)[0]
     rb = cpu_run(oracle_mod, w2, bc2, g2, 30, threads=8)[0]
     assert np.array_equal(oa, ra) and np.array_equal(ob, rb)
+
+
+def test_background_without_hyperdiffusion_streaming_kernel(gpu, oracle_mod):
+    """The BG form of flux_kernel (hyperdiffusion off, background + gravity) over several strips and chunks against
+    the oracle on every cell, and bit-equal to the tiled kernel."""
+    import torch
+    w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(700, 520)
+    s = gpu.Smaug(700, 520, gamma, bc, bg=torch.from_numpy(bg), gx=gx, gy=gy, hd_on=0)
+    assert s.kernel_name().startswith("flux_kernel")
+    s.close()
+    a = gpu_run(gpu, w, bc, gamma, 12, bg=bg, gx=gx, gy=gy, hd_on=0)
+    t = gpu_run(gpu, w, bc, gamma, 12, bg=bg, gx=gx, gy=gy, hd_on=0, kernel=0)
+    b = cpu_run(oracle_mod, w, bc, gamma, 12, bg=bg, gx=gx, gy=gy, hd_on=0, threads=16)
+    check(*a, *b)
+    assert np.array_equal(a[0], t[0]) and a[1] == t[1]
+    # uniform background, periodic, RK2
+    W, bcp, gamma = si.orszag_tang(300, 280)
+    bgu = si.uniform_background(300, 280, 0.1, 0.2, 0.05, 0.03)
+    W[0] -= 0.1; W[3] -= 0.2; W[4] -= 0.05; W[5] -= 0.03
+    a = gpu_run(gpu, W, bcp, gamma, 10, bg=bgu, hd_on=0, rk_order=2)
+    b = cpu_run(oracle_mod, W, bcp, gamma, 10, bg=bgu, hd_on=0, rk_order=2, threads=16)
+    check(*a, *b)
