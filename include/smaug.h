@@ -125,8 +125,7 @@ int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
 /* Name of the fused stage kernel the context's current parameters select (static string, never NULL;
  * "?" for a NULL context): "split_kernel<128>" (role-split streaming form), "march_kernel<256>"
  * (single-role streaming form), "flux_kernel<128>" (streaming form without hyperdiffusion) or
- * "stage_kernel<32,8,512>" (tiled form: gravity on a zero background without hyperdiffusion, or forced by
- * SMAUG_PARAM_KERNEL = 0). */
+ * "stage_kernel<32,8,512>" (tiled form: forced by SMAUG_PARAM_KERNEL = 0). */
 const char* smaug_get_kernel_name(smaug_ctx* ctx);
 
 /* Device time, in milliseconds, spent in the fused stage kernels (summed over launches) and the number of

@@ -297,11 +297,11 @@ int launch_split(smaug_ctx* c, const StageArgs& a) {
 constexpr int FLUX_NT = SMAUG_FLUX_NT;
 
 // Streaming form without hyperdiffusion (smaug_flux_kernel.cuh): HD off, with (BG) or without a background.
-template <bool BG>
+template <bool BG, bool GRAV = false>
 int launch_flux_t(smaug_ctx* c, const StageArgs& a) {
   static bool configured = false;
   constexpr size_t smem = FluxSmem<FLUX_NT, BG>::BYTES;
-  auto kern = flux_kernel<FLUX_NT, BG>;
+  auto kern = flux_kernel<FLUX_NT, BG, GRAV>;
   if (!configured) {
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
@@ -327,13 +327,14 @@ int launch_flux_t(smaug_ctx* c, const StageArgs& a) {
 }
 
 int launch_flux(smaug_ctx* c, const StageArgs& a) {
-  return c->has_bg ? launch_flux_t<true>(c, a) : launch_flux_t<false>(c, a);
+  if (c->has_bg) return launch_flux_t<true>(c, a);
+  return a.prm.grav_on ? launch_flux_t<false, true>(c, a) : launch_flux_t<false>(c, a);
 }
 
-// The streaming kernels cover everything except gravity on a zero background without hyperdiffusion, which
-// runs in the tiled kernel (as does everything when SMAUG_PARAM_KERNEL = 0).
+// The streaming kernels cover every configuration; the tiled kernel runs when SMAUG_PARAM_KERNEL = 0 (tests), and
+// hyperdiffusion-on cases when SMAUG_PARAM_KERNEL = 1 excludes the split kernel and march_kernel does not apply.
 bool plain(const smaug_ctx* c) { return !c->has_bg && c->gx == 0.0 && c->gy == 0.0; }
-bool uses_flux(const smaug_ctx* c) { return (plain(c) || c->has_bg) && !c->hd_on && c->kernel_mode != 0; }
+bool uses_flux(const smaug_ctx* c) { return !c->hd_on && c->kernel_mode != 0; }
 bool uses_split(const smaug_ctx* c) { return c->hd_on && c->kernel_mode == 2; }
 bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 1; }
 

@@ -34,7 +34,7 @@ struct FluxSmem {
   static constexpr int CTAS_PER_SM = NT <= 128 ? (BG ? 3 : 4) : 2;
 };
 
-template <int NT, bool BG = false>
+template <int NT, bool BG = false, bool GRAV = false>      // GRAV: gravity on a zero background
 __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel(const StageArgs a, const MarchGeom mg) {
   using S = FluxSmem<NT, BG>;
   constexpr int DEPTH = S::DEPTH, NIN = S::NIN;
@@ -167,6 +167,11 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
       fy[4][C_MY] = fma(my, vy, -(by * by)) + ptt;
       fy[4][C_E] = fma(vy, h, -(by * btv));
       fy[4][C_B] = fma(vy, bx, -(by * vx));
+      if constexpr (GRAV) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { hvx[k] = hvx[k + 1]; hvy[k] = hvy[k + 1]; }
+        hvx[4] = vx; hvy[4] = vy;
+      }
     }
     __syncthreads();
 
@@ -188,6 +193,12 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
       R[F_E] = fma(cdx[C_E], idx_, cdy[C_E] * idy_) * (-1.0 / 12.0);
       R[F_BX] = (cdy[C_B] * idy_) * (-1.0 / 12.0);        // F_x(bx) == 0
       R[F_BY] = fma(cdx[C_B], idx_, 0.0) * (-1.0 / 12.0); // F_y(by) == 0
+      if constexpr (!BG && GRAV) {     // gravity on a zero background (c-10: rho~ is the total density)
+        const double rt = a.in.p[F_RHO][gj];
+        R[F_MX] = fma(rt, a.prm.gx, R[F_MX]);
+        R[F_MY] = fma(rt, a.prm.gy, R[F_MY]);
+        R[F_E] = fma(rt, fma(a.prm.gy, hvy[2], a.prm.gx * hvx[2]), R[F_E]);
+      }
       [[maybe_unused]] double jrb = 0.0, jeb = 0.0, jBbx = 0.0, jBby = 0.0;
       if constexpr (BG) {
         // energy source S_e (c-2) and gravity (c-10) at the tail cell (row j = r - 2: histories index 2)

@@ -450,3 +450,15 @@ def test_background_without_hyperdiffusion_streaming_kernel(gpu, oracle_mod):
     a = gpu_run(gpu, W, bcp, gamma, 10, bg=bgu, hd_on=0, rk_order=2)
     b = cpu_run(oracle_mod, W, bcp, gamma, 10, bg=bgu, hd_on=0, rk_order=2, threads=16)
     check(*a, *b)
+
+
+def test_gravity_on_zero_background_without_hyperdiffusion(gpu, oracle_mod):
+    """flux_kernel's GRAV form: the hydrostatic column of the printed equations (zero background, HD off), several
+    strips; against the oracle and the tiled kernel."""
+    w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(300, 200, split=False, pulse=2e-2)
+    assert bg is None
+    a = gpu_run(gpu, w, bc, gamma, 15, gx=0.3, gy=gy, hd_on=0)
+    t = gpu_run(gpu, w, bc, gamma, 15, gx=0.3, gy=gy, hd_on=0, kernel=0)
+    b = cpu_run(oracle_mod, w, bc, gamma, 15, gx=0.3, gy=gy, hd_on=0)
+    check(*a, *b)
+    assert np.array_equal(a[0], t[0])
