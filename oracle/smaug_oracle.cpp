@@ -17,6 +17,12 @@
 //   rk4_step               P6 (temporal order 4), P4 (RK4 amplification factor), P12 (restart)
 //   gravity (c-10)         G1 (hydrostatic background stays exactly static), G2 (free fall: closed form),
 //                          G3 (hydrostatic balance of PAPER.md:35 to 4th order), G4 (split == unsplit, 4th order)
+// Round-2 pins (tests/test_oracle_pins_r2.py; each fails on the seeded mistake named in its docstring):
+//   hd_mixed_fluxes, energy   M1 (uniform drift U: viscous R_e contains U * closed-form mixed R_mx; x<->y mirror),
+//                             M2 (uniform B0: ohmic R_e contains B0 * closed-form mixed R_bx; mirror)
+//   fill_ghosts during steps  F1 (fixed ghost strips incl. corners bitwise frozen while a pulse runs into them; the
+//                             interior differs from the open run), F2 (frozen values == np.pad 'edge' of the set_state data)
+//   flux / rhs (non-linear)   R1 (rhs of a flowing magnetised state == PAPER.md:35 differentiated analytically, order 4)
 // "Parity unpinned" against the SAC/SMAUG codes themselves: the paper prints no field values and its
 // figures are not in the container.
 //
