@@ -38,10 +38,10 @@ WORKLOADS = {
     "orszag_tang_1000": (1000, 1000, "ot"),
     "brio_wu_800": (800, 1, "bw"),
     # SURVEY 8(f) NEXT-2 (not a BASELINE config): stratified magnetised atmosphere with a pulse, non-uniform
-    # background + gravity, periodic in x, open in y -- runs in the tiled kernel
+    # background + gravity, periodic in x, open in y -- split_kernel<128, .., BG>
     "stratified_4000": (4000, 4000, "strat"),
     # SURVEY 8(d) extra row: the 8000^2 Orszag-Tang state as a perturbation on a uniform non-zero background
-    # (exercises the background loads and the energy source) -- tiled kernel
+    # (exercises the background loads and the energy source) -- split_kernel<128, .., BG>
     "orszag_tang_8000_bg": (8000, 8000, "otbg"),
 }
 # Algorithmic HBM bytes per cell-update of the fused step as built: per stage the
@@ -49,11 +49,9 @@ WORKLOADS = {
 # accumulator; stage 4 reads it:  96 + 192 + 144 + 144 = 576 B (SURVEY 8(d) counts 624 for its variant).
 BYTES_PER_CELL_UPDATE = 576.0
 STAGES_PER_STEP = 4
-# Second ceiling, reported beside the HBM roofline: fp64-pipe thread-instructions the
-# split kernel executes per output cell and stage (DFMA + DADD + DMUL + DSETP, static SASS count of the two
-# role loops: 398 per column pair in the X loop + 552 per two rows in the Y loop, times 128/120 for the strip
-# halo), against 64 fp64 lanes per SM and clock.
-FP64_INSTR_PER_CELL_STAGE = (398 / 2 + 552 / 2) * 128 / 120
+# Second ceiling, reported beside the HBM roofline: fp64-pipe thread-instructions the stage
+# kernel executes per cell and launch (DFMA + DADD + DMUL + DSETP), taken from the committed ncu capture
+# (sm__inst_executed_pipe_fp64.sum x 32 / cells; profiles/stage_kernel_ncu.json), against 64 fp64 lanes per SM and clock.
 FP64_LANES_PER_SM = 64
 N_SM = 148
 METRIC = "fp64 MHD cell-updates/s"
@@ -74,9 +72,11 @@ def make_state(name):
     return w, bc, gamma, None, (0.0, 0.0)
 
 
-def bytes_per_cell_update(has_bg):
-    """Algorithmic HBM bytes per cell-update: 576 (see above) + the four background planes read once per stage."""
-    return BYTES_PER_CELL_UPDATE + (STAGES_PER_STEP * 4 * 8 if has_bg else 0)
+def bytes_per_cell_update(has_bg, rk_order=4):
+    """Algorithmic HBM bytes per cell-update: RK4 576 (see above); RK2 (midpoint) 96 + 144 = 240 (stage 2 reads w1 with
+    its halo and w^n pointwise, writes w^{n+1}); Euler 96; + the four background planes read once per stage."""
+    stages = {4: 4, 2: 2, 1: 1}[rk_order]
+    return {4: BYTES_PER_CELL_UPDATE, 2: 240.0, 1: 96.0}[rk_order] + (stages * 4 * 8 if has_bg else 0)
 
 
 def peaks():
@@ -89,15 +89,18 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def ncu_traffic(name):
-    """DRAM bytes per stage-kernel launch from the committed ncu capture, if one exists for this workload."""
-    p = os.path.join(ROOT, "profiles", "stage_kernel_traffic.json")
+def ncu_capture(key):
+    """Per-launch counters of the stage kernel from the committed `ncu --set full` capture of this workload key
+    (profiles/stage_kernel_ncu.json, written from the capture named there), or {}: `dram_bytes` = dram__bytes_read.sum +
+    dram__bytes_write.sum, `fp64_thread_inst_per_cell` = 32 x sm__inst_executed_pipe_fp64.sum / cells (mean of the RK
+    stages).  These are constants of a committed capture, not measurements of this run: `capture` says which."""
+    p = os.path.join(ROOT, "profiles", "stage_kernel_ncu.json")
     if os.path.exists(p):
         try:
-            return json.load(open(p)).get(name)
+            return json.load(open(p)).get(key) or {}
         except Exception:  # noqa: BLE001
-            return None
-    return None
+            return {}
+    return {}
 
 
 class ClockSampler:
@@ -230,7 +233,8 @@ def run_ours(args):
     bg_dev = None if bg_np is None else torch.from_numpy(bg_np).to(dev)
     has_bg = bg_np is not None
     del w_np, bg_np
-    sim = pkg.Smaug(nx, ny, gamma, bc, bg=bg_dev, device=dev, hd_on=0 if args.no_hd else 1, gx=gx, gy=gy)
+    sim = pkg.Smaug(nx, ny, gamma, bc, bg=bg_dev, device=dev, hd_on=0 if args.no_hd else 1, gx=gx, gy=gy,
+                    rk_order=args.rk_order)
     del bg_dev
     sim.set_state(w_host)
 
@@ -271,8 +275,11 @@ def run_ours(args):
         e2e = replica_value(cells, K, world, e2e_ms)
         peak, peak_src = peaks()
         info = sim.kernel_info()
-        bpcu = bytes_per_cell_update(has_bg)
-        per_launch_bytes = bpcu / STAGES_PER_STEP * cells
+        stages = {4: 4, 2: 2, 1: 1}[args.rk_order]
+        bpcu = bytes_per_cell_update(has_bg, args.rk_order)
+        per_launch_bytes = bpcu / stages * cells
+        cap = ncu_capture(name + ("_nohd" if args.no_hd else "") + ("_rk%d" % args.rk_order if args.rk_order != 4 else ""))
+        fp64_per_cell = cap.get("fp64_thread_inst_per_cell")
         avg_launch_ms = stage_ms / max(stage_n, 1)
         achieved = per_launch_bytes / (avg_launch_ms * 1e-3) / 1e9 if stage_n else None
         state_bytes = 6 * 8 * cells
@@ -280,23 +287,25 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": 4,
+            "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": args.rk_order,
                        "background": ("stratified, g = (%g, %g)" % (gx, gy) if gy or gx else "uniform") if has_bg else "zero", "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "working set >> L2, no flush needed" if cells * 48 > 4e8 else
                              "working set comparable to L2 (126 MB): DRAM traffic is below algorithmic"},
             "hbm_gbs_algorithmic": value / world * bpcu / 1e9,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": (achieved / peak) if achieved else None, "traffic": ncu_traffic(name),
+                         "frac": (achieved / peak) if achieved else None, "traffic": cap.get("dram_bytes"),
+                         "traffic_source": cap.get("capture"),
                          "peak_source": peak_src, "kernel": f"smaug::{sim.kernel_name()} (fused RK stage)",
                          "bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_launch_ms,
                          "launches_timed": stage_n, "stage_kernel_share_of_step": stage_ms / ms,
                          "note": None if stage_n else "--no-kernel-timing: steps replayed as CUDA graphs, no per-kernel events",
                          "launch": info},
-            "fp64_pipe": ({"achieved": FP64_INSTR_PER_CELL_STAGE * cells / (avg_launch_ms * 1e-3) / 1e12,
+            "fp64_pipe": ({"achieved": fp64_per_cell * cells / (avg_launch_ms * 1e-3) / 1e12,
                            "peak": N_SM * FP64_LANES_PER_SM * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12,
-                           "unit": "T fp64-instr/s", "instr_per_cell_stage": FP64_INSTR_PER_CELL_STAGE,
-                           "note": "secondary ceiling; only meaningful for split_kernel<128>"}
-                          if stage_n and not args.no_hd and not has_bg else None),
+                           "unit": "T fp64-instr/s", "instr_per_cell_stage": fp64_per_cell,
+                           "note": "secondary ceiling: fp64-pipe thread-instructions per cell and launch from the "
+                                   "committed ncu capture (sm__inst_executed_pipe_fp64), x cells / measured duration"}
+                          if stage_n and fp64_per_cell else None),
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
                     "d2h_bytes_per_step": state_bytes / K,
                     "note": "smaug_set_state(host) + smaug_step(K) + smaug_get_state(host), pinned host memory"},
@@ -332,6 +341,8 @@ def main():
     ap.add_argument("--no-kernel-timing", action="store_true",
                     help="no CUDA events around the stage kernels (roofline = null); smaug_step then replays CUDA "
                          "graphs of whole steps, which is what a user gets -- matters on launch-bound small grids")
+    ap.add_argument("--rk-order", type=int, default=4, choices=[4, 2],
+                    help="4: classical RK4 (PAPER.md:45, the default); 2: midpoint rule (SURVEY 8(f) NEXT-4 extra row)")
     ap.add_argument("--no-hd", action="store_true",
                     help="hyperdiffusion off (the 'Without HD' column of the paper's Table 1); extra row, not the default")
     args = ap.parse_args()

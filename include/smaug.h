@@ -18,8 +18,10 @@
  *   - Arrays are fp64, SoA, field-major, row-major with x fastest, INTERIOR CELLS ONLY:
  *       state      w  [6][ny][nx]  order rho~, mx, my, e~, bx~, by~
  *       background bg [4][ny][nx]  order rho_b, e_b, Bbx, Bby          (NULL = zero background)
- *     Pointers may be HOST or DEVICE memory (detected with cudaPointerGetAttributes); the caller owns
- *     them and the library copies; nothing is retained after the call returns.
+ *     Pointers may be HOST or DEVICE memory (unified addressing: the copies are cudaMemcpyDefault); the
+ *     caller owns them and the library copies; nothing is retained after the call returns.
+ *   - Device: a context lives on the device of its workspace (smaug_create: the device current at the call);
+ *     every entry point makes that device current for the duration of the call and restores the caller's.
  *   - Grid: cell centres x_i = (i+1/2) Lx/nx, y_j = (j+1/2) Ly/ny; Lx = Ly = 1 by default.  Ghost width 3.
  *   - Return value: 0 = SMAUG_OK, negative = error; smaug_last_error() gives a thread-local message.
  *     No exception crosses the ABI.  No global state except that message.
@@ -133,6 +135,16 @@ const char* smaug_get_kernel_name(smaug_ctx* ctx);
  * smaug_set_kernel_timing(ctx, 1).  Reading synchronises the stream.  */
 int smaug_set_kernel_timing(smaug_ctx* ctx, int on);
 int smaug_get_kernel_timing(smaug_ctx* ctx, double* stage_ms, long long* stage_launches);
+
+/* Exactness self-test of the library's branch-free fp64 division helpers ("Division"): on
+ * about `draws` seeded operand sets with binary exponents uniform in [exp_lo, exp_hi] (values below 2^-1022 are
+ * denormals), counts the results that differ in any bit from the compiler's IEEE-754 `/`:
+ *   out[0] ddiv(a, b) vs a / b,   out[1] drcp(b) vs 1 / b,   out[2] ratio_div(m3, m1) vs m3 / m1 and
+ *   out[3] kappa_ratio(m3, m1, cv) vs (m1 > 0 ? cv * (m3 / m1) : 0) on ratio-like operands 0 <= m3 <= 4 m1 (incl.
+ *   m1 = 0),   out[4] = draws actually made per test.
+ * The stage kernels call ddiv / drcp on ordinary numbers only and route every hyperviscosity ratio through
+ * kappa_ratio (or its fast path, taken only when every M1 of the warp is >= 2^-923).  Runs on the current device. */
+int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, long long draws, unsigned long long out[5]);
 
 void smaug_destroy(smaug_ctx* ctx); /* NULL is a no-op */
 

@@ -46,12 +46,17 @@ def lib() -> C.CDLL:
     """Load libsmaug.so (never builds implicitly on a box without nvcc: fails loudly instead)."""
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        if os.environ.get("SMAUG_LIB"):
+            pass                            # an explicitly chosen variant build is loaded as it is
+        elif os.path.exists(nvcc):
             try:
-                build()
+                build()                     # no-op unless the library is missing or older than csrc/ or smaug.h
             except Exception as e:  # noqa: BLE001
-                raise RuntimeError(f"libsmaug.so is missing and could not be built ({e}); "
+                raise RuntimeError(f"libsmaug.so is missing or stale and could not be built ({e}); "
                                    "there is no CPU fallback") from e
+        elif not os.path.exists(LIB_PATH):
+            raise RuntimeError("libsmaug.so is missing and there is no nvcc to build it; there is no CPU fallback")
         L = C.CDLL(LIB_PATH)
         dp, vp = C.POINTER(C.c_double), C.c_void_p
         L.smaug_last_error.restype = C.c_char_p
@@ -74,6 +79,8 @@ def lib() -> C.CDLL:
         L.smaug_get_kernel_name.restype = C.c_char_p
         L.smaug_set_kernel_timing.argtypes = [vp, C.c_int]
         L.smaug_get_kernel_timing.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
+        L.smaug_selftest_division.argtypes = [C.c_int, C.c_int, C.c_ulonglong, C.c_longlong,
+                                              C.POINTER(C.c_ulonglong)]
         L.smaug_destroy.argtypes = [vp]
         L.smaug_destroy.restype = None
         _lib = L
@@ -100,6 +107,13 @@ def _ptr(x):
         return C.c_void_p(x.data_ptr())
     assert x.flags["C_CONTIGUOUS"] and x.dtype.name == "float64"
     return C.c_void_p(x.ctypes.data)
+
+
+def selftest_division(exp_lo: int, exp_hi: int, seed: int = 1, draws: int = 1 << 26) -> dict:
+    """smaug_selftest_division: mismatch counts of the division helpers against `/` on the current device."""
+    o = (C.c_ulonglong * 5)()
+    _check(lib().smaug_selftest_division(int(exp_lo), int(exp_hi), int(seed), int(draws), o))
+    return dict(ddiv=o[0], drcp=o[1], ratio_div=o[2], kappa_ratio=o[3], draws=o[4])
 
 
 class Smaug:

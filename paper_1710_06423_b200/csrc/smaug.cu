@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "smaug_flux_kernel.cuh"
+#include "smaug_selftest.cuh"
 
 using namespace smaug;
 
@@ -45,6 +46,30 @@ int fail(int code, const std::string& msg) {
 constexpr int TW = SMAUG_TW, TH = SMAUG_TH, NT = SMAUG_NT;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Makes the context's device current for the duration of an ABI call and restores the caller's afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE attribute of a kernel: set it once per
+// (kernel instantiation, device).  `mask` is the instantiation's own static bit set of configured devices.
+template <typename K>
+cudaError_t configure_smem(K kern, size_t smem, int device, unsigned long long& mask) {
+  if (device >= 0 && device < 64 && (mask >> device & 1ULL)) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess && device >= 0 && device < 64) mask |= 1ULL << device;
+  return e;
+}
 
 struct Layout {
   int pitch;
@@ -101,6 +126,7 @@ struct smaug_ctx {
   int kernel_mode = 2;      // SMAUG_PARAM_KERNEL: 2 role-split streaming kernel, 1 single-role streaming kernel
                             // (both only without background and with hyperdiffusion), 0 always the tile kernel
   int n_sm = 148;
+  int device = 0;           // the device the workspace lives on; every ABI entry makes it current (DeviceGuard)
   // CUDA-graph replay of whole time steps (launch-bound small grids; SMAUG_PARAM_GRAPH).  One step is 9 launches
   // whose arguments are fixed except for the reduction-set parity (state_set 0 <-> 4), so three executables cover
   // every call: a step from set 0, a step from set 4, and the pair starting at set 0.  They are captured on a
@@ -146,7 +172,7 @@ int launch_ghost(smaug_ctx* c, const Planes6& pl, int nplanes, int freeze) {
 
 int launch_wavespeeds(smaug_ctx* c, const Planes6& w, int set) {
   const long long n = (long long)c->g.nx * c->g.ny;
-  const int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 8);
+  const int blocks = (int)std::min<long long>((n + 255) / 256, (long long)c->n_sm * 8);
   unsigned long long* slots = c->sc->red[set];
   if (c->has_bg)
     wavespeed_kernel<true><<<blocks, 256, 0, c->stream>>>(c->g, cview(w), c->bg, c->gamma, slots);
@@ -159,13 +185,10 @@ int launch_wavespeeds(smaug_ctx* c, const Planes6& w, int set) {
 
 template <bool BG, bool HD>
 int launch_stage_t(smaug_ctx* c, const StageArgs& a) {
-  static bool configured = false;
+  static unsigned long long configured = 0;     // devices on which this instantiation has its smem limit raised
   constexpr size_t smem = Tile<TW, TH, BG>::BYTES;
   auto kern = stage_kernel<TW, TH, NT, BG, HD>;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
-  }
+  CU(configure_smem(kern, smem, c->device, configured));
   dim3 grid((c->g.nx + TW - 1) / TW, (c->g.ny + TH - 1) / TH);
   c->last_ctas = (int)(grid.x * grid.y);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -188,16 +211,13 @@ constexpr int MARCH_NT = SMAUG_MARCH_NT;
 
 // Streaming form (smaug_march_kernel.cuh): no background, hyperdiffusion on.
 int launch_march(smaug_ctx* c, const StageArgs& a) {
-  static bool configured = false;
+  static unsigned long long configured = 0;     // devices on which this instantiation has its smem limit raised
   constexpr size_t smem = MarchSmem<MARCH_NT>::BYTES;
   auto kern = march_kernel<MARCH_NT>;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
-  }
+  CU(configure_smem(kern, smem, c->device, configured));
   const int W = MARCH_NT - 2 * NG;
   const int strips = (c->g.nx + W - 1) / W;
-  const int target = 148 * 8;
+  const int target = c->n_sm * 8;
   int nchunks = std::max(1, (target + strips - 1) / strips);
   MarchGeom mg;
   mg.rows_per_cta = std::max(32, (c->g.ny + nchunks - 1) / nchunks);
@@ -240,13 +260,10 @@ int pick_rows_per_cta(int ny, int strips, int n_sm, int warm_rows = 2 * NG) {
 
 template <int COMBINE, int WS, bool BG = false, bool GRAV = false>
 int launch_split_t(smaug_ctx* c, const StageArgs& a) {
-  static bool configured = false;
+  static unsigned long long configured = 0;     // devices on which this instantiation has its smem limit raised
   constexpr size_t smem = SplitSmem<SPLIT_NC, BG>::BYTES;
   auto kern = split_kernel<SPLIT_NC, COMBINE, WS, BG, GRAV>;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
-  }
+  CU(configure_smem(kern, smem, c->device, configured));
   const int W = SPLIT_NC - 8;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
@@ -299,13 +316,10 @@ constexpr int FLUX_NT = SMAUG_FLUX_NT;
 // Streaming form without hyperdiffusion (smaug_flux_kernel.cuh): HD off, with (BG) or without a background.
 template <bool BG, bool GRAV = false>
 int launch_flux_t(smaug_ctx* c, const StageArgs& a) {
-  static bool configured = false;
+  static unsigned long long configured = 0;     // devices on which this instantiation has its smem limit raised
   constexpr size_t smem = FluxSmem<FLUX_NT, BG>::BYTES;
   auto kern = flux_kernel<FLUX_NT, BG, GRAV>;
-  if (!configured) {
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
-  }
+  CU(configure_smem(kern, smem, c->device, configured));
   const int W = FLUX_NT - 4;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
@@ -544,10 +558,22 @@ int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], con
   }
   smaug_ctx* c = new (std::nothrow) smaug_ctx();
   if (!c) return fail(SMAUG_ENOMEM, "host allocation failed");
+  // the context lives on the device of the caller's workspace, else on the current device; it is recorded and
+  // made current by every later call (the caller's current device is restored on return)
   {
-    int dev = 0, n_sm = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); dev = 0; }
+    if (workspace) {
+      cudaPointerAttributes at;
+      if (cudaPointerGetAttributes(&at, workspace) == cudaSuccess && at.type == cudaMemoryTypeDevice) dev = at.device;
+      else cudaGetLastError();
+    }
+    c->device = dev;
+  }
+  DeviceGuard guard_(c->device);
+  {
+    int n_sm = 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && n_sm > 0)
       c->n_sm = n_sm;
   }
   c->has_bg = bg != nullptr;
@@ -598,6 +624,7 @@ int smaug_create(int nx, int ny, double gamma, const int bc[4], const double* bg
 
 void smaug_destroy(smaug_ctx* c) {
   if (!c) return;
+  DeviceGuard guard_(c->device);
   cudaStreamSynchronize(c->stream);
   invalidate_graphs(c);
   if (c->gstream) {
@@ -614,6 +641,7 @@ void smaug_destroy(smaug_ctx* c) {
 
 int smaug_set_stream(smaug_ctx* c, void* stream) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   CU(cudaStreamSynchronize(c->stream));
   c->stream = (cudaStream_t)stream;
   invalidate_graphs(c);
@@ -622,6 +650,7 @@ int smaug_set_stream(smaug_ctx* c, void* stream) {
 
 int smaug_set_param(smaug_ctx* c, int key, double v) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   invalidate_graphs(c);      // parameters are baked into captured kernel arguments
   switch (key) {
     case SMAUG_PARAM_LX: if (!(v > 0)) break; c->Lx = v; return SMAUG_OK;
@@ -644,6 +673,7 @@ int smaug_set_param(smaug_ctx* c, int key, double v) {
 
 int smaug_set_state(smaug_ctx* c, const double* w) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   if (!w) return fail(SMAUG_EINVAL, "w is NULL");
   int rc = copy_in(c, w, c->buf[0].p, NF);
   if (rc) return rc;
@@ -663,6 +693,7 @@ int smaug_set_state(smaug_ctx* c, const double* w) {
 
 int smaug_step_async(smaug_ctx* c, int n_steps, double cfl) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   if (n_steps < 0) return fail(SMAUG_EINVAL, "n_steps must be >= 0");
   if (!(c->fixed_dt > 0.0) && !(cfl > 0.0)) return fail(SMAUG_EINVAL, "cfl must be > 0");
   // Whole steps as CUDA-graph replays: worth it when launches are a visible share of the step (small grids);
@@ -700,6 +731,7 @@ int smaug_step(smaug_ctx* c, int n_steps, double cfl) {
 
 int smaug_get_state(smaug_ctx* c, double* w) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   if (!w) return fail(SMAUG_EINVAL, "w is NULL");
   const Grid& g = c->g;
   for (int f = 0; f < NF; ++f)
@@ -711,6 +743,7 @@ int smaug_get_state(smaug_ctx* c, double* w) {
 
 int smaug_get_time(smaug_ctx* c, double* t, double* last_dt) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   int rc = sync_and_status(c);
   double v[2];
   CU(cudaMemcpy(v, &c->sc->dt, 2 * sizeof(double), cudaMemcpyDeviceToHost));
@@ -721,6 +754,7 @@ int smaug_get_time(smaug_ctx* c, double* t, double* last_dt) {
 
 int smaug_get_wavespeeds(smaug_ctx* c, double out[4]) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
   int rc = sync_and_status(c);
   CU(cudaMemcpy(out, c->sc->red[c->state_set], 4 * sizeof(double), cudaMemcpyDeviceToHost));
@@ -729,6 +763,7 @@ int smaug_get_wavespeeds(smaug_ctx* c, double out[4]) {
 
 int smaug_get_launch_count(smaug_ctx* c, long long* n) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   if (!n) return fail(SMAUG_EINVAL, "n is NULL");
   *n = c->launches;
   return SMAUG_OK;
@@ -736,6 +771,7 @@ int smaug_get_launch_count(smaug_ctx* c, long long* n) {
 
 int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
   if (uses_flux(c)) {                                      // streaming kernel without HD: a strip of NT-4 columns
     out[0] = FLUX_NT - 4; out[1] = 1; out[2] = FLUX_NT;
@@ -764,6 +800,7 @@ const char* smaug_get_kernel_name(smaug_ctx* c) {
 
 int smaug_set_kernel_timing(smaug_ctx* c, int on) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   CU(cudaStreamSynchronize(c->stream));
   c->timing = on != 0;
   c->ev_used = 0;
@@ -778,10 +815,34 @@ int smaug_set_kernel_timing(smaug_ctx* c, int on) {
 
 int smaug_get_kernel_timing(smaug_ctx* c, double* stage_ms, long long* stage_launches) {
   if (int rc = check_ctx(c)) return rc;
+  DeviceGuard guard_(c->device);
   CU(cudaStreamSynchronize(c->stream));
   if (int rc = collect_timing(c)) return rc;
   if (stage_ms) *stage_ms = c->stage_ms;
   if (stage_launches) *stage_launches = c->stage_launches;
+  return SMAUG_OK;
+}
+
+int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, long long draws, unsigned long long out[5]) {
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  if (exp_lo > exp_hi || exp_lo < -1074 || exp_hi > 1000 || draws < 1) return fail(SMAUG_EINVAL, "bad exponent range or draw count");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(SMAUG_ECUDA, "no CUDA device: libsmaug has no CPU fallback");
+  }
+  const int blocks = 1184, threads = 256;
+  const int per_thread = (int)std::min<long long>(std::max<long long>(1, draws / ((long long)blocks * threads)), 1 << 20);
+  unsigned long long* d = nullptr;
+  CU(cudaMalloc((void**)&d, 5 * sizeof(unsigned long long)));
+  cudaError_t e = cudaMemset(d, 0, 5 * sizeof(unsigned long long));
+  if (e == cudaSuccess) {
+    division_selftest_kernel<<<blocks, threads>>>(exp_lo, exp_hi, seed, per_thread, d);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpy(out, d, 5 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(SMAUG_ECUDA, std::string("division self-test: ") + cudaGetErrorString(e));
   return SMAUG_OK;
 }
 

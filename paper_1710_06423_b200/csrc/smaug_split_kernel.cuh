@@ -146,6 +146,29 @@ __device__ __forceinline__ double kappa_q(double m3, double m1, double cv, int& 
 }
 constexpr int ORDINARY_HI = 0x06400000;     // high word of 2^-923: below it ratio_div rescales
 
+#ifndef SMAUG_KAPPA_FAST
+#define SMAUG_KAPPA_FAST 0      // 1: the guarded kappa of a family is the plain exact division, redone with the zero
+#endif                          //    guard and the 2^200 rescue only when a warp vote finds an M1 below 2^-923 (same
+                                //    bits: the rescue scales by 1.0 above that); the redo is a few lines, not a section
+// kappa of N ratios of one family (N = 2: the two interfaces of a column pair; N = 1: one y-interface)
+template <int N>
+__device__ __forceinline__ void kappa_family(const double (&m3)[N], const double (&m1)[N], double cv, double (&k)[N]) {
+#if SMAUG_KAPPA_FAST
+  int lo = __double2hiint(m1[0]);
+#pragma unroll
+  for (int q = 1; q < N; ++q) lo = min(lo, __double2hiint(m1[q]));
+#pragma unroll
+  for (int q = 0; q < N; ++q) k[q] = cv * ddiv(m3[q], m1[q]);
+  if (__any_sync(0xffffffffu, lo < ORDINARY_HI)) {
+#pragma unroll
+    for (int q = 0; q < N; ++q) k[q] = kappa_ratio(m3[q], m1[q], cv);
+  }
+#else
+#pragma unroll
+  for (int q = 0; q < N; ++q) k[q] = kappa_ratio(m3[q], m1[q], cv);
+#endif
+}
+
 // kappa at the TWO adjacent interfaces (u[2] | u[3]) and (u[3] | u[4]) of the seven cells u[0..6] (c-5).
 // d0, d1: the first differences across the two interfaces.
 template <bool GUARD>
@@ -160,8 +183,15 @@ __device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0,
   const double am = amax(amax(a[1], a[2]), amax(a[3], a[4]));
   const double m3_0 = dabs(amax(t[0], tm)), m3_1 = dabs(amax(tm, t[3]));
   const double m1_0 = dabs(amax(a[0], am)), m1_1 = dabs(amax(am, a[5]));
-  k0 = kappa_q<GUARD>(m3_0, m1_0, cv, lo);
-  k1 = kappa_q<GUARD>(m3_1, m1_1, cv, lo);
+  if (GUARD) {
+    const double m3[2] = {m3_0, m3_1}, m1[2] = {m1_0, m1_1};
+    double k[2];
+    kappa_family<2>(m3, m1, cv, k);
+    k0 = k[0]; k1 = k[1];
+  } else {
+    k0 = kappa_q<GUARD>(m3_0, m1_0, cv, lo);
+    k1 = kappa_q<GUARD>(m3_1, m1_1, cv, lo);
+  }
   d0 = a[2];
   d1 = a[3];
 }
@@ -177,6 +207,12 @@ __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, doubl
   const double m3 = dabs(amax(amax(t0, t1), t2));
   const double m1 = dabs(amax(amax(amax(a0, a1), amax(a2, a3)), a4));
   d1_mid = a2;
+  if (GUARD) {
+    const double m3a[1] = {m3}, m1a[1] = {m1};
+    double k[1];
+    kappa_family<1>(m3a, m1a, cv, k);
+    return k[0];
+  }
   return kappa_q<GUARD>(m3, m1, cv, lo);
 }
 
