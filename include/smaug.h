@@ -39,7 +39,8 @@
 extern "C" {
 #endif
 
-typedef struct smaug_ctx smaug_ctx; /* opaque, library-owned */
+typedef struct smaug_ctx smaug_ctx;     /* opaque, library-owned */
+typedef struct smaug_group smaug_group; /* opaque: a px x py decomposition of one grid into contexts (see below) */
 
 enum { SMAUG_BC_PERIODIC = 0, SMAUG_BC_OPEN = 1, SMAUG_BC_FIXED = 2 };
 
@@ -147,6 +148,38 @@ int smaug_get_kernel_timing(smaug_ctx* ctx, double* stage_ms, long long* stage_l
 int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, long long draws, unsigned long long out[5]);
 
 void smaug_destroy(smaug_ctx* ctx); /* NULL is a no-op */
+
+/* ---- Domain decomposition (SURVEY.md 8(f) NEXT-1; PAPER.md:25 Fig. 1, :55-59 "the full domain is divided into
+ * sub-regions", :61-73 exchange_halo) ----------------------------------------------------------------------------
+ * A group splits the nx-by-ny grid into px x py near-equal blocks (block column a covers global columns
+ * [a nx / px, (a+1) nx / px), rows likewise), one context per block, member b * px + a on device devices[b * px + a]
+ * (devices == NULL: all on the current device; distinct devices need peer access to each other).  The paper's
+ * exchange_halo (gather -> D2H -> MPI_Isend/Irecv -> H2D -> scatter per field) becomes one small kernel per member and
+ * RK stage that PULLS the member's ghost cells (width 3, 6 fields, corners included) straight out of the owning
+ * neighbours' planes (peer pointers: same-device pointers on one GPU, NVLink P2P mappings across GPUs); the global
+ * boundary kinds `bc` (periodic / open / fixed, as in smaug_create) are applied on the global grid.  The four
+ * wave-speed maxima (c-4) are reduced by every member's stage kernels into the leader's slots with atomicMax, so dt
+ * and v_t are global (the paper's implied MAX all-reduce).  Members step in lockstep: per stage, all exchanges run
+ * after all members' previous stage (events between the members' streams), then all stage kernels.
+ * Contract: a decomposed run is BIT-IDENTICAL to the single-context run of the same global problem.
+ * State / background arrays are the GLOBAL ones, [6][ny][nx] / [4][ny][nx], host or device; the group scatters and
+ * gathers the blocks.  All group calls synchronise before returning.  Errors as for the context calls. */
+int smaug_group_create(int px, int py, int nx, int ny, double gamma, const int bc[4], const double* bg,
+                       const int* devices, smaug_group** out);
+int smaug_group_size(smaug_group* grp, int* px, int* py);
+int smaug_group_set_param(smaug_group* grp, int key, double value);   /* forwarded to every member; LX, LY are global */
+int smaug_group_set_state(smaug_group* grp, const double* w);
+int smaug_group_step(smaug_group* grp, int n_steps, double cfl);
+int smaug_group_get_state(smaug_group* grp, double* w);
+int smaug_group_get_time(smaug_group* grp, double* t, double* last_dt);
+int smaug_group_get_wavespeeds(smaug_group* grp, double out[4]);
+/* kernels launched so far: stage / dt / reduction kernels of all members, and exchange (halo) kernels */
+int smaug_group_get_launch_count(smaug_group* grp, long long* stage_and_aux, long long* exchange);
+void smaug_group_destroy(smaug_group* grp); /* destroys the members too; NULL is a no-op */
+/* Host-only view of the decomposition logic (needs no GPU; used by the CPU tests): for ghost cell (i, j) -- local
+ * indices outside [0, nx_m) x [0, ny_m) -- of member `member`, out = { x0, y0, nx_m, ny_m of the member,  source member
+ * (-1: the cell is never rewritten: fixed global side, freeze == 0),  source local i,  source local j }. */
+int smaug_group_map_cell(int px, int py, int nx, int ny, const int bc[4], int member, int i, int j, int freeze, int out[7]);
 
 const char* smaug_last_error(void);
 

@@ -83,6 +83,19 @@ def lib() -> C.CDLL:
                                               C.POINTER(C.c_ulonglong)]
         L.smaug_destroy.argtypes = [vp]
         L.smaug_destroy.restype = None
+        ip = C.POINTER(C.c_int)
+        L.smaug_group_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, ip, vp, ip, C.POINTER(vp)]
+        L.smaug_group_size.argtypes = [vp, ip, ip]
+        L.smaug_group_set_param.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug_group_set_state.argtypes = [vp, vp]
+        L.smaug_group_step.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug_group_get_state.argtypes = [vp, vp]
+        L.smaug_group_get_time.argtypes = [vp, dp, dp]
+        L.smaug_group_get_wavespeeds.argtypes = [vp, dp]
+        L.smaug_group_get_launch_count.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.smaug_group_destroy.argtypes = [vp]
+        L.smaug_group_destroy.restype = None
+        L.smaug_group_map_cell.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, ip, C.c_int, C.c_int, C.c_int, C.c_int, ip]
         _lib = L
     return _lib
 
@@ -203,6 +216,76 @@ class Smaug:
             lib().smaug_destroy(self._h)
             self._h = None
             self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # noqa: BLE001
+            pass
+
+
+def group_map_cell(px, py, nx, ny, bc, member, i, j, freeze=0):
+    """smaug_group_map_cell (host only): ((x0, y0, nx_m, ny_m), (source member or -1, si, sj))."""
+    o = (C.c_int * 7)()
+    _check(lib().smaug_group_map_cell(px, py, nx, ny, (C.c_int * 4)(*[int(b) for b in bc]), member, i, j, int(freeze), o))
+    return (o[0], o[1], o[2], o[3]), (o[4], o[5], o[6])
+
+
+class SmaugGroup:
+    """A px x py decomposition of one nx-by-ny problem into contexts that exchange halos through peer pointers and share
+    one wave-speed reduction (smaug_group_* in include/smaug.h).  Arrays are the GLOBAL state / background."""
+
+    def __init__(self, px, py, nx, ny, gamma, bc, bg=None, devices=None, **params):
+        L = lib()
+        self.px, self.py, self.nx, self.ny = int(px), int(py), int(nx), int(ny)
+        h = C.c_void_p()
+        bc_arr = (C.c_int * 4)(*[int(b) for b in bc])
+        dev_arr = None if devices is None else (C.c_int * (self.px * self.py))(*[int(d) for d in devices])
+        if bg is not None:
+            assert tuple(bg.shape) == (4, ny, nx)
+        _check(L.smaug_group_create(self.px, self.py, self.nx, self.ny, float(gamma), bc_arr, _ptr(bg), dev_arr, C.byref(h)))
+        self._h = h
+        for k, v in params.items():
+            self.set_param(k, v)
+
+    def set_param(self, key, value):
+        k = PARAMS[key] if isinstance(key, str) else int(key)
+        _check(lib().smaug_group_set_param(self._h, k, float(value)))
+
+    def set_state(self, w):
+        assert tuple(w.shape) == (6, self.ny, self.nx)
+        _check(lib().smaug_group_set_state(self._h, _ptr(w)))
+
+    def step(self, n_steps, cfl=0.3):
+        _check(lib().smaug_group_step(self._h, int(n_steps), float(cfl)))
+
+    def get_state(self, out=None):
+        import torch
+        if out is None:
+            out = torch.empty((6, self.ny, self.nx), dtype=torch.float64, device="cuda")
+        assert tuple(out.shape) == (6, self.ny, self.nx)
+        _check(lib().smaug_group_get_state(self._h, _ptr(out)))
+        return out
+
+    def time(self):
+        t, dt = C.c_double(), C.c_double()
+        _check(lib().smaug_group_get_time(self._h, C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def wavespeeds(self):
+        o = (C.c_double * 4)()
+        _check(lib().smaug_group_get_wavespeeds(self._h, o))
+        return list(o)
+
+    def launch_count(self):
+        a, b = C.c_longlong(), C.c_longlong()
+        _check(lib().smaug_group_get_launch_count(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().smaug_group_destroy(self._h)
+            self._h = None
 
     def __del__(self):
         try:

@@ -14,6 +14,7 @@
 
 #include "smaug_flux_kernel.cuh"
 #include "smaug_selftest.cuh"
+#include "smaug_group.cuh"
 
 using namespace smaug;
 
@@ -127,6 +128,12 @@ struct smaug_ctx {
                             // (both only without background and with hyperdiffusion), 0 always the tile kernel
   int n_sm = 148;
   int device = 0;           // the device the workspace lives on; every ABI entry makes it current (DeviceGuard)
+  // member of a decomposition group (smaug_group_*): the GLOBAL cell counts fix Delta and the n = 1 rule of c-7, the
+  // reduction slots / dt / t / status are the group leader's, the ghost fill is the group's exchange kernel
+  smaug_group* group = nullptr;
+  int geo_nx = 0, geo_ny = 0;     // global interior size (= g.nx, g.ny outside a group)
+  DeviceScalars* own_sc = nullptr;
+  double* bg_owned = nullptr;     // background block allocated by the group (freed in smaug_destroy)
   // CUDA-graph replay of whole time steps (launch-bound small grids; SMAUG_PARAM_GRAPH).  One step is 9 launches
   // whose arguments are fixed except for the reduction-set parity (state_set 0 <-> 4), so three executables cover
   // every call: a step from set 0, a step from set 4, and the pair starting at set 0.  They are captured on a
@@ -141,6 +148,21 @@ struct smaug_ctx {
   int launches_per_step = 0;
 };
 
+// A px x py decomposition of one global grid into member contexts.  The group owns its members.
+struct smaug_group {
+  int px = 1, py = 1, NX = 0, NY = 0;
+  int gbc[4] = {0, 0, 0, 0};
+  bool has_bg = false;
+  std::vector<smaug_ctx*> m;            // member b * px + a
+  std::vector<int> x0, y0;              // px + 1 / py + 1 prefix offsets
+  std::vector<GroupTable*> table;       // device copy of the table on every member's device
+  std::vector<cudaEvent_t> ev;          // one per member, for the inter-stream barrier
+  bool one_stream = false;              // every member on the same device and stream: no events needed
+  int state_set = 0;
+  long long exchange_launches = 0;
+  bool pending_status = false;
+};
+
 namespace {
 
 CPlanes6 cview(const Planes6& p) {
@@ -152,8 +174,8 @@ CPlanes6 cview(const Planes6& p) {
 Params make_params(const smaug_ctx* c) {
   Params p;
   p.gamma = c->gamma;
-  p.inv_dx = c->g.nx / c->Lx;
-  p.inv_dy = c->g.ny / c->Ly;
+  p.inv_dx = c->geo_nx / c->Lx;
+  p.inv_dy = c->geo_ny / c->Ly;
   p.c_rho = c->c_rho; p.c_mom = c->c_mom; p.c_e = c->c_e; p.c_b = c->c_b;
   p.hd_on = c->hd_on;
   p.gx = c->gx; p.gy = c->gy;
@@ -360,11 +382,9 @@ int launch_stage(smaug_ctx* c, const StageArgs& a) {
   return c->hd_on ? launch_stage_t<false, true>(c, a) : launch_stage_t<false, false>(c, a);
 }
 
-// One stage: ghost fill of the input buffer, then the fused kernel.
-int run_stage(smaug_ctx* c, int in, int base, int acc_in, int out, int acc_out, double coef, int combine,
-              int red_in, int red_out, int ws_mode) {
-  int rc = launch_ghost(c, c->buf[in], NF, 0);
-  if (rc) return rc;
+// The fused kernel of one stage (the ghosts of buffer `in` must be filled).
+int run_stage_kernel(smaug_ctx* c, int in, int base, int acc_in, int out, int acc_out, double coef, int combine,
+                     int red_in, int red_out, int ws_mode) {
   StageArgs a;
   a.g = c->g;
   a.prm = make_params(c);
@@ -383,29 +403,49 @@ int run_stage(smaug_ctx* c, int in, int base, int acc_in, int out, int acc_out, 
   return launch_stage(c, a);
 }
 
+// One stage: ghost fill of the input buffer, then the fused kernel.
+int run_stage(smaug_ctx* c, int in, int base, int acc_in, int out, int acc_out, double coef, int combine,
+              int red_in, int red_out, int ws_mode) {
+  int rc = launch_ghost(c, c->buf[in], NF, 0);
+  if (rc) return rc;
+  return run_stage_kernel(c, in, base, acc_in, out, acc_out, coef, combine, red_in, red_out, ws_mode);
+}
+
+// The stages of one time step as a table (c-6), shared by the single-context path and the group path.
+struct StageSpec { int in, base, acc_in, out, acc_out; double coef; int combine, red_in, red_out, ws; };
+int stage_table(const smaug_ctx* c, int A, int B, StageSpec st[4]) {
+  const int vt_mode = c->hd_on ? WS_VT : WS_NONE;
+  if (c->rk_order == 4) {
+    st[0] = {0, 0, 3, 1, 3, 0.5, COMBINE_BASE, A, 1, vt_mode};            // w1 = wn + dt/2 R(wn)
+    st[1] = {1, 0, 3, 2, 3, 0.5, COMBINE_ACC, 1, 2, vt_mode};             // w2; acc = (w1 - wn) + 2 w2
+    st[2] = {2, 0, 3, 1, 3, 1.0, COMBINE_BASE, 2, 3, vt_mode};            // w3 = wn + dt R(w2)
+    st[3] = {1, 0, 3, 0, 3, 1.0 / 6.0, COMBINE_FINAL, 3, B, WS_FULL};     // w^{n+1}
+    return 4;
+  }
+  if (c->rk_order == 2) {
+    st[0] = {0, 0, 3, 1, 3, 0.5, COMBINE_BASE, A, 1, vt_mode};
+    // in-place on buf[0] is safe: base is read and out written by the same thread at the same cell only
+    st[1] = {1, 0, 3, 0, 3, 1.0, COMBINE_BASE, 1, B, WS_FULL};
+    return 2;
+  }
+  st[0] = {0, 0, 3, 1, 3, 1.0, COMBINE_BASE, A, B, WS_FULL};             // Euler: the caller swaps buf[0], buf[1]
+  return 1;
+}
+
 // One full time step (c-6, c-7).  The state lives in buf[0] before and after.
 int enqueue_step(smaug_ctx* c, double cfl) {
   const int A = c->state_set, B = A == 0 ? 4 : 0;
-  const int vt_mode = c->hd_on ? WS_VT : WS_NONE;
   dt_kernel<<<1, 32, 0, c->stream>>>(c->sc, A, (1u << 1) | (1u << 2) | (1u << 3) | (1u << B), cfl,
-                                     c->fixed_dt, c->Lx / c->g.nx, c->Ly / c->g.ny, c->g.nx, c->g.ny);
+                                     c->fixed_dt, c->Lx / c->geo_nx, c->Ly / c->geo_ny, c->geo_nx, c->geo_ny);
   c->launches++;
   CU(cudaGetLastError());
+  StageSpec st[4];
+  const int ns = stage_table(c, A, B, st);
   int rc = SMAUG_OK;
-  if (c->rk_order == 4) {
-    //            in base acc_in out acc_out  c     combine        red_in red_out ws
-    rc = run_stage(c, 0, 0, 3, 1, 3, 0.5, COMBINE_BASE, A, 1, vt_mode);            // w1 = wn + dt/2 R(wn)
-    if (!rc) rc = run_stage(c, 1, 0, 3, 2, 3, 0.5, COMBINE_ACC, 1, 2, vt_mode);    // w2; acc = (w1+2w2-wn)/3
-    if (!rc) rc = run_stage(c, 2, 0, 3, 1, 3, 1.0, COMBINE_BASE, 2, 3, vt_mode);   // w3 = wn + dt R(w2)
-    if (!rc) rc = run_stage(c, 1, 0, 3, 0, 3, 1.0 / 6.0, COMBINE_FINAL, 3, B, WS_FULL);  // w^{n+1}
-  } else if (c->rk_order == 2) {
-    rc = run_stage(c, 0, 0, 3, 1, 3, 0.5, COMBINE_BASE, A, 1, vt_mode);
-    // in-place on buf[0] is safe: base is read and out written by the same thread at the same cell only
-    if (!rc) rc = run_stage(c, 1, 0, 3, 0, 3, 1.0, COMBINE_BASE, 1, B, WS_FULL);
-  } else {
-    rc = run_stage(c, 0, 0, 3, 1, 3, 1.0, COMBINE_BASE, A, B, WS_FULL);
-    if (!rc) std::swap(c->buf[0], c->buf[1]);
-  }
+  for (int k = 0; k < ns && !rc; ++k)
+    rc = run_stage(c, st[k].in, st[k].base, st[k].acc_in, st[k].out, st[k].acc_out, st[k].coef, st[k].combine,
+                   st[k].red_in, st[k].red_out, st[k].ws);
+  if (!rc && c->rk_order == 1) std::swap(c->buf[0], c->buf[1]);
   c->state_set = B;
   return rc;
 }
@@ -580,6 +620,7 @@ int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], con
   c->L = make_layout(nx, ny, c->has_bg);
   c->g.nx = nx; c->g.ny = ny; c->g.pitch = c->L.pitch; c->g.plane = c->L.plane;
   for (int s = 0; s < 4; ++s) c->g.bc[s] = bc[s];
+  c->geo_nx = nx; c->geo_ny = ny;
   c->gamma = gamma;
   c->stream = (cudaStream_t)stream;
   if (workspace) {
@@ -600,6 +641,7 @@ int smaug_create_in_workspace(int nx, int ny, double gamma, const int bc[4], con
   if (cudaMemsetAsync(c->base, 0, c->L.total, c->stream) != cudaSuccess)
     return cleanup(fail(SMAUG_ECUDA, "cudaMemsetAsync failed"));
   c->sc = (DeviceScalars*)(c->base + c->L.scalars_off);
+  c->own_sc = c->sc;
   const size_t plane_bytes = c->L.state_bytes / NF;
   for (int b = 0; b < 4; ++b)
     for (int f = 0; f < NF; ++f) c->buf[b].p[f] = (double*)(c->base + c->L.bufs_off[b] + f * plane_bytes);
@@ -634,6 +676,7 @@ void smaug_destroy(smaug_ctx* c) {
     cudaEventDestroy(c->gev_out);
   }
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->bg_owned) cudaFree(c->bg_owned);
   if (c->owns && c->base) cudaFree(c->base);
   cudaGetLastError();
   delete c;
@@ -695,6 +738,7 @@ int smaug_step_async(smaug_ctx* c, int n_steps, double cfl) {
   if (int rc = check_ctx(c)) return rc;
   DeviceGuard guard_(c->device);
   if (n_steps < 0) return fail(SMAUG_EINVAL, "n_steps must be >= 0");
+  if (c->group) return fail(SMAUG_EINVAL, "this context is a member of a group: step it with smaug_group_step");
   if (!(c->fixed_dt > 0.0) && !(cfl > 0.0)) return fail(SMAUG_EINVAL, "cfl must be > 0");
   // Whole steps as CUDA-graph replays: worth it when launches are a visible share of the step (small grids);
   // harmless otherwise.  Not while per-kernel timing events are wanted, and not for Euler (its buffers swap).
@@ -843,6 +887,389 @@ int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, lon
   if (e == cudaSuccess) e = cudaMemcpy(out, d, 5 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
   cudaFree(d);
   if (e != cudaSuccess) return fail(SMAUG_ECUDA, std::string("division self-test: ") + cudaGetErrorString(e));
+  return SMAUG_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// Decomposition group.  Host side: member creation, the exchange launches,
+// the inter-stream barrier, the lockstep stage loop.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+
+// near-equal blocks ("equal sub-regions"): block column a covers global columns [a nx / px, (a+1) nx / px)
+GroupGeom group_geom(int px, int py, int nx, int ny, const int bc[4]) {
+  GroupGeom G;
+  std::memset(&G, 0, sizeof(G));
+  G.px = px; G.py = py; G.NX = nx; G.NY = ny;
+  for (int s = 0; s < 4; ++s) G.gbc[s] = bc[s];
+  for (int a = 0; a <= px; ++a) G.x0[a] = (int)((long long)a * nx / px);
+  for (int b = 0; b <= py; ++b) G.y0[b] = (int)((long long)b * ny / py);
+  return G;
+}
+
+int group_check(smaug_group* g) {
+  if (!g) return fail(SMAUG_EINVAL, "NULL group");
+  return SMAUG_OK;
+}
+
+// Every member's stream waits for everything enqueued so far on every other member's stream.
+int group_barrier(smaug_group* g) {
+  if (g->one_stream) return SMAUG_OK;
+  const int n = (int)g->m.size();
+  for (int k = 0; k < n; ++k) {
+    DeviceGuard dg(g->m[k]->device);
+    CU(cudaEventRecord(g->ev[k], g->m[k]->stream));
+  }
+  for (int k = 0; k < n; ++k) {
+    DeviceGuard dg(g->m[k]->device);
+    for (int o = 0; o < n; ++o)
+      if (o != k) CU(cudaStreamWaitEvent(g->m[k]->stream, g->ev[o], 0));
+  }
+  return SMAUG_OK;
+}
+
+int group_sync(smaug_group* g) {
+  for (smaug_ctx* c : g->m) {
+    DeviceGuard dg(c->device);
+    CU(cudaStreamSynchronize(c->stream));
+  }
+  return SMAUG_OK;
+}
+
+// exchange fill of buffer `buf` (0..3, 4 = background) of every member; the members' interiors must be complete
+int group_exchange(smaug_group* g, int buf, int nplanes, int freeze) {
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    smaug_ctx* c = g->m[k];
+    DeviceGuard dg(c->device);
+    const long long total = 2LL * NG * (c->g.nx + 2 * NG) + 2LL * NG * c->g.ny;
+    const int blocks = (int)std::min<long long>((total + 255) / 256, 1024);
+    group_ghost_fill_kernel<<<dim3(blocks, nplanes), 256, 0, c->stream>>>(g->table[k], (int)k, buf, freeze);
+    c->launches++;
+    g->exchange_launches++;
+    CU(cudaGetLastError());
+  }
+  return SMAUG_OK;
+}
+
+int group_upload_tables(smaug_group* g) {
+  GroupTable T;
+  std::memset(&T, 0, sizeof(T));
+  T.geo = group_geom(g->px, g->py, g->NX, g->NY, g->gbc);
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    const smaug_ctx* c = g->m[k];
+    T.pitch[k] = c->g.pitch;
+    for (int b = 0; b < 4; ++b)
+      for (int f = 0; f < NF; ++f) T.planes[k][b][f] = c->buf[b].p[f];
+    for (int f = 0; f < NF; ++f) T.planes[k][4][f] = f < NBG ? const_cast<double*>(c->bg.p[f]) : nullptr;
+  }
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    DeviceGuard dg(g->m[k]->device);
+    CU(cudaMemcpy(g->table[k], &T, sizeof(T), cudaMemcpyHostToDevice));
+  }
+  return SMAUG_OK;
+}
+
+// one time step of the whole group: leader's dt, then per stage { exchange ; stage kernels } with barriers between
+int group_enqueue_step(smaug_group* g, double cfl) {
+  smaug_ctx* L = g->m[0];
+  const int A = g->state_set, B = A == 0 ? 4 : 0;
+  int rc = group_barrier(g);                      // every member's last stage has reduced into set A
+  if (rc) return rc;
+  {
+    DeviceGuard dg(L->device);
+    dt_kernel<<<1, 32, 0, L->stream>>>(L->sc, A, (1u << 1) | (1u << 2) | (1u << 3) | (1u << B), cfl, L->fixed_dt,
+                                       L->Lx / g->NX, L->Ly / g->NY, g->NX, g->NY);
+    L->launches++;
+    CU(cudaGetLastError());
+  }
+  StageSpec st[4];
+  const int ns = stage_table(L, A, B, st);
+  for (int k = 0; k < ns; ++k) {
+    if ((rc = group_barrier(g))) return rc;       // dt / the previous stage of EVERY member is complete
+    if ((rc = group_exchange(g, st[k].in, NF, 0))) return rc;
+    for (smaug_ctx* c : g->m) {
+      DeviceGuard dg(c->device);
+      if ((rc = run_stage_kernel(c, st[k].in, st[k].base, st[k].acc_in, st[k].out, st[k].acc_out, st[k].coef,
+                                 st[k].combine, st[k].red_in, st[k].red_out, st[k].ws)))
+        return rc;
+    }
+  }
+  if (L->rk_order == 1) {                         // Euler: buffers swap -> the tables' plane pointers follow
+    for (smaug_ctx* c : g->m) std::swap(c->buf[0], c->buf[1]);
+    if ((rc = group_sync(g))) return rc;
+    if ((rc = group_upload_tables(g))) return rc;
+  }
+  g->state_set = B;
+  return SMAUG_OK;
+}
+
+int group_status(smaug_group* g) {
+  int rc = group_sync(g);
+  if (rc) return rc;
+  if (g->pending_status) {
+    smaug_ctx* L = g->m[0];
+    DeviceGuard dg(L->device);
+    int status = 0;
+    CU(cudaMemcpy(&status, &L->sc->status, sizeof(int), cudaMemcpyDeviceToHost));
+    g->pending_status = false;
+    if (status) return fail(SMAUG_ENONFINITE, "a time step was non-finite or <= 0");
+  }
+  return SMAUG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void smaug_group_destroy(smaug_group* g) {
+  if (!g) return;
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    if (!g->m[k]) continue;
+    DeviceGuard dg(g->m[k]->device);
+    cudaStream_t st = g->m[k]->stream;
+    cudaStreamSynchronize(st);
+    if (k < g->table.size() && g->table[k]) cudaFree(g->table[k]);
+    if (k < g->ev.size() && g->ev[k]) cudaEventDestroy(g->ev[k]);
+    g->m[k]->group = nullptr;
+    smaug_destroy(g->m[k]);
+    if (st) cudaStreamDestroy(st);
+  }
+  cudaGetLastError();
+  delete g;
+}
+
+int smaug_group_create(int px, int py, int nx, int ny, double gamma, const int bc[4], const double* bg,
+                       const int* devices, smaug_group** out) {
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!bc) return fail(SMAUG_EINVAL, "bc is NULL");
+  if (px < 1 || py < 1 || px > GROUP_MAX_SIDE || py > GROUP_MAX_SIDE) return fail(SMAUG_EINVAL, "px, py must be in 1..8");
+  if (nx < px || ny < py) return fail(SMAUG_EINVAL, "every sub-domain needs at least one cell along each axis");
+  for (int s = 0; s < 4; ++s)
+    if (bc[s] < 0 || bc[s] > 2) return fail(SMAUG_EINVAL, "unknown boundary kind");
+  for (int ax = 0; ax < 2; ++ax)
+    if ((bc[2 * ax] == SMAUG_BC_PERIODIC) != (bc[2 * ax + 1] == SMAUG_BC_PERIODIC))
+      return fail(SMAUG_EINVAL, "periodic must be set on both sides of an axis");
+  if (!(gamma > 1.0)) return fail(SMAUG_EINVAL, "gamma must be > 1");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(SMAUG_ECUDA, "no CUDA device: libsmaug has no CPU fallback");
+  }
+  const int n = px * py;
+  int cur = 0;
+  if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); cur = 0; }
+  std::vector<int> dev(n, cur);
+  if (devices)
+    for (int k = 0; k < n; ++k) {
+      if (devices[k] < 0 || devices[k] >= ndev) return fail(SMAUG_EINVAL, "device index out of range");
+      dev[k] = devices[k];
+    }
+  // the members read each other's planes and the leader's reduction slots: peer access between every device pair
+  for (int k = 0; k < n; ++k)
+    for (int o = 0; o < n; ++o) {
+      if (dev[k] == dev[o]) continue;
+      int can = 0;
+      if (cudaDeviceCanAccessPeer(&can, dev[k], dev[o]) != cudaSuccess || !can) {
+        cudaGetLastError();
+        return fail(SMAUG_ECUDA, "the devices of a group need peer access to each other (NVLink / P2P)");
+      }
+      DeviceGuard dg(dev[k]);
+      const cudaError_t e = cudaDeviceEnablePeerAccess(dev[o], 0);
+      if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled)
+        return fail(SMAUG_ECUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
+      cudaGetLastError();
+    }
+  smaug_group* g = new (std::nothrow) smaug_group();
+  if (!g) return fail(SMAUG_ENOMEM, "host allocation failed");
+  g->px = px; g->py = py; g->NX = nx; g->NY = ny; g->has_bg = bg != nullptr;
+  for (int s = 0; s < 4; ++s) g->gbc[s] = bc[s];
+  g->x0.resize(px + 1); g->y0.resize(py + 1);
+  {
+    const GroupGeom G = group_geom(px, py, nx, ny, bc);
+    for (int a = 0; a <= px; ++a) g->x0[a] = G.x0[a];
+    for (int b = 0; b <= py; ++b) g->y0[b] = G.y0[b];
+  }
+  g->m.assign(n, nullptr); g->table.assign(n, nullptr); g->ev.assign(n, nullptr);
+  auto cleanup = [&](int rc) { const std::string keep = g_err; smaug_group_destroy(g); g_err = keep; return rc; };
+  const int member_bc[4] = {SMAUG_BC_OPEN, SMAUG_BC_OPEN, SMAUG_BC_OPEN, SMAUG_BC_OPEN};   // placeholder: the group fills
+  std::vector<double> sub;              // host staging of a member's background block when bg is a host pointer
+  for (int b = 0; b < py; ++b)
+    for (int a = 0; a < px; ++a) {
+      const int k = b * px + a;
+      const int mnx = g->x0[a + 1] - g->x0[a], mny = g->y0[b + 1] - g->y0[b];
+      DeviceGuard dg(dev[k]);
+      cudaStream_t st = nullptr;
+      if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess)
+        return cleanup(fail(SMAUG_ECUDA, "cudaStreamCreate failed"));
+      smaug_ctx* c = nullptr;
+      // the background block is copied below (strided out of the global array); create with a dummy non-NULL marker
+      int rc = smaug_create_in_workspace(mnx, mny, gamma, member_bc, nullptr, nullptr, 0, st, &c);
+      if (rc) { cudaStreamDestroy(st); return cleanup(rc); }
+      g->m[k] = c;
+      c->group = g;
+      c->geo_nx = nx; c->geo_ny = ny;
+      c->use_graph = 0;
+      if (cudaMalloc((void**)&g->table[k], sizeof(GroupTable)) != cudaSuccess) return cleanup(fail(SMAUG_ENOMEM, "cudaMalloc of the group table failed"));
+      if (cudaEventCreateWithFlags(&g->ev[k], cudaEventDisableTiming) != cudaSuccess) return cleanup(fail(SMAUG_ECUDA, "cudaEventCreate failed"));
+    }
+  if (bg) {
+    // members were created without a background: give each one its block of the four planes now
+    for (int k = 0; k < n; ++k) {
+      smaug_ctx* c = g->m[k];
+      DeviceGuard dg(c->device);
+      const int a = k % px, b = k / px;
+      const size_t plane_bytes = c->L.state_bytes / NF;
+      double* mem = nullptr;
+      if (cudaMalloc((void**)&mem, NBG * plane_bytes) != cudaSuccess) return cleanup(fail(SMAUG_ENOMEM, "cudaMalloc of a background block failed"));
+      c->bg_owned = mem;
+      if (cudaMemsetAsync(mem, 0, NBG * plane_bytes, c->stream) != cudaSuccess) return cleanup(fail(SMAUG_ECUDA, "cudaMemsetAsync failed"));
+      for (int f = 0; f < NBG; ++f) {
+        c->bg.p[f] = (const double*)((char*)mem + f * plane_bytes);
+        const double* src = bg + ((size_t)f * ny + g->y0[b]) * nx + g->x0[a];
+        if (cudaMemcpy2DAsync((double*)c->bg.p[f] + cell_addr(c->g, 0, 0), (size_t)c->g.pitch * sizeof(double), src,
+                              (size_t)nx * sizeof(double), (size_t)c->g.nx * sizeof(double), c->g.ny, cudaMemcpyDefault,
+                              c->stream) != cudaSuccess)
+          return cleanup(fail(SMAUG_ECUDA, "copy of a background block failed"));
+      }
+      c->has_bg = true;
+    }
+  }
+  // shared scalars: the leader's
+  for (int k = 1; k < n; ++k) g->m[k]->sc = g->m[0]->sc;
+  g->one_stream = false;
+  int rc = group_upload_tables(g);
+  if (!rc && bg) {
+    rc = group_sync(g);
+    if (!rc) rc = group_exchange(g, 4, NBG, 1);       // c-8: background ghosts once (periodic -> wrap, else nearest interior)
+  }
+  if (!rc) rc = group_sync(g);
+  if (rc) return cleanup(rc);
+  *out = g;
+  return SMAUG_OK;
+}
+
+int smaug_group_size(smaug_group* g, int* px, int* py) {
+  if (int rc = group_check(g)) return rc;
+  if (px) *px = g->px;
+  if (py) *py = g->py;
+  return SMAUG_OK;
+}
+
+int smaug_group_set_param(smaug_group* g, int key, double value) {
+  if (int rc = group_check(g)) return rc;
+  if (key == SMAUG_PARAM_GRAPH) return SMAUG_OK;      // groups always launch plainly
+  for (smaug_ctx* c : g->m)
+    if (int rc = smaug_set_param(c, key, value)) return rc;
+  return SMAUG_OK;
+}
+
+int smaug_group_set_state(smaug_group* g, const double* w) {
+  if (int rc = group_check(g)) return rc;
+  if (!w) return fail(SMAUG_EINVAL, "w is NULL");
+  int rc = group_sync(g);
+  if (rc) return rc;
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    smaug_ctx* c = g->m[k];
+    DeviceGuard dg(c->device);
+    const int a = (int)k % g->px, b = (int)k / g->px;
+    for (int f = 0; f < NF; ++f) {
+      const double* src = w + ((size_t)f * g->NY + g->y0[b]) * g->NX + g->x0[a];
+      CU(cudaMemcpy2DAsync(c->buf[0].p[f] + cell_addr(c->g, 0, 0), (size_t)c->g.pitch * sizeof(double), src,
+                           (size_t)g->NX * sizeof(double), (size_t)c->g.nx * sizeof(double), c->g.ny,
+                           cudaMemcpyDefault, c->stream));
+    }
+  }
+  {
+    smaug_ctx* L = g->m[0];
+    DeviceGuard dg(L->device);
+    CU(cudaMemsetAsync(L->sc, 0, sizeof(DeviceScalars), L->stream));
+  }
+  if ((rc = group_barrier(g))) return rc;
+  if ((rc = group_exchange(g, 0, NF, 1))) return rc;   // fixed sides are frozen here, as in smaug_set_state
+  for (smaug_ctx* c : g->m) {
+    DeviceGuard dg(c->device);
+    for (int b = 1; b <= 2; ++b)
+      for (int f = 0; f < NF; ++f)
+        CU(cudaMemcpyAsync(c->buf[b].p[f], c->buf[0].p[f], (size_t)c->g.plane * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    c->state_set = 0;
+    if ((rc = launch_wavespeeds(c, c->buf[0], 0))) return rc;
+  }
+  g->state_set = 0;
+  g->pending_status = false;
+  return group_sync(g);
+}
+
+int smaug_group_step(smaug_group* g, int n_steps, double cfl) {
+  if (int rc = group_check(g)) return rc;
+  if (n_steps < 0) return fail(SMAUG_EINVAL, "n_steps must be >= 0");
+  if (!(g->m[0]->fixed_dt > 0.0) && !(cfl > 0.0)) return fail(SMAUG_EINVAL, "cfl must be > 0");
+  for (int s = 0; s < n_steps; ++s)
+    if (int rc = group_enqueue_step(g, cfl)) return rc;
+  if (n_steps > 0) g->pending_status = true;
+  return group_status(g);
+}
+
+int smaug_group_get_state(smaug_group* g, double* w) {
+  if (int rc = group_check(g)) return rc;
+  if (!w) return fail(SMAUG_EINVAL, "w is NULL");
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    smaug_ctx* c = g->m[k];
+    DeviceGuard dg(c->device);
+    const int a = (int)k % g->px, b = (int)k / g->px;
+    for (int f = 0; f < NF; ++f) {
+      double* dst = w + ((size_t)f * g->NY + g->y0[b]) * g->NX + g->x0[a];
+      CU(cudaMemcpy2DAsync(dst, (size_t)g->NX * sizeof(double), c->buf[0].p[f] + cell_addr(c->g, 0, 0),
+                           (size_t)c->g.pitch * sizeof(double), (size_t)c->g.nx * sizeof(double), c->g.ny,
+                           cudaMemcpyDefault, c->stream));
+    }
+  }
+  return group_status(g);
+}
+
+int smaug_group_get_time(smaug_group* g, double* t, double* last_dt) {
+  if (int rc = group_check(g)) return rc;
+  int rc = group_status(g);
+  smaug_ctx* L = g->m[0];
+  DeviceGuard dg(L->device);
+  double v[2];
+  CU(cudaMemcpy(v, &L->sc->dt, 2 * sizeof(double), cudaMemcpyDeviceToHost));
+  if (last_dt) *last_dt = v[0];
+  if (t) *t = v[1];
+  return rc;
+}
+
+int smaug_group_get_wavespeeds(smaug_group* g, double out[4]) {
+  if (int rc = group_check(g)) return rc;
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  int rc = group_status(g);
+  smaug_ctx* L = g->m[0];
+  DeviceGuard dg(L->device);
+  CU(cudaMemcpy(out, L->sc->red[g->state_set], 4 * sizeof(double), cudaMemcpyDeviceToHost));
+  return rc;
+}
+
+int smaug_group_get_launch_count(smaug_group* g, long long* stage_and_aux, long long* exchange) {
+  if (int rc = group_check(g)) return rc;
+  long long n = 0;
+  for (smaug_ctx* c : g->m) n += c->launches;
+  if (stage_and_aux) *stage_and_aux = n - g->exchange_launches;
+  if (exchange) *exchange = g->exchange_launches;
+  return SMAUG_OK;
+}
+
+int smaug_group_map_cell(int px, int py, int nx, int ny, const int bc[4], int member, int i, int j, int freeze, int out[7]) {
+  if (!bc || !out) return fail(SMAUG_EINVAL, "NULL argument");
+  if (px < 1 || py < 1 || px > GROUP_MAX_SIDE || py > GROUP_MAX_SIDE || nx < px || ny < py || member < 0 || member >= px * py)
+    return fail(SMAUG_EINVAL, "bad decomposition");
+  const GroupGeom G = group_geom(px, py, nx, ny, bc);
+  const int a = member % px, b = member / px;
+  out[0] = G.x0[a]; out[1] = G.y0[b]; out[2] = G.x0[a + 1] - G.x0[a]; out[3] = G.y0[b + 1] - G.y0[b];
+  int sm = -1, si = 0, sj = 0;
+  const bool written = group_source_cell(G, member, i, j, freeze, &sm, &si, &sj);
+  out[4] = written ? sm : -1; out[5] = si; out[6] = sj;
   return SMAUG_OK;
 }
 
