@@ -16,7 +16,39 @@
 #pragma once
 #include "smaug_split_kernel.cuh"
 
+#ifndef SMAUG_FLUX_L2HINT
+#define SMAUG_FLUX_L2HINT 0     // 1: L2 eviction priorities -- in stages 2 and 4 the stage-input rows (read with their halo by the
+#endif                          // cp.async ring and once more pointwise two rows later) are fetched with evict_last, RK operands and
+                                // results go through with evict_first.  Measured at 8000^2 (profiles/r02_notes.md): DRAM bytes of
+                                // stage 2 / 4 fall from 1.29x / 1.08x to 1.12x / 1.05x of the algorithmic bytes, but stages 1 / 3
+                                // get slower and the step does not get faster (7.61 vs 7.53 ms): the kernel is bound by bytes in
+                                // flight over ~20 concurrent plane streams (5.2 TB/s of real DRAM traffic in stage 2), not by
+                                // the excess bytes.  Kept as a build option, off.
+
 namespace smaug {
+
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+  unsigned long long p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+  unsigned long long p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void cp_async8_hint(double* smem_dst, const double* gsrc, unsigned long long pol) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
+}
+__device__ __forceinline__ double ld_hint(const double* p, unsigned long long pol) {
+  double v;
+  asm volatile("ld.global.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ void st_hint(double* p, double v, unsigned long long pol) {
+  asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
 
 // BG = true: a background (with or without gravity): the four background planes ride in the landing ring, the
 // fluxes take their background terms (c-2), vx / vy of the head row go into a second ring for the x-derivatives of
@@ -63,10 +95,28 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
   int fetched = ystart - 2;                               // next row to fetch
   const int last_row = g.ny + NG - 1;
   int slot_f = 0;                                         // landing slot of the next row to fetch
+#if SMAUG_FLUX_L2HINT
+  const unsigned long long pol_keep = l2_policy_evict_last(), pol_once = l2_policy_evict_first();
+#endif
+#if SMAUG_FLUX_L2HINT
+#define LD_ONCE(p) ld_hint((p), pol_once)
+#define ST_ONCE(p, v) st_hint((p), (v), pol_once)
+#else
+#define LD_ONCE(p) (*(p))
+#define ST_ONCE(p, v) (*(p) = (v))
+#endif
   auto fetch_row = [&]() {
     double* dst = INR + slot_f * NIN * NT + tid;
+#if SMAUG_FLUX_L2HINT
+    if (combine != COMBINE_BASE) {
 #pragma unroll
-    for (int f = 0; f < NF; ++f) cp_async8(dst + f * NT, a.in.p[f] + gin);
+      for (int f = 0; f < NF; ++f) cp_async8_hint(dst + f * NT, a.in.p[f] + gin, pol_keep);
+    } else
+#endif
+    {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) cp_async8(dst + f * NT, a.in.p[f] + gin);
+    }
     if constexpr (BG) {
 #pragma unroll
       for (int k = 0; k < NBG; ++k) cp_async8(dst + (NF + k) * NT, a.bg.p[k] + gin);
@@ -97,10 +147,10 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
     if (tail_on) {
       if (combine == COMBINE_FINAL) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = a.acc_in.p[f][gj]; }
+        for (int f = 0; f < NF; ++f) { jin[f] = a.in.p[f][gj]; jacc[f] = LD_ONCE(a.acc_in.p[f] + gj); }
       } else {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) jbase[f] = a.base.p[f][gj];
+        for (int f = 0; f < NF; ++f) jbase[f] = LD_ONCE(a.base.p[f] + gj);
         if (combine == COMBINE_ACC) {
 #pragma unroll
           for (int f = 0; f < NF; ++f) jin[f] = a.in.p[f][gj];
@@ -231,10 +281,10 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
       }
       if (col_out) {            // then cl == ci: gj is the address of the output cell as well
 #pragma unroll
-        for (int f = 0; f < NF; ++f) a.out.p[f][gj] = o[f];
+        for (int f = 0; f < NF; ++f) ST_ONCE(a.out.p[f] + gj, o[f]);
         if (combine == COMBINE_ACC) {
 #pragma unroll
-          for (int f = 0; f < NF; ++f) a.acc_out.p[f][gj] = fma(2.0, o[f], jin[f] - jbase[f]);
+          for (int f = 0; f < NF; ++f) ST_ONCE(a.acc_out.p[f] + gj, fma(2.0, o[f], jin[f] - jbase[f]));
         }
         if (ws_mode != WS_NONE) {
           double w4[4];
@@ -254,5 +304,8 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
   cp_async_wait<0>();
   if (ws_mode != WS_NONE) block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], ws_mode == WS_FULL ? 0 : 2);
 }
+
+#undef LD_ONCE
+#undef ST_ONCE
 
 }  // namespace smaug

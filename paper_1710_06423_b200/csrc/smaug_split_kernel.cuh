@@ -147,7 +147,7 @@ __device__ __forceinline__ double kappa_q(double m3, double m1, double cv, int& 
 constexpr int ORDINARY_HI = 0x06400000;     // high word of 2^-923: below it ratio_div rescales
 
 #ifndef SMAUG_KAPPA_FAST
-#define SMAUG_KAPPA_FAST 0      // 1: the guarded kappa of a family is the plain exact division, redone with the zero
+#define SMAUG_KAPPA_FAST 1      // 1: the guarded kappa of a family is the plain exact division, redone with the zero
 #endif                          //    guard and the 2^200 rescue only when a warp vote finds an M1 below 2^-923 (same
                                 //    bits: the rescue scales by 1.0 above that); the redo is a few lines, not a section
 // kappa of N ratios of one family (N = 2: the two interfaces of a column pair; N = 1: one y-interface)
