@@ -62,9 +62,12 @@ enum { /* keys of smaug_set_param */
   SMAUG_PARAM_C_B = 6,      /*   0.02 */
   SMAUG_PARAM_RK_ORDER = 7, /* 4 (default), 2 (midpoint) or 1 (forward Euler) */
   SMAUG_PARAM_FIXED_DT = 8, /* > 0: use this dt instead of the CFL step; 0 (default): CFL */
-  SMAUG_PARAM_KERNEL = 9,   /* 2 (default): role-split streaming stage kernel where applicable (hyperdiffusion on;
-                               with or without a background); 1: single-role streaming kernel where applicable
-                               (no background); 0: always the tile kernel.  All are bit-identical; the switch exists for tests and profiling. */
+  SMAUG_PARAM_KERNEL = 9,   /* which fused stage kernel runs.  2 (default): the fastest applicable form -- the role-split
+                               streaming kernel (hyperdiffusion on), the streaming flux kernel (off), and for a
+                               one-dimensional problem (ny = 1, nx <= 976, y-boundary not fixed, no background, RK4 / RK2) the small-grid path:
+                               whole time steps in one persistent cluster launch.  3: as 2 without the small-grid path.
+                               1: single-role streaming kernel where applicable (no background).  0: always the tiled
+                               kernel.  All forms are bit-identical; the switch exists for tests and profiling. */
   SMAUG_PARAM_GX = 10,      /* uniform gravitational acceleration g = (GX, GY) of PAPER.md:35 ("rho g", "rho g.v"); */
   SMAUG_PARAM_GY = 11,      /*   default 0.  Split form (c-10): the background is taken to be in magneto-hydrostatic
                                balance  grad p_tb - (B_b.grad)B_b = rho_b g,  so gravity acts on the perturbed
@@ -127,8 +130,8 @@ int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
 
 /* Name of the fused stage kernel the context's current parameters select (static string, never NULL;
  * "?" for a NULL context): "split_kernel<128>" (role-split streaming form), "march_kernel<256>"
- * (single-role streaming form), "flux_kernel<128>" (streaming form without hyperdiffusion) or
- * "stage_kernel<32,8,512>" (tiled form: forced by SMAUG_PARAM_KERNEL = 0). */
+ * (single-role streaming form), "flux_kernel<128>" (streaming form without hyperdiffusion),
+ * "line_step_kernel<128>" (small-grid path) or "stage_kernel<32,8,512>" (tiled form: SMAUG_PARAM_KERNEL = 0). */
 const char* smaug_get_kernel_name(smaug_ctx* ctx);
 
 /* Device time, in milliseconds, spent in the fused stage kernels (summed over launches) and the number of

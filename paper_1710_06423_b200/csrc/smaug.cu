@@ -15,6 +15,7 @@
 #include "smaug_flux_kernel.cuh"
 #include "smaug_selftest.cuh"
 #include "smaug_group.cuh"
+#include "smaug_line_kernel.cuh"
 
 using namespace smaug;
 
@@ -127,6 +128,8 @@ struct smaug_ctx {
   int kernel_mode = 2;      // SMAUG_PARAM_KERNEL: 2 role-split streaming kernel, 1 single-role streaming kernel
                             // (both only without background and with hyperdiffusion), 0 always the tile kernel
   int n_sm = 148;
+  long long line_stage_equiv = 0;   // stages run inside line launches beyond the one the event pair counts (timing)
+  bool line_ok = true;      // cleared if the device refuses the cluster launch of the small-grid path
   int device = 0;           // the device the workspace lives on; every ABI entry makes it current (DeviceGuard)
   // member of a decomposition group (smaug_group_*): the GLOBAL cell counts fix Delta and the n = 1 rule of c-7, the
   // reduction slots / dt / t / status are the group leader's, the ghost fill is the group's exchange kernel
@@ -370,8 +373,15 @@ int launch_flux(smaug_ctx* c, const StageArgs& a) {
 // The streaming kernels cover every configuration; the tiled kernel runs when SMAUG_PARAM_KERNEL = 0 (tests), and
 // hyperdiffusion-on cases when SMAUG_PARAM_KERNEL = 1 excludes the split kernel and march_kernel does not apply.
 bool plain(const smaug_ctx* c) { return !c->has_bg && c->gx == 0.0 && c->gy == 0.0; }
+// The small-grid path (smaug_line_kernel.cuh): a one-dimensional problem that one cluster of <= 8 CTAs covers, the
+// y-boundary periodic or open (ghost rows are then copies of the row), no background, RK4 or RK2, not a member of a
+// group, default kernel selection.
+bool uses_line(const smaug_ctx* c) {
+  return c->kernel_mode == 2 && !c->has_bg && !c->group && c->g.ny == 1 && c->g.nx <= LINE_MAX_NX &&
+         c->g.bc[2] != BC_FIXED && c->g.bc[3] != BC_FIXED && (c->rk_order == 4 || c->rk_order == 2) && c->line_ok;
+}
 bool uses_flux(const smaug_ctx* c) { return !c->hd_on && c->kernel_mode != 0; }
-bool uses_split(const smaug_ctx* c) { return c->hd_on && c->kernel_mode == 2; }
+bool uses_split(const smaug_ctx* c) { return c->hd_on && c->kernel_mode >= 2; }
 bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_mode == 1; }
 
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
@@ -448,6 +458,51 @@ int enqueue_step(smaug_ctx* c, double cfl) {
   if (!rc && c->rk_order == 1) std::swap(c->buf[0], c->buf[1]);
   c->state_set = B;
   return rc;
+}
+
+// n whole time steps of a one-dimensional problem in one persistent cluster launch.
+template <bool HD>
+int launch_line_t(smaug_ctx* c, int n_steps, double cfl) {
+  static unsigned long long configured = 0;
+  constexpr size_t smem = LineSmem::BYTES;
+  auto kern = line_step_kernel<HD>;
+  CU(configure_smem(kern, smem, c->device, configured));
+  LineArgs la;
+  la.g = c->g;
+  la.prm = make_params(c);
+  for (int b = 0; b < 4; ++b) la.buf[b] = c->buf[b];
+  la.sc = c->sc;
+  la.state_set = c->state_set;
+  la.n_steps = n_steps;
+  la.rk_order = c->rk_order;
+  la.cfl = cfl; la.fixed_dt = c->fixed_dt;
+  la.dx = c->Lx / c->geo_nx; la.dy = c->Ly / c->geo_ny;
+  const int ntiles = (c->g.nx + LINE_W - 1) / LINE_W;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(ntiles); cfg.blockDim = dim3(LINE_NT); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = ntiles; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing && c->ev_used + 2 <= c->ev.size()) {
+    e0 = c->ev[c->ev_used++];
+    e1 = c->ev[c->ev_used++];
+    CU(cudaEventRecord(e0, c->stream));
+  }
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, la);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    c->line_ok = false;                 // fall back to the ordinary launch sequence for this context
+    if (e0) c->ev_used -= 2;
+    return 1;
+  }
+  if (e1) CU(cudaEventRecord(e1, c->stream));
+  c->last_ctas = ntiles;
+  c->launches++;
+  c->line_stage_equiv += (long long)n_steps * (c->rk_order == 4 ? 4 : 2) - 1;   // the event pair counts as one launch
+  if (n_steps & 1) c->state_set = c->state_set == 0 ? 4 : 0;
+  return SMAUG_OK;
 }
 
 void invalidate_graphs(smaug_ctx* c) {
@@ -548,6 +603,8 @@ int collect_timing(smaug_ctx* c) {
     c->stage_launches++;
   }
   c->ev_used = 0;
+  c->stage_launches += c->line_stage_equiv;
+  c->line_stage_equiv = 0;
   return SMAUG_OK;
 }
 
@@ -705,7 +762,7 @@ int smaug_set_param(smaug_ctx* c, int key, double v) {
     case SMAUG_PARAM_C_B: if (!(v >= 0)) break; c->c_b = v; return SMAUG_OK;
     case SMAUG_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c->rk_order = (int)v; return SMAUG_OK;
     case SMAUG_PARAM_FIXED_DT: if (!(v >= 0)) break; c->fixed_dt = v; return SMAUG_OK;
-    case SMAUG_PARAM_KERNEL: if (v != 0 && v != 1 && v != 2) break; c->kernel_mode = (int)v; return SMAUG_OK;
+    case SMAUG_PARAM_KERNEL: if (v != 0 && v != 1 && v != 2 && v != 3) break; c->kernel_mode = (int)v; return SMAUG_OK;
     case SMAUG_PARAM_GRAPH: c->use_graph = v != 0.0; return SMAUG_OK;
     case SMAUG_PARAM_GX: if (!std::isfinite(v)) break; c->gx = v; return SMAUG_OK;
     case SMAUG_PARAM_GY: if (!std::isfinite(v)) break; c->gy = v; return SMAUG_OK;
@@ -740,6 +797,14 @@ int smaug_step_async(smaug_ctx* c, int n_steps, double cfl) {
   if (n_steps < 0) return fail(SMAUG_EINVAL, "n_steps must be >= 0");
   if (c->group) return fail(SMAUG_EINVAL, "this context is a member of a group: step it with smaug_group_step");
   if (!(c->fixed_dt > 0.0) && !(cfl > 0.0)) return fail(SMAUG_EINVAL, "cfl must be > 0");
+  if (n_steps > 0 && uses_line(c)) {
+    const int rc = c->hd_on ? launch_line_t<true>(c, n_steps, cfl) : launch_line_t<false>(c, n_steps, cfl);
+    if (rc == SMAUG_OK) {
+      c->pending_status = true;
+      return SMAUG_OK;
+    }
+    if (rc < 0) return rc;              // rc == 1: the cluster launch was refused; use the ordinary sequence below
+  }
   // Whole steps as CUDA-graph replays: worth it when launches are a visible share of the step (small grids);
   // harmless otherwise.  Not while per-kernel timing events are wanted, and not for Euler (its buffers swap).
   if (c->use_graph && !c->timing && c->rk_order != 1 && n_steps > 0 &&
@@ -817,7 +882,9 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (int rc = check_ctx(c)) return rc;
   DeviceGuard guard_(c->device);
   if (!out) return fail(SMAUG_EINVAL, "out is NULL");
-  if (uses_flux(c)) {                                      // streaming kernel without HD: a strip of NT-4 columns
+  if (uses_line(c)) {                                      // small-grid path: one cluster of tiles, whole steps per launch
+    out[0] = LINE_W; out[1] = 1; out[2] = LINE_NT; out[3] = (int)LineSmem::BYTES;
+  } else if (uses_flux(c)) {                               // streaming kernel without HD: a strip of NT-4 columns
     out[0] = FLUX_NT - 4; out[1] = 1; out[2] = FLUX_NT;
     out[3] = (int)(c->has_bg ? FluxSmem<FLUX_NT, true>::BYTES : FluxSmem<FLUX_NT>::BYTES);
   } else if (uses_split(c)) {   // role-split streaming kernel: a strip of NC-8 columns
@@ -836,6 +903,7 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
 
 const char* smaug_get_kernel_name(smaug_ctx* c) {
   if (!c) return "?";
+  if (uses_line(c)) return "line_step_kernel<128>";
   if (uses_flux(c)) return FLUX_NT == 128 ? "flux_kernel<128>" : "flux_kernel";
   if (uses_split(c)) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
   if (uses_march(c)) return "march_kernel<256>";
@@ -850,6 +918,7 @@ int smaug_set_kernel_timing(smaug_ctx* c, int on) {
   c->ev_used = 0;
   c->stage_ms = 0;
   c->stage_launches = 0;
+  c->line_stage_equiv = 0;
   if (c->timing && c->ev.empty()) {
     c->ev.resize(2048);
     for (auto& e : c->ev) CU(cudaEventCreate(&e));

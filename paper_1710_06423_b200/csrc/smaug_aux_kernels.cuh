@@ -96,13 +96,12 @@ __device__ __forceinline__ int wrap_idx(int i, int n) {
   return r < 0 ? r + n : r;
 }
 
-__global__ void __launch_bounds__(256) ghost_fill_kernel(Grid g, Planes6 pl, int freeze) {
-  double* p = pl.p[blockIdx.y];
+// the ghost cells of one plane, shared out over `nthreads` threads of which this is number `t`
+__device__ __forceinline__ void ghost_fill_plane(const Grid& g, double* p, int freeze, long long t, long long nthreads) {
   const int wpad = g.nx + 2 * NG;
   const long long n_y = 2LL * NG * wpad;                 // cells in the 6 ghost rows
   const long long total = n_y + 2LL * NG * g.ny;         // + 6 ghost columns of every interior row
-  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total;
-       q += (long long)gridDim.x * blockDim.x) {
+  for (long long q = t; q < total; q += nthreads) {
     int i, j;
     if (q < n_y) {
       const int row = (int)(q / wpad);
@@ -130,14 +129,19 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(Grid g, Planes6 pl, int
   }
 }
 
+__global__ void __launch_bounds__(256) ghost_fill_kernel(Grid g, Planes6 pl, int freeze) {
+  ghost_fill_plane(g, pl.p[blockIdx.y], freeze, (long long)blockIdx.x * blockDim.x + threadIdx.x,
+                   (long long)gridDim.x * blockDim.x);
+}
+
 // ------------------------------------------------------------------------------------------------
 // dt (c-7), one thread:  dt = cfl * min_d(Delta_d / cmax_d), an axis with n = 1 excluded; or fixed_dt.
 // Also advances t, raises the sticky status on a non-finite / non-positive dt, and clears the reduction
 // sets the coming step will accumulate into (bit mask `clear_sets`).
 // ------------------------------------------------------------------------------------------------
-__global__ void dt_kernel(DeviceScalars* s, int state_set, unsigned clear_sets, double cfl, double fixed_dt,
-                          double dx, double dy, int nx, int ny) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
+__device__ __forceinline__ void dt_body(DeviceScalars* s, int state_set, unsigned clear_sets, double cfl, double fixed_dt,
+                                        double dx, double dy, int nx, int ny) {
+  {
     double dt = fixed_dt;
     if (!(fixed_dt > 0.0)) {
       const double cx = __longlong_as_double((long long)s->red[state_set][0]);
@@ -155,6 +159,11 @@ __global__ void dt_kernel(DeviceScalars* s, int state_set, unsigned clear_sets, 
         s->red[k][0] = 0ULL; s->red[k][1] = 0ULL; s->red[k][2] = 0ULL; s->red[k][3] = 0ULL;
       }
   }
+}
+
+__global__ void dt_kernel(DeviceScalars* s, int state_set, unsigned clear_sets, double cfl, double fixed_dt,
+                          double dx, double dy, int nx, int ny) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) dt_body(s, state_set, clear_sets, cfl, fixed_dt, dx, dy, nx, ny);
 }
 
 __global__ void clear_red_kernel(DeviceScalars* s, unsigned clear_sets) {

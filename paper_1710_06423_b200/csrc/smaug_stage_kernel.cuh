@@ -118,10 +118,11 @@ __device__ __forceinline__ void kappa_run(const double* __restrict__ u, int s, d
   }
 }
 
+// One RK stage on the TH x TW tile whose first interior cell is (x0, y0); all NT threads of the CTA call it together.
+// Reads a.in with its halo (ghosts filled), writes the tile's cells of a.out (and a.acc_out), reduces into a.sc->red.
 template <int TW, int TH, int NT, bool BG, bool HD>
-__global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
+__device__ __forceinline__ void stage_tile(const StageArgs& a, const int x0, const int y0, double* const smem) {
   using T = Tile<TW, TH, BG>;
-  extern __shared__ double smem[];
   double* const U = smem + T::OFF_U;
   double* const KX = smem + T::OFF_KX;
   double* const KY = smem + T::OFF_KY;
@@ -130,7 +131,6 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
   double* const red_sh = smem + T::OFF_RED;
   const Grid& g = a.g;
   const int tid = threadIdx.x;
-  const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;   // interior coordinates of the tile origin
   const double gamma = a.prm.gamma, gm1 = a.prm.gamma - 1.0;
 
   // ---------------------------------------------------------------- P1: stage derived planes + fluxes
@@ -424,6 +424,12 @@ __global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
   }
   if (a.ws_mode != WS_NONE)
     block_max4_atomic(wsmax, red_sh, a.sc->red[a.red_out], a.ws_mode == WS_FULL ? 0 : 2);
+}
+
+template <int TW, int TH, int NT, bool BG, bool HD>
+__global__ void __launch_bounds__(NT) stage_kernel(const StageArgs a) {
+  extern __shared__ double smem[];
+  stage_tile<TW, TH, NT, BG, HD>(a, blockIdx.x * TW, blockIdx.y * TH, smem);
 }
 
 }  // namespace smaug

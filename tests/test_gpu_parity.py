@@ -490,3 +490,47 @@ def test_gravity_on_zero_background_without_hyperdiffusion(gpu, oracle_mod):
     b = cpu_run(oracle_mod, w, bc, gamma, 15, gx=0.3, gy=gy, hd_on=0)
     check(*a, *b)
     assert np.array_equal(a[0], t[0])
+
+
+# ----------------------------------------------------------------------------- small-grid path (one-dimensional problems)
+@pytest.mark.parametrize("nx,bc,params", [
+    (800, (1, 1, 0, 0), {}), (976, (0, 0, 0, 0), {}), (129, (2, 1, 0, 0), dict(c_mom=0.2)), (127, (1, 2, 0, 0), dict(rk_order=2)),
+    (5, (0, 0, 0, 0), {}), (1, (0, 0, 0, 0), dict(fixed_dt=1e-3)), (300, (1, 1, 0, 0), dict(hd_on=0)), (513, (0, 0, 0, 0), dict(gx=0.3, gy=-0.2)),
+    (640, (2, 2, 1, 1), {}), (122, (0, 0, 1, 1), dict(hd_on=0, rk_order=2)), (123, (1, 1, 0, 0), {})])
+def test_line_kernel_whole_steps_in_one_launch(gpu, oracle_mod, nx, bc, params):
+    """The persistent cluster kernel of the small-grid path (ny = 1): against the oracle on every cell, against the
+    ordinary launch sequence (SMAUG_PARAM_KERNEL = 3), odd and even step counts per call (the reduction-set parity
+    flips inside the launch), several calls in a row, and one launch for all the steps of a call."""
+    import torch
+    if nx >= 8:
+        w, _, gamma = si.brio_wu(nx, 1)
+        w[1] += 0.05 * w[0] * np.sin(2 * np.pi * si.centres(nx))[None, :]
+    else:
+        w, _, gamma = si.smooth_random(nx, 1, seed=4, amp=5e-2)
+    s = gpu.Smaug(nx, 1, gamma, bc, **params)
+    assert s.kernel_name().startswith("line_step_kernel")
+    s.set_state(torch.from_numpy(w))
+    n0 = s.launch_count()
+    for n in (7, 1, 12):
+        s.step(n, 0.3)
+    assert s.launch_count() - n0 == 3                      # one launch per smaug_step call
+    a = (s.get_state().cpu().numpy(), s.time(), s.wavespeeds())
+    s.close()
+    b = cpu_run(oracle_mod, w, bc, gamma, 20, threads=1, **params)
+    check(*a, *b)
+    c = gpu_run(gpu, w, bc, gamma, 20, kernel=3, **params)
+    assert np.array_equal(a[0], c[0]) and a[1] == c[1] and list(a[2]) == list(c[2])
+
+
+def test_line_kernel_does_not_apply_beyond_one_cluster(gpu):
+    w, bc, gamma = si.brio_wu(977, 1)
+    s = gpu.Smaug(977, 1, gamma, bc)
+    assert s.kernel_name().startswith("split_kernel")
+    s.close()
+    s = gpu.Smaug(100, 1, gamma, (1, 1, 2, 2))             # a fixed y-boundary keeps ghost rows that are not copies
+    assert s.kernel_name().startswith("split_kernel")
+    s.close()
+    w, bc, gamma = si.brio_wu(64, 2)
+    s = gpu.Smaug(64, 2, gamma, bc)
+    assert s.kernel_name().startswith("split_kernel")
+    s.close()
