@@ -330,6 +330,55 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_decomp(args):
+    """--decomp PXxPY: the decomposed run of the workload on one device beside the unsplit run of the same steps
+    (the decomposition's own cost: exchange kernels, barriers between the members' streams, smaller launches)."""
+    import torch
+    import paper_1710_06423_b200 as pkg
+    pkg.lib()
+    px, py = (int(v) for v in args.decomp.lower().split("x"))
+    name = args.workload
+    nx, ny, _ = WORKLOADS[name]
+    w_np, bc, gamma, bg_np, (gx, gy) = make_state(name)
+    w_host = torch.from_numpy(w_np).pin_memory()
+    bg = None if bg_np is None else torch.from_numpy(bg_np).cuda()
+    params = dict(hd_on=0 if args.no_hd else 1, gx=gx, gy=gy, rk_order=args.rk_order)
+    K, W = args.steps, args.warmup
+
+    def timed(sim):
+        sim.set_state(w_host)
+        sim.step(W, 0.3)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sim.step(K, 0.3)                      # synchronises before returning
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) * 1e3
+
+    one = pkg.Smaug(nx, ny, gamma, bc, bg=bg, **params)
+    ms_one = timed(one)
+    t_one = one.time()
+    one.close()
+    grp = pkg.SmaugGroup(px, py, nx, ny, gamma, bc, bg=bg, **params)
+    ms_grp = timed(grp)
+    t_grp = grp.time()
+    n_stage, n_exch = grp.launch_count()
+    grp.close()
+    cells = float(nx) * ny
+    line = {
+        "metric": METRIC, "value": cells * K / (ms_grp * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W,
+        "ms_per_step": ms_grp / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": args.rk_order,
+                   "decomposition": f"{px}x{py} members on one device (smaug_group_*)",
+                   "timing": "host wall clock around the synchronising step call, after a device synchronise"},
+        "unsplit": {"value": cells * K / (ms_one * 1e-3), "ms_per_step": ms_one / K},
+        "decomposition_cost": ms_grp / ms_one - 1.0,
+        "bit_identical_time": list(t_grp) == list(t_one),
+        "gpu_launches": n_stage + n_exch, "exchange_launches": n_exch,
+    }
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -343,11 +392,16 @@ def main():
                          "graphs of whole steps, which is what a user gets -- matters on launch-bound small grids")
     ap.add_argument("--rk-order", type=int, default=4, choices=[4, 2],
                     help="4: classical RK4 (PAPER.md:45, the default); 2: midpoint rule (SURVEY 8(f) NEXT-4 extra row)")
+    ap.add_argument("--decomp", default=None, metavar="PXxPY",
+                    help="extra row (SURVEY 8(f) NEXT-1): run the workload as a PX x PY decomposition group on ONE device "
+                         "(halo pull through peer pointers, shared reduction, lockstep stages) and report its rate")
     ap.add_argument("--no-hd", action="store_true",
                     help="hyperdiffusion off (the 'Without HD' column of the paper's Table 1); extra row, not the default")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomp:
+        run_decomp(args)
     else:
         run_ours(args)
 

@@ -149,11 +149,13 @@ constexpr int ORDINARY_HI = 0x06400000;     // high word of 2^-923: below it rat
 #ifndef SMAUG_KAPPA_FAST
 #define SMAUG_KAPPA_FAST 1      // 1: the guarded kappa of a family is the plain exact division, redone with the zero
 #endif                          //    guard and the 2^200 rescue only when a warp vote finds an M1 below 2^-923 (same
-                                //    bits: the rescue scales by 1.0 above that); the redo is a few lines, not a section
+                                //    bits: the rescue scales by 1.0 above that); the redo is a few lines, not a section.
+                                //    8000^2: 3.30 -> 3.24 ms per stage without a background; the background form loses
+                                //    4.6 % with it (1.067 -> 1.116 ms at 4000^2), so it is taken for BG = false only
 // kappa of N ratios of one family (N = 2: the two interfaces of a column pair; N = 1: one y-interface)
-template <int N>
+template <int N, bool FAST>
 __device__ __forceinline__ void kappa_family(const double (&m3)[N], const double (&m1)[N], double cv, double (&k)[N]) {
-#if SMAUG_KAPPA_FAST
+  if constexpr (FAST) {
   int lo = __double2hiint(m1[0]);
 #pragma unroll
   for (int q = 1; q < N; ++q) lo = min(lo, __double2hiint(m1[q]));
@@ -163,15 +165,15 @@ __device__ __forceinline__ void kappa_family(const double (&m3)[N], const double
 #pragma unroll
     for (int q = 0; q < N; ++q) k[q] = kappa_ratio(m3[q], m1[q], cv);
   }
-#else
+  } else {
 #pragma unroll
   for (int q = 0; q < N; ++q) k[q] = kappa_ratio(m3[q], m1[q], cv);
-#endif
+  }
 }
 
 // kappa at the TWO adjacent interfaces (u[2] | u[3]) and (u[3] | u[4]) of the seven cells u[0..6] (c-5).
 // d0, d1: the first differences across the two interfaces.
-template <bool GUARD>
+template <bool GUARD, bool FAST = false>
 __device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0, double& k1, double& d0,
                                        double& d1, int& lo) {
   double a[6], t[4];
@@ -186,7 +188,7 @@ __device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0,
   if (GUARD) {
     const double m3[2] = {m3_0, m3_1}, m1[2] = {m1_0, m1_1};
     double k[2];
-    kappa_family<2>(m3, m1, cv, k);
+    kappa_family<2, FAST>(m3, m1, cv, k);
     k0 = k[0]; k1 = k[1];
   } else {
     k0 = kappa_q<GUARD>(m3_0, m1_0, cv, lo);
@@ -197,7 +199,7 @@ __device__ __forceinline__ void kappa7(const double u[7], double cv, double& k0,
 }
 
 // kappa at ONE interface from six cells, max chains with free |.| modifiers (same value as kappa6)
-template <bool GUARD>
+template <bool GUARD, bool FAST = false>
 __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, double u3, double u4, double u5,
                                           double cv, double& d1_mid, int& lo) {
   const double a0 = u1 - u0, a1 = u2 - u1, a2 = u3 - u2, a3 = u4 - u3, a4 = u5 - u4;
@@ -210,7 +212,7 @@ __device__ __forceinline__ double kappa6m(double u0, double u1, double u2, doubl
   if (GUARD) {
     const double m3a[1] = {m3}, m1a[1] = {m1};
     double k[1];
-    kappa_family<1>(m3a, m1a, cv, k);
+    kappa_family<1, FAST>(m3a, m1a, cv, k);
     return k[0];
   }
   return kappa_q<GUARD>(m3, m1, cv, lo);
@@ -323,6 +325,7 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) s
 (const StageArgs a, const MarchGeom mg) {
   using S = SplitSmem<NC, BG>;
   constexpr bool TM = S::TM;
+  constexpr bool KFAST = SMAUG_KAPPA_FAST != 0 && !BG;
   constexpr int PW = S::PW, NXT = NC / 2, NTH = NC + NC / 2;
   extern __shared__ __align__(16) double smem[];
   double* const UP = smem + S::OFF_UP;
@@ -486,24 +489,24 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) s
         };
         // kappa_x(rho~) on the perturbed density; the interface weights rho-bar use the total density
         if constexpr (BG) gather(6, rhot[0], rhot[1]); else gather(0, rho[0], rho[1]);
-        kappa7<GUARD>(u, cv_rho, k0, k1, d0, d1, lo);
+        kappa7<GUARD, KFAST>(u, cv_rho, k0, k1, d0, d1, lo);
         const double rho_r = BG ? UPr[0 * PW + tp + 2] : u[4];           // total density of the cell right of the pair
         const double rbar0 = 0.5 * (rho[0] + rho[1]), rbar1 = 0.5 * (rho[1] + rho_r);
         px[0][C_RHO] = k0 * d0; px[1][C_RHO] = k1 * d1;
         gather(1, vx[0], vx[1]);
-        kappa7<GUARD>(u, cv_mom, k0, k1, d0, d1, lo);
+        kappa7<GUARD, KFAST>(u, cv_mom, k0, k1, d0, d1, lo);
         px[0][C_MX] = (rbar0 * k0) * d0; px[1][C_MX] = (rbar1 * k1) * d1;
         const double vxbar0 = 0.5 * (u[2] + u[3]), vxbar1 = 0.5 * (u[3] + u[4]);
         gather(2, vy[0], vy[1]);
-        kappa7<GUARD>(u, cv_mom, kxv[0], kxv[1], d0, d1, lo);
+        kappa7<GUARD, KFAST>(u, cv_mom, kxv[0], kxv[1], d0, d1, lo);
         px[0][C_MY] = ((0.5 * rbar0) * kxv[0]) * d0; px[1][C_MY] = ((0.5 * rbar1) * kxv[1]) * d1;
         const double vybar0 = 0.5 * (u[2] + u[3]), vybar1 = 0.5 * (u[3] + u[4]);
         dcx_vy[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_vy[1] = cd12v(u[1], u[2], u[4], u[5]);
         gather(3, eps[0], eps[1]);
-        kappa7<GUARD>(u, cv_e, k0, k1, d0, d1, lo);
+        kappa7<GUARD, KFAST>(u, cv_e, k0, k1, d0, d1, lo);
         const double p_eps0 = k0 * d0, p_eps1 = k1 * d1;
         gather(4, by[0], by[1]);
-        kappa7<GUARD>(u, cv_b, kxb[0], kxb[1], d0, d1, lo);
+        kappa7<GUARD, KFAST>(u, cv_b, kxb[0], kxb[1], d0, d1, lo);
         px[0][C_B] = kxb[0] * d0; px[1][C_B] = kxb[1] * d1;
         dcx_by[0] = cd12v(u[0], u[1], u[3], u[4]); dcx_by[1] = cd12v(u[1], u[2], u[4], u[5]);
         // ohmic coupling with the TOTAL transverse field (u[] holds by~ here)
@@ -686,11 +689,11 @@ __global__ void __launch_bounds__(NC + NC / 2, SplitSmem<NC, BG>::CTAS_PER_SM) s
         constexpr bool GUARD = decltype(GUARD_)::value;
         int lo = 0x7fffffff;
         double d_rho, d_vx, d_vy, d_e, d_bx;
-        const double k_rho = kappa6m<GUARD>(hr[0], hr[1], hr[2], hr[3], hr[4], hr[5], cv_rho, d_rho, lo);
-        kyv = kappa6m<GUARD>(hvx[0], hvx[1], hvx[2], hvx[3], hvx[4], hvx[5], cv_mom, d_vx, lo);
-        const double k_vy = kappa6m<GUARD>(hvy[0], hvy[1], hvy[2], hvy[3], hvy[4], hvy[5], cv_mom, d_vy, lo);
-        const double k_e = kappa6m<GUARD>(he[0], he[1], he[2], he[3], he[4], he[5], cv_e, d_e, lo);
-        kyb = kappa6m<GUARD>(hbx[0], hbx[1], hbx[2], hbx[3], hbx[4], hbx[5], cv_b, d_bx, lo);
+        const double k_rho = kappa6m<GUARD, KFAST>(hr[0], hr[1], hr[2], hr[3], hr[4], hr[5], cv_rho, d_rho, lo);
+        kyv = kappa6m<GUARD, KFAST>(hvx[0], hvx[1], hvx[2], hvx[3], hvx[4], hvx[5], cv_mom, d_vx, lo);
+        const double k_vy = kappa6m<GUARD, KFAST>(hvy[0], hvy[1], hvy[2], hvy[3], hvy[4], hvy[5], cv_mom, d_vy, lo);
+        const double k_e = kappa6m<GUARD, KFAST>(he[0], he[1], he[2], he[3], he[4], he[5], cv_e, d_e, lo);
+        kyb = kappa6m<GUARD, KFAST>(hbx[0], hbx[1], hbx[2], hbx[3], hbx[4], hbx[5], cv_b, d_bx, lo);
         const double rbar = BG ? 0.5 * ((rb0 + hr[2]) + (rb1 + hr[3])) : 0.5 * (hr[2] + hr[3]);
         const double p_rho = k_rho * d_rho;
         const double p_mx = ((0.5 * rbar) * kyv) * d_vx;
