@@ -13,6 +13,10 @@
 #include <vector>
 
 #include "smaug_flux_kernel.cuh"
+#ifndef SMAUG_PRODUCT_ONLY             // -DSMAUG_PRODUCT_ONLY: a library without the two second implementations
+#include "smaug_march_kernel.cuh"      // (SMAUG_PARAM_KERNEL = 0 / 1 is then refused); the default build carries them:
+#include "smaug_stage_kernel.cuh"      // the parity tests run every form against the oracle and against each other
+#endif
 #include "smaug_selftest.cuh"
 #include "smaug_group.cuh"
 #include "smaug_line_kernel.cuh"
@@ -208,6 +212,7 @@ int launch_wavespeeds(smaug_ctx* c, const Planes6& w, int set) {
   return SMAUG_OK;
 }
 
+#ifndef SMAUG_PRODUCT_ONLY
 template <bool BG, bool HD>
 int launch_stage_t(smaug_ctx* c, const StageArgs& a) {
   static unsigned long long configured = 0;     // devices on which this instantiation has its smem limit raised
@@ -261,6 +266,8 @@ int launch_march(smaug_ctx* c, const StageArgs& a) {
   CU(cudaGetLastError());
   return SMAUG_OK;
 }
+
+#endif   // SMAUG_PRODUCT_ONLY
 
 #ifndef SMAUG_SPLIT_NC
 #define SMAUG_SPLIT_NC 128
@@ -387,9 +394,13 @@ bool uses_march(const smaug_ctx* c) { return plain(c) && c->hd_on && c->kernel_m
 int launch_stage(smaug_ctx* c, const StageArgs& a) {
   if (uses_flux(c)) return launch_flux(c, a);
   if (uses_split(c)) return launch_split(c, a);
+#ifndef SMAUG_PRODUCT_ONLY
   if (uses_march(c)) return launch_march(c, a);
   if (c->has_bg) return c->hd_on ? launch_stage_t<true, true>(c, a) : launch_stage_t<true, false>(c, a);
   return c->hd_on ? launch_stage_t<false, true>(c, a) : launch_stage_t<false, false>(c, a);
+#else
+  return fail(SMAUG_EINVAL, "this build carries no second implementations (SMAUG_PARAM_KERNEL = 0 / 1)");
+#endif
 }
 
 // The fused kernel of one stage (the ghosts of buffer `in` must be filled).
@@ -890,13 +901,16 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   } else if (uses_split(c)) {   // role-split streaming kernel: a strip of NC-8 columns
     out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
     out[3] = (int)(c->has_bg ? SplitSmem<SPLIT_NC, true>::BYTES : SplitSmem<SPLIT_NC>::BYTES);
-  } else if (uses_march(c)) {   // streaming kernel: a strip of NT-6 columns
+  }
+#ifndef SMAUG_PRODUCT_ONLY
+  else if (uses_march(c)) {   // streaming kernel: a strip of NT-6 columns
     out[0] = MARCH_NT - 2 * NG; out[1] = 1; out[2] = MARCH_NT;
     out[3] = (int)MarchSmem<MARCH_NT>::BYTES;
   } else {
     out[0] = TW; out[1] = TH; out[2] = NT;
     out[3] = (int)(c->has_bg ? Tile<TW, TH, true>::BYTES : Tile<TW, TH, false>::BYTES);
   }
+#endif
   out[4] = c->last_ctas;
   return SMAUG_OK;
 }

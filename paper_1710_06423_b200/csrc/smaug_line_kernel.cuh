@@ -23,7 +23,7 @@
 #pragma once
 #include <cooperative_groups.h>
 
-#include "smaug_march_kernel.cuh"
+#include "smaug_stage_common.cuh"
 
 namespace smaug {
 

@@ -18,13 +18,9 @@
 //   head  : Phi_x difference of row r -> ring; G(. ; y)(r); C_y(r) = F_y(r) - G -> ring
 //   tail C: central y-difference of C_y(j) from the ring; R(j); RK combine; write row j; wave-speed maxima
 #pragma once
-#include "smaug_stage_kernel.cuh"
+#include "smaug_stage_common.cuh"
 
 namespace smaug {
-
-struct MarchGeom {
-  int rows_per_cta;   // output rows per CTA (chunk height)
-};
 
 template <int NT>
 struct MarchSmem {
@@ -40,31 +36,6 @@ struct MarchSmem {
   static constexpr int TOTAL = OFF_RED + 4 * 32;
   static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
 };
-
-// kappa at ONE interface from the six cells u[0..5] = cells -2 .. +3 around it (interface between u[2], u[3]).
-__device__ __forceinline__ double kappa6(double u0, double u1, double u2, double u3, double u4, double u5,
-                                         double cv, double& d1_mid) {
-  const double a0 = u1 - u0, a1 = u2 - u1, a2 = u3 - u2, a3 = u4 - u3, a4 = u5 - u4;   // D1 at -2 .. +2
-  const double t0 = dabs(fma(3.0, a1, -(u3 - u0)));     // D3 at interface -1
-  const double t1 = dabs(fma(3.0, a2, -(u4 - u1)));     // D3 at interface  0
-  const double t2 = dabs(fma(3.0, a3, -(u5 - u2)));     // D3 at interface +1
-  const double m3 = dmax(dmax(t0, t1), t2);
-  const double m1 = dmax(dmax(dmax(dabs(a0), dabs(a1)), dmax(dabs(a2), dabs(a3))), dabs(a4));
-  d1_mid = a2;
-  return kappa_ratio(m3, m1, cv);
-}
-
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
-  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-__device__ __forceinline__ double cd12v(double m2, double m1, double p1, double p2) {
-  return fma(8.0, p1 - m1, -(p2 - m2));
-}
 
 template <int NT>
 __global__ void __launch_bounds__(NT, 1) march_kernel(const StageArgs a, const MarchGeom mg) {

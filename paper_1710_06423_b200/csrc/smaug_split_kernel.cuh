@@ -29,7 +29,7 @@
 #pragma once
 #include <type_traits>
 
-#include "smaug_march_kernel.cuh"
+#include "smaug_stage_common.cuh"
 
 #ifndef SMAUG_SPLIT_DECOUPLE
 #define SMAUG_SPLIT_DECOUPLE 1

@@ -17,36 +17,9 @@
 //   P4  per cell: central differences of (F - G), interface-flux differences, source, RK combine, write,
 //       wave-speed maxima -> warp shuffles -> one atomicMax pass per CTA
 #pragma once
-#include "smaug_aux_kernels.cuh"
+#include "smaug_stage_common.cuh"
 
 namespace smaug {
-
-// What the epilogue does with R (c-6).  dt is read from device memory (no host sync).
-//   COMBINE_BASE : out = base + c dt R                      (stages 1..3 of RK4; Euler; midpoint)
-//   COMBINE_ACC  : out = base + c dt R;  acc = (in - base) + 2 out          (stage 2 of RK4)
-//   COMBINE_FINAL: out = in + (acc - 2 in)/3 + c dt R       (stage 4 of RK4, c = 1/6)
-// which is w^{n+1} = (w1 + 2 w2 + w3 - w^n)/3 + dt/6 R(w3), algebraically the classical RK4 update,
-// grouped so that R == 0 returns w^n bit for bit.
-enum { COMBINE_BASE = 0, COMBINE_ACC = 1, COMBINE_FINAL = 2 };
-// Wave-speed reduction of the written state: none, only {a^2, b^2} (v_t of the next stage), or all four.
-enum { WS_NONE = 0, WS_VT = 1, WS_FULL = 2 };
-
-struct StageArgs {
-  Grid g;
-  Params prm;
-  CPlanes6 in;       // stage input (ghost-filled), read with its halo
-  CPlanes6 base;     // w^n            (COMBINE_BASE / COMBINE_ACC)
-  CPlanes6 acc_in;   // accumulator    (COMBINE_FINAL)
-  Planes6 out;       // stage output (interior written)
-  Planes6 acc_out;   // accumulator    (COMBINE_ACC)
-  CPlanes4 bg;       // background (ghost-filled), only dereferenced when BG
-  DeviceScalars* sc;
-  int red_in;        // reduction set holding the maxima of `in`  (v_t)
-  int red_out;       // reduction set receiving the maxima of `out`
-  double c;          // RK coefficient multiplying dt R
-  int combine;
-  int ws_mode;
-};
 
 constexpr int odd_up(int v) { return (v % 2 == 0) ? v + 1 : v; }   // odd pitch: conflict-free columns
 
@@ -81,16 +54,6 @@ struct Tile {
 };
 
 enum { U_RHO = 0, U_VX, U_VY, U_EPS, U_BX, U_BY, U_RHOT, U_BXT, U_BYT };   // last three: background only
-enum { K_RHO = 0, K_VX = 1, K_VY = 2, K_EPS = 3, K_B = 4 };                 // kappa families; Phi components
-enum { C_RHO = 0, C_MX = 1, C_MY = 2, C_E = 3, C_B = 4 };
-
-// max of two non-negative doubles: one DSETP + two selects (fmax() costs ~7 instructions on sm_100a
-// because of its NaN-quieting semantics).  max is exact, so any evaluation order is bit-safe.
-__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
-// |x| as one integer op on the high word (keeps the fp64 pipe free; bit-identical to fabs)
-__device__ __forceinline__ double dabs(double x) {
-  return __hiloint2double(__double2hiint(x) & 0x7fffffff, __double2loint(x));
-}
 
 // kappa = cv * (M3 / M1) for n <= R consecutive interfaces of one line (c-5).  u points at the cell left of
 // the first interface (interface k lies between cells k and k+1); cells -2 .. R+2 are read with stride s.
