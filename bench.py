@@ -281,7 +281,7 @@ def run_ours(args):
         cap = ncu_capture(name + ("_nohd" if args.no_hd else "") + ("_rk%d" % args.rk_order if args.rk_order != 4 else ""))
         fp64_per_cell = cap.get("fp64_thread_inst_per_cell")
         avg_launch_ms = stage_ms / max(stage_n, 1)
-        achieved = per_launch_bytes / (avg_launch_ms * 1e-3) / 1e9 if stage_n else None
+        achieved = per_launch_bytes / (avg_launch_ms * 1e-3) / 1e9 if stage_n and avg_launch_ms > 0 else None
         state_bytes = 6 * 8 * cells
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -305,7 +305,7 @@ def run_ours(args):
                            "unit": "T fp64-instr/s", "instr_per_cell_stage": fp64_per_cell,
                            "note": "secondary ceiling: fp64-pipe thread-instructions per cell and launch from the "
                                    "committed ncu capture (sm__inst_executed_pipe_fp64), x cells / measured duration"}
-                          if stage_n and fp64_per_cell else None),
+                          if stage_n and avg_launch_ms > 0 and fp64_per_cell else None),
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
                     "d2h_bytes_per_step": state_bytes / K,
                     "note": "smaug_set_state(host) + smaug_step(K) + smaug_get_state(host), pinned host memory"},

@@ -511,7 +511,7 @@ int launch_line_t(smaug_ctx* c, int n_steps, double cfl) {
   if (e1) CU(cudaEventRecord(e1, c->stream));
   c->last_ctas = ntiles;
   c->launches++;
-  c->line_stage_equiv += (long long)n_steps * (c->rk_order == 4 ? 4 : 2) - 1;   // the event pair counts as one launch
+  if (e1) c->line_stage_equiv += (long long)n_steps * (c->rk_order == 4 ? 4 : 2) - 1;   // the event pair counts as one launch
   if (n_steps & 1) c->state_set = c->state_set == 0 ? 4 : 0;
   return SMAUG_OK;
 }
