@@ -105,7 +105,11 @@ int smaug_set_state(smaug_ctx* ctx, const double* w);
 /* Advance n_steps time steps: per step  dt = cfl * min_d(Delta_d / cmax_d)  (c-7; an axis with n = 1 is
  * excluded; or SMAUG_PARAM_FIXED_DT), then the RK stages, each = ghost fill + fused RHS/hyperdiffusion/
  * RK-combine/wavespeed-reduction kernel.  dt and the maxima stay on the device; the host synchronises
- * once, at the end, to read the status.  Returns SMAUG_ENONFINITE if any dt was non-finite or <= 0. */
+ * once, at the end, to read the status.  Returns SMAUG_ENONFINITE if any dt was non-finite or <= 0.
+ * Non-finite CELLS are not detected as such: the wave-speed maxima start at 0 and skip NaNs and negative values
+ * (c-4), so a local blow-up (NaN cells, negative pressure) leaves dt finite and the call returns SMAUG_OK with a
+ * state that contains NaNs; callers that need the check test the state they read back.  Bit-identity with the
+ * oracle is claimed for finite states only. */
 int smaug_step(smaug_ctx* ctx, int n_steps, double cfl);
 
 /* Same, but only enqueues the work; the status is picked up by the next synchronising call. */
