@@ -1,6 +1,8 @@
-// smaug.cu -- host side of libsmaug.so: the C ABI of include/smaug.h, device memory layout, and the
-// launch sequence of one time step.  No torch types, no CPU fallback: every numerical step is a kernel
-// from smaug_aux_kernels.cuh / smaug_stage_kernel.cuh.
+// smaug.cu -- host side of libsmaug.so: the C ABI of include/smaug.h, device memory layout, the launch sequence of
+// one time step (plain launches, CUDA-graph replays, the one-launch path of 1-D problems) and the decomposition
+// groups.  No torch types, no CPU fallback: every numerical step is a kernel from smaug_aux_kernels.cuh and the stage
+// kernels smaug_split_kernel.cuh / smaug_flux_kernel.cuh / smaug_line_kernel.cuh (second implementations:
+// smaug_stage_kernel.cuh, smaug_march_kernel.cuh).
 #include "../../include/smaug.h"
 
 #include <algorithm>
