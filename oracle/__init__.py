@@ -16,13 +16,17 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "smaug_oracle.cpp")
 _LIB = os.path.join(_HERE, "liboracle_smaug.so")
+_SRC3 = os.path.join(_HERE, "smaug3d_oracle.cpp")       # the 3-D form: a separate library (no shared code)
+_LIB3 = os.path.join(_HERE, "liboracle_smaug3d.so")
 
 BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2
 (P_LX, P_LY, P_HD_ON, P_C_RHO, P_C_MOM, P_C_E, P_C_B, P_RK_ORDER, P_FIXED_DT) = range(9)
 P_GX, P_GY = 10, 11
+P_LZ, P_GZ = 13, 14
 ENONFINITE = -4
 
 _lib = None
+_lib3 = None
 
 
 def _cpu_has_fma() -> bool:
@@ -33,15 +37,20 @@ def _cpu_has_fma() -> bool:
         return False
 
 
-def build(force: bool = False) -> str:
-    """Compile liboracle_smaug.so next to its source if missing or stale; return its path."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+def _compile(src: str, out: str, force: bool) -> str:
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(src):
         cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared"]
         if _cpu_has_fma():
             cmd.append("-mfma")      # std::fma -> one hardware instruction (same bits as the libm fallback)
-        cmd += ["-o", _LIB, _SRC]
+        cmd += ["-o", out, src]
         subprocess.run(cmd, check=True)
-    return _LIB
+    return out
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle_smaug.so (and the 3-D oracle's library) next to the sources if missing or stale."""
+    _compile(_SRC3, _LIB3, force)
+    return _compile(_SRC, _LIB, force)
 
 
 def lib() -> C.CDLL:
@@ -171,3 +180,102 @@ def central_diff_1d(f_padded, h):
     out = np.empty(n)
     _check(lib().oracle_central_diff_1d(_dp(f), n, float(h), _dp(out)))
     return out
+
+
+# ------------------------------------------------------------------------------------------------ three dimensions
+def lib3() -> C.CDLL:
+    global _lib3
+    if _lib3 is None:
+        L = C.CDLL(_compile(_SRC3, _LIB3, False))
+        dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p
+        L.oracle3_last_error.restype = C.c_char_p
+        L.oracle3_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, ip, C.POINTER(vp)]
+        L.oracle3_destroy.argtypes = [vp]
+        L.oracle3_destroy.restype = None
+        L.oracle3_set_param.argtypes = [vp, C.c_int, C.c_double]
+        L.oracle3_set_threads.argtypes = [vp, C.c_int]
+        L.oracle3_set_state.argtypes = [vp, dp]
+        L.oracle3_get_state.argtypes = [vp, dp]
+        L.oracle3_get_time.argtypes = [vp, dp, dp]
+        L.oracle3_step.argtypes = [vp, C.c_int, C.c_double]
+        L.oracle3_rhs.argtypes = [vp, dp]
+        L.oracle3_wavespeeds.argtypes = [vp, dp]
+        L.oracle3_get_padded.argtypes = [vp, C.c_int, dp]
+        _lib3 = L
+    return _lib3
+
+
+class Oracle3D:
+    """One context of the 3-D oracle (smaug3d_oracle.cpp).  State: numpy float64 [8, nz, ny, nx] =
+    (rho, mx, my, mz, e, bx, by, bz); bc = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi); zero background."""
+
+    _KEYS = dict(lx=P_LX, ly=P_LY, lz=P_LZ, hd_on=P_HD_ON, c_rho=P_C_RHO, c_mom=P_C_MOM, c_e=P_C_E, c_b=P_C_B,
+                 rk_order=P_RK_ORDER, fixed_dt=P_FIXED_DT, gx=P_GX, gy=P_GY, gz=P_GZ)
+
+    def __init__(self, nx, ny, nz, gamma, bc, threads=1, **params):
+        L = lib3()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        h = C.c_void_p()
+        self._chk(L.oracle3_create(self.nx, self.ny, self.nz, float(gamma), (C.c_int * 6)(*[int(b) for b in bc]), C.byref(h)))
+        self._h = h
+        if threads != 1:
+            self._chk(L.oracle3_set_threads(self._h, int(threads)))
+        for k, v in params.items():
+            self.set_param(k, v)
+
+    @staticmethod
+    def _chk(rc):
+        if rc != 0:
+            raise RuntimeError(f"oracle3 error {rc}: {lib3().oracle3_last_error().decode()}")
+
+    @property
+    def shape(self):
+        return (8, self.nz, self.ny, self.nx)
+
+    def set_param(self, key, value):
+        k = self._KEYS[key] if isinstance(key, str) else int(key)
+        self._chk(lib3().oracle3_set_param(self._h, k, float(value)))
+
+    def set_state(self, w):
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        assert w.shape == self.shape
+        self._chk(lib3().oracle3_set_state(self._h, _dp(w)))
+
+    def get_state(self):
+        w = np.empty(self.shape)
+        self._chk(lib3().oracle3_get_state(self._h, _dp(w)))
+        return w
+
+    def step(self, n_steps, cfl=0.3):
+        self._chk(lib3().oracle3_step(self._h, int(n_steps), float(cfl)))
+
+    def time(self):
+        t, dt = C.c_double(), C.c_double()
+        self._chk(lib3().oracle3_get_time(self._h, C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def rhs(self):
+        r = np.empty(self.shape)
+        self._chk(lib3().oracle3_rhs(self._h, _dp(r)))
+        return r
+
+    def wavespeeds(self):
+        o = np.empty(5)
+        self._chk(lib3().oracle3_wavespeeds(self._h, _dp(o)))
+        return o
+
+    def padded(self, f):
+        o = np.empty((self.nz + 6, self.ny + 6, self.nx + 6))
+        self._chk(lib3().oracle3_get_padded(self._h, int(f), _dp(o)))
+        return o
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib3().oracle3_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

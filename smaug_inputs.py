@@ -146,3 +146,101 @@ def rel_l2(a: np.ndarray, ref: np.ndarray) -> np.ndarray:
     den = np.sqrt((ref ** 2).reshape(ref.shape[0], -1).sum(1))
     fallback = den.max() if den.max() > 0 else 1.0
     return num / np.where(den > 0, den, fallback)
+
+
+# ------------------------------------------------------------------------------------------------ three dimensions
+# State [8, nz, ny, nx] = (rho, mx, my, mz, e, bx, by, bz); bc = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi).
+FIELDS3 = ("rho", "mx", "my", "mz", "e", "bx", "by", "bz")
+
+
+def prim_to_cons3(rho, v, p, b, gamma: float) -> np.ndarray:
+    rho, vx, vy, vz, p, bx, by, bz = np.broadcast_arrays(rho, v[0], v[1], v[2], p, b[0], b[1], b[2])
+    e = p / (gamma - 1.0) + 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * (bx * bx + by * by + bz * bz)
+    return np.ascontiguousarray(np.stack([rho, rho * vx, rho * vy, rho * vz, e, bx, by, bz]).astype(np.float64))
+
+
+def grid3(nx: int, ny: int, nz: int, lengths=(1.0, 1.0, 1.0)):
+    x = centres(nx, lengths[0])[None, None, :]
+    y = centres(ny, lengths[1])[None, :, None]
+    z = centres(nz, lengths[2])[:, None, None]
+    return x, y, z
+
+
+def orszag_tang_3d(nx: int, ny: int | None = None, nz: int | None = None, gamma: float = 5.0 / 3.0, eps: float = 0.2):
+    """A three-dimensional Orszag-Tang-like vortex (the paper prints no 3-D configuration; this recipe is ours, DESIGN.md
+    section 9): the BASELINE.json Orszag-Tang state modulated along z, plus a z-flow and a z-field,
+      rho = 25/(36 pi), p = 5/(12 pi), m(z) = 1 + eps sin 2 pi z,
+      v = (-m sin 2 pi y, m sin 2 pi x, eps sin 2 pi z),  B = (-m sin 2 pi y, m sin 4 pi x, eps sin 2 pi x) / sqrt(4 pi)
+    (every component of B is independent of its own coordinate: div B = 0), periodic.  Returns (w[8,nz,ny,nx], bc, gamma)."""
+    ny = nx if ny is None else ny
+    nz = nx if nz is None else nz
+    x, y, z = grid3(nx, ny, nz)
+    one = np.ones((nz, ny, nx))
+    rho = 25.0 / (36.0 * np.pi) * one
+    p = 5.0 / (12.0 * np.pi) * one
+    b0 = 1.0 / np.sqrt(4.0 * np.pi)
+    m = 1.0 + eps * np.sin(2 * np.pi * z)
+    v = (-m * np.sin(2 * np.pi * y) * one, m * np.sin(2 * np.pi * x) * one, eps * np.sin(2 * np.pi * z) * one)
+    b = (-b0 * m * np.sin(2 * np.pi * y) * one, b0 * m * np.sin(4 * np.pi * x) * one, b0 * eps * np.sin(2 * np.pi * x) * one)
+    return prim_to_cons3(rho, v, p, b, gamma), (BC_PERIODIC,) * 6, gamma
+
+
+def smooth_random_3d(nx: int, ny: int, nz: int, seed: int = 1710, kmax: int = 2, amp: float = 1e-2,
+                     gamma: float = 5.0 / 3.0, lengths=(1.0, 1.0, 1.0)):
+    """Periodic random smooth 3-D state: the Orszag-Tang mean (rho, p), mean field (0.2, 0.1, -0.15), plus Fourier modes
+    |k| <= kmax of relative amplitude `amp` on each of the eight primitive variables.  Returns (w, bc, gamma)."""
+    rng = np.random.default_rng(seed)
+    x, y, z = grid3(nx, ny, nz, lengths)
+
+    def field(scale):
+        f = np.zeros((nz, ny, nx))
+        norm = 0.0
+        for kx in range(-kmax, kmax + 1):
+            for ky in range(-kmax, kmax + 1):
+                for kz in range(0, kmax + 1):
+                    if kx * kx + ky * ky + kz * kz > kmax * kmax or (kx == 0 and ky == 0 and kz == 0):
+                        continue
+                    a, ph = rng.normal(), rng.uniform(0, 2 * np.pi)
+                    f += a * np.cos(2 * np.pi * (kx * x / lengths[0] + ky * y / lengths[1] + kz * z / lengths[2]) + ph)
+                    norm += abs(a)
+        return scale * amp * f / norm
+
+    rho0, p0 = 25.0 / (36.0 * np.pi), 5.0 / (12.0 * np.pi)
+    rho = rho0 + field(rho0)
+    p = p0 + field(p0)
+    v = (field(1.0), field(1.0), field(1.0))
+    b = (0.2 + field(1.0), 0.1 + field(1.0), -0.15 + field(1.0))
+    return prim_to_cons3(rho, v, p, b, gamma), (BC_PERIODIC,) * 6, gamma
+
+
+def extrude_2d(w2: np.ndarray, nz: int) -> np.ndarray:
+    """A 2-D state [6, ny, nx] as the z-invariant 3-D state [8, nz, ny, nx] with mz = bz = 0."""
+    _, ny, nx = w2.shape
+    w3 = np.zeros((8, nz, ny, nx))
+    for f3, f2 in ((0, 0), (1, 1), (2, 2), (4, 3), (5, 4), (6, 5)):
+        w3[f3] = w2[f2][None, :, :]
+    return w3
+
+
+_SWAPS = {      # axis swap -> (transpose of [f, z, y, x], field order)
+    "xy": ((0, 1, 3, 2), (0, 2, 1, 3, 4, 6, 5, 7)),
+    "xz": ((0, 3, 2, 1), (0, 3, 2, 1, 4, 7, 6, 5)),
+    "yz": ((0, 2, 1, 3), (0, 1, 3, 2, 4, 5, 7, 6)),
+}
+
+
+def swap_axes_3d(w: np.ndarray, which: str) -> np.ndarray:
+    """The mirrored problem with two axes (and the matching vector components) exchanged; which = 'xy', 'xz' or 'yz'."""
+    tr, order = _SWAPS[which]
+    return np.ascontiguousarray(np.transpose(w, tr)[list(order)])
+
+
+def swap_triple(t, which: str):
+    """Exchange the entries of a per-axis triple (x, y, z) -- or of the six per-side boundary kinds -- the same way."""
+    a, b = "xyz".index(which[0]), "xyz".index(which[1])
+    t = list(t)
+    if len(t) == 3:
+        t[a], t[b] = t[b], t[a]
+    else:
+        t[2 * a:2 * a + 2], t[2 * b:2 * b + 2] = t[2 * b:2 * b + 2], t[2 * a:2 * a + 2]
+    return tuple(t)
