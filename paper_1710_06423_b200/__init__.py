@@ -31,13 +31,13 @@ def _sources():
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/smaug.cu for sm_100a into libsmaug.so (in-tree) if missing or stale."""
-    newest = max(os.path.getmtime(p) for p in _sources() + [os.path.join(INCLUDE, "smaug.h")])
+    """Compile csrc/smaug.cu and csrc/smaug3d.cu for sm_100a into libsmaug.so (in-tree) if missing or stale."""
+    newest = max(os.path.getmtime(p) for p in _sources() + [os.path.join(INCLUDE, "smaug.h"), os.path.join(INCLUDE, "smaug3d.h")])
     if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         extra = os.environ.get("SMAUG_NVCC_EXTRA", "").split()     # e.g. -DSMAUG_TW=24 for tuning sweeps
         cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu")]
+              ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu"), os.path.join(_CSRC, "smaug3d.cu")]
         subprocess.run(cmd, check=True)
     return LIB_PATH
 
@@ -96,6 +96,21 @@ def lib() -> C.CDLL:
         L.smaug_group_destroy.argtypes = [vp]
         L.smaug_group_destroy.restype = None
         L.smaug_group_map_cell.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, ip, C.c_int, C.c_int, C.c_int, C.c_int, ip]
+        L.smaug3_last_error.restype = C.c_char_p
+        L.smaug3_workspace_bytes.restype = C.c_size_t
+        L.smaug3_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.smaug3_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, ip, vp, C.POINTER(vp)]
+        L.smaug3_destroy.argtypes = [vp]
+        L.smaug3_destroy.restype = None
+        L.smaug3_set_param.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug3_set_state.argtypes = [vp, vp]
+        L.smaug3_step.argtypes = [vp, C.c_int, C.c_double]
+        L.smaug3_get_state.argtypes = [vp, vp]
+        L.smaug3_get_time.argtypes = [vp, dp, dp]
+        L.smaug3_get_wavespeeds.argtypes = [vp, dp]
+        L.smaug3_get_launch_count.argtypes = [vp, C.POINTER(C.c_longlong)]
+        L.smaug3_set_kernel_timing.argtypes = [vp, C.c_int]
+        L.smaug3_get_kernel_timing.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         _lib = L
     return _lib
 
@@ -285,6 +300,99 @@ class SmaugGroup:
     def close(self):
         if getattr(self, "_h", None):
             lib().smaug_group_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # noqa: BLE001
+            pass
+
+
+PARAMS3 = dict(lx=0, ly=1, hd_on=2, c_rho=3, c_mom=4, c_e=5, c_b=6, rk_order=7, fixed_dt=8, gx=10, gy=11, lz=13, gz=14)
+KERNEL_KINDS3 = ("ghost fill + dt", "derived quantities", "kappa / interface fluxes", "cell-centred fluxes", "assembly")
+
+
+class Smaug3DError(RuntimeError):
+    def __init__(self, code: int):
+        self.code = code
+        super().__init__(f"smaug3 error {code}: {lib().smaug3_last_error().decode()}")
+
+
+def _check3(rc: int) -> None:
+    if rc != 0:
+        raise Smaug3DError(rc)
+
+
+class Smaug3D:
+    """One 3-D context: smaug3_create / set_state / step / get_state / destroy (include/smaug3d.h).  State: float64
+    ``[8, nz, ny, nx]`` = (rho, mx, my, mz, e, bx, by, bz), torch (cuda or cpu) tensors or numpy arrays; the library owns
+    its device memory; work is enqueued on torch's current stream of ``device`` at construction time."""
+
+    def __init__(self, nx, ny, nz, gamma, bc, device="cuda:0", **params):
+        import torch
+        L = lib()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+            h = C.c_void_p()
+            _check3(L.smaug3_create(self.nx, self.ny, self.nz, float(gamma), (C.c_int * 6)(*[int(b) for b in bc]),
+                                    C.c_void_p(stream), C.byref(h)))
+        self._h = h
+        for k, v in params.items():
+            self.set_param(k, v)
+
+    @property
+    def shape(self):
+        return (8, self.nz, self.ny, self.nx)
+
+    def set_param(self, key, value):
+        k = PARAMS3[key] if isinstance(key, str) else int(key)
+        _check3(lib().smaug3_set_param(self._h, k, float(value)))
+
+    def set_state(self, w):
+        assert tuple(w.shape) == self.shape
+        _check3(lib().smaug3_set_state(self._h, _ptr(w)))
+
+    def step(self, n_steps, cfl=0.3):
+        _check3(lib().smaug3_step(self._h, int(n_steps), float(cfl)))
+
+    def get_state(self, out=None):
+        import torch
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        assert tuple(out.shape) == self.shape
+        _check3(lib().smaug3_get_state(self._h, _ptr(out)))
+        return out
+
+    def time(self):
+        t, dt = C.c_double(), C.c_double()
+        _check3(lib().smaug3_get_time(self._h, C.byref(t), C.byref(dt)))
+        return t.value, dt.value
+
+    def wavespeeds(self):
+        o = (C.c_double * 5)()
+        _check3(lib().smaug3_get_wavespeeds(self._h, o))
+        return list(o)
+
+    def launch_count(self):
+        n = C.c_longlong()
+        _check3(lib().smaug3_get_launch_count(self._h, C.byref(n)))
+        return n.value
+
+    def set_kernel_timing(self, on=True):
+        _check3(lib().smaug3_set_kernel_timing(self._h, int(on)))
+
+    def kernel_timing(self):
+        """{kind: (milliseconds, launches)} accumulated since set_kernel_timing(True)."""
+        ms, n = (C.c_double * 5)(), (C.c_longlong * 5)()
+        _check3(lib().smaug3_get_kernel_timing(self._h, ms, n))
+        return {k: (ms[i], n[i]) for i, k in enumerate(KERNEL_KINDS3)}
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().smaug3_destroy(self._h)
             self._h = None
 
     def __del__(self):

@@ -1,0 +1,863 @@
+// smaug3d.cu -- the three-dimensional form of the SMAUG+ hot path on B200 (C ABI in
+// include/smaug3d.h).  fp64, sm_100a, -fmad=false: the arithmetic contract of DESIGN.md section 4 holds (every
+// formula is the explicit IEEE operation sequence the 3-D oracle documents; results are bit-identical to it).
+// Product code: shares nothing with oracle/.
+//
+// First 3-D form: an RK stage is a short sequence of streaming kernels over padded volumes in HBM,
+//   ghost3_kernel     ghost cells of the stage input, six sides, edges and corners by composing the three maps (c-8)
+//   derive3_kernel    v = m (1/rho), eps on every padded cell (c-2)
+//   kappa3_kernel<d>  per interface along d: the seven hyperviscosity ratios (c-5) and the interface fluxes Phi_d of
+//                     all fields; keeps kappa_d(v_k), kappa_d(b_k), k != d, for the mixed terms
+//   cflux3_kernel<k>  per cell: C_k = F_k - G_k (c-2 fluxes minus the mixed fluxes of c-5 / c-11)
+//   assemble3_kernel  per cell: R = -sum_k d^c_k C_k + gravity + sum_d (Phi_d+ - Phi_d-)/Delta_d, the RK combine in
+//                     the epilogue, the store, and the wave-speed maxima of the written state (warp shuffles, one
+//                     atomicMax pass per CTA)
+// thread per cell, x fastest (coalesced), stencil neighbours through L1/L2.  dt, t and the maxima stay on the
+// device; one host synchronisation per smaug3_step call.  DESIGN.md section 5 has the byte counts and what a fused
+// 2.5-D march (the 2-D kernel's design carried to 3-D) would save.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/smaug3d.h"
+#include "smaug_device.cuh"
+
+namespace smaug3 {
+
+using smaug::ddiv;
+using smaug::drcp;
+using smaug::kappa_ratio;
+using smaug::NG;
+using smaug::XOFF;
+
+constexpr int NF = 8;
+enum { F_RHO = 0, F_MX = 1, F_MY = 2, F_MZ = 3, F_E = 4, F_BX = 5, F_BY = 6, F_BZ = 7 };
+enum { BC_PERIODIC = 0, BC_OPEN = 1, BC_FIXED = 2 };
+enum { COMBINE_BASE = 0, COMBINE_ACC = 1, COMBINE_FINAL = 2 };
+enum { WS_VT = 1, WS_FULL = 2 };
+constexpr int NRED = 5;       // reduction sets
+constexpr int NDER = 4;       // vx, vy, vz, eps
+constexpr int NPHI = 7;       // Phi_d / C_d components: rho, mx, my, mz, e, b_l1, b_l2 (l1 < l2, both != d)
+constexpr int NKM = 4;        // kappa_d(v_k1), kappa_d(v_k2), kappa_d(b_k1), kappa_d(b_k2), k1 < k2, both != d
+
+// Padded volume: (nz + 6) planes of (ny + 6) rows of `pitch` doubles; interior cell (i, j, k) at
+// ((k + 3)(ny + 6) + (j + 3)) pitch + i + 16 (interior column 0 is 128-byte aligned).
+struct Grid3 {
+  int n[3];
+  int pitch, rows;          // rows = ny + 6
+  long long plane, vol;     // doubles per plane / per volume
+  int bc[6];
+};
+__host__ __device__ inline long long addr3(const Grid3& g, int i, int j, int k) {
+  return ((long long)(k + NG) * g.rows + (j + NG)) * g.pitch + (i + XOFF);
+}
+__host__ __device__ inline long long stride3(const Grid3& g, int d) { return d == 0 ? 1 : (d == 1 ? g.pitch : g.plane); }
+
+struct V8 { double* p[NF]; };
+struct CV8 { const double* p[NF]; };
+struct V7 { double* p[NPHI]; };
+struct CV7 { const double* p[NPHI]; };
+struct V4 { double* p[4]; };
+struct CV4 { const double* p[4]; };
+
+struct Scalars3 {
+  unsigned long long red[NRED][5];      // {cmax_x, cmax_y, cmax_z, max a^2, max b^2} as fp64 bit patterns (>= 0)
+  double dt, t;
+  int status, pad;
+};
+
+struct Params3 {
+  double gamma;
+  double inv_d[3];
+  double c_rho, c_mom, c_e, c_b;
+  double g[3];
+  int grav_on;
+};
+
+__device__ __forceinline__ double dabs(double x) { return __hiloint2double(__double2hiint(x) & 0x7fffffff, __double2loint(x)); }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double cd12v(double m2, double m1, double p1, double p2) { return fma(8.0, p1 - m1, -(p2 - m2)); }
+__device__ __forceinline__ double cd12p(const double* f, long long s) { return fma(8.0, f[s] - f[-s], -(f[2 * s] - f[-2 * s])); }
+
+// kappa at the interface between p[0] and p[s] from the six cells p[-2s .. 3s] (c-5); d_mid = p[s] - p[0]
+__device__ __forceinline__ double kappa_at(const double* p, long long s, double cv, double& d_mid, double& lo, double& hi) {
+  const double u0 = p[-2 * s], u1 = p[-s], u2 = p[0], u3 = p[s], u4 = p[2 * s], u5 = p[3 * s];
+  const double a0 = u1 - u0, a1 = u2 - u1, a2 = u3 - u2, a3 = u4 - u3, a4 = u5 - u4;
+  const double t0 = dabs(fma(3.0, a1, -(u3 - u0)));
+  const double t1 = dabs(fma(3.0, a2, -(u4 - u1)));
+  const double t2 = dabs(fma(3.0, a3, -(u5 - u2)));
+  const double m3 = dmax(dmax(t0, t1), t2);
+  const double m1 = dmax(dmax(dmax(dabs(a0), dabs(a1)), dmax(dabs(a2), dabs(a3))), dabs(a4));
+  d_mid = a2;
+  lo = u2;
+  hi = u3;
+  return kappa_ratio(m3, m1, cv);
+}
+
+__device__ __forceinline__ int wrap_idx(int i, int n) {
+  int r = i % n;
+  return r < 0 ? r + n : r;
+}
+
+// ------------------------------------------------------------------------------------------------ ghost fill (c-8)
+// The oracle fills x over interior (j, k), then y over the padded x-extent, then z over the padded x- and y-extents.
+// Composed: a ghost cell takes the cell reached by mapping z, then y, then x (periodic: wrap, open: clamp); a FIXED
+// side is never rewritten -- if the outermost out-of-range axis (z before y before x) is fixed the cell is skipped,
+// and a fixed axis met later stops the mapping (the source is then a frozen ghost).  freeze: fixed acts like open
+// (set_state).  Reads interior cells or frozen ghosts, writes other ghosts: no race within the launch.
+__global__ void __launch_bounds__(128) ghost3_kernel(Grid3 g, V8 w, int freeze) {
+  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - NG;
+  const int j = (int)blockIdx.y - NG, k = (int)blockIdx.z - NG;
+  if (i >= g.n[0] + NG) return;
+  int c[3] = {i, j, k};
+  if (c[0] >= 0 && c[0] < g.n[0] && c[1] >= 0 && c[1] < g.n[1] && c[2] >= 0 && c[2] < g.n[2]) return;
+  bool first = true;
+#pragma unroll
+  for (int a = 2; a >= 0; --a) {
+    if (c[a] >= 0 && c[a] < g.n[a]) continue;
+    const int kind = g.bc[2 * a + (c[a] < 0 ? 0 : 1)];
+    if (kind == BC_FIXED && !freeze) {
+      if (first) return;
+      break;
+    }
+    c[a] = kind == BC_PERIODIC ? wrap_idx(c[a], g.n[a]) : (c[a] < 0 ? 0 : g.n[a] - 1);
+    first = false;
+  }
+  const long long dst = addr3(g, i, j, k), src = addr3(g, c[0], c[1], c[2]);
+#pragma unroll
+  for (int f = 0; f < NF; ++f) w.p[f][dst] = w.p[f][src];
+}
+
+// ------------------------------------------------------------------------------------------------ derived (c-2)
+__global__ void __launch_bounds__(128) derive3_kernel(Grid3 g, CV8 w, V4 der) {
+  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - NG;
+  if (i >= g.n[0] + NG) return;
+  const long long q = addr3(g, i, (int)blockIdx.y - NG, (int)blockIdx.z - NG);
+  const double rr = drcp(w.p[F_RHO][q]);
+  const double mx = w.p[F_MX][q], my = w.p[F_MY][q], mz = w.p[F_MZ][q];
+  const double vx = mx * rr, vy = my * rr, vz = mz * rr;
+  const double bx = w.p[F_BX][q], by = w.p[F_BY][q], bz = w.p[F_BZ][q];
+  const double b2h = 0.5 * fma(bz, bz, fma(by, by, bx * bx));
+  const double ke = 0.5 * fma(mz, vz, fma(my, vy, mx * vx));
+  der.p[0][q] = vx; der.p[1][q] = vy; der.p[2][q] = vz;
+  der.p[3][q] = (w.p[F_E][q] - ke) - b2h;
+}
+
+// ------------------------------------------------------------------------------------------------ kappa, Phi (c-5)
+// One thread per interface (cell q | cell q + stride(D)); interfaces -1 .. n-1 along D, cells [-2, n+2) across it
+// (the mixed terms read kappa there).  Phi = g kappa (q_b - q_a); energy: Phi(eps) + sum_l vbar_l Phi(m_l)
+// + sum_{l != D} Bbar_l Phi(b_l), l ascending, v before B (c-11).
+template <int D>
+__global__ void __launch_bounds__(128) kappa3_kernel(Grid3 g, Params3 prm, CV8 w, CV4 der, const Scalars3* sc, int red_in,
+                                                     V7 phi, V4 km) {
+  constexpr int A1 = D == 0 ? 1 : 0, A2 = D == 2 ? 1 : 2;          // the two axes across D, ascending
+  int c[3];
+  c[0] = (int)(blockIdx.x * blockDim.x + threadIdx.x) + (D == 0 ? -1 : -2);
+  c[1] = (int)blockIdx.y + (D == 1 ? -1 : -2);
+  c[2] = (int)blockIdx.z + (D == 2 ? -1 : -2);
+  if (c[0] >= (D == 0 ? g.n[0] : g.n[0] + 2)) return;
+  const long long q = addr3(g, c[0], c[1], c[2]);
+  const long long s = stride3(g, D);
+  const double vt = sqrt(__longlong_as_double((long long)sc->red[red_in][3])) +
+                    sqrt(__longlong_as_double((long long)sc->red[red_in][4]));
+  const double cv_rho = prm.c_rho * vt, cv_mom = prm.c_mom * vt, cv_e = prm.c_e * vt, cv_b = prm.c_b * vt;
+  double d, lo, hi;
+  const double k_rho = kappa_at(w.p[F_RHO] + q, s, cv_rho, d, lo, hi);
+  const double rbar = 0.5 * (lo + hi);
+  phi.p[0][q] = k_rho * d;
+  const double k_e = kappa_at(der.p[3] + q, s, cv_e, d, lo, hi);
+  double e = k_e * d;
+  double kv[3];
+#pragma unroll
+  for (int l = 0; l < 3; ++l) {
+    kv[l] = kappa_at(der.p[l] + q, s, cv_mom, d, lo, hi);
+    const double gl = l == D ? rbar : 0.5 * rbar;
+    const double pm = (gl * kv[l]) * d;
+    phi.p[1 + l][q] = pm;
+    e = fma(0.5 * (lo + hi), pm, e);
+  }
+  km.p[0][q] = kv[A1];
+  km.p[1][q] = kv[A2];
+  {
+    const double kb = kappa_at(w.p[F_BX + A1] + q, s, cv_b, d, lo, hi);
+    const double pb = kb * d;
+    phi.p[5][q] = pb;
+    km.p[2][q] = kb;
+    e = fma(0.5 * (lo + hi), pb, e);
+  }
+  {
+    const double kb = kappa_at(w.p[F_BX + A2] + q, s, cv_b, d, lo, hi);
+    const double pb = kb * d;
+    phi.p[6][q] = pb;
+    km.p[3][q] = kb;
+    e = fma(0.5 * (lo + hi), pb, e);
+  }
+  phi.p[4][q] = e;
+}
+
+// ------------------------------------------------------------------------------------------------ C_k = F_k - G_k
+// One thread per cell, [-2, n+2) along K, interior across it.  F: c-2.  G (hyperdiffusion on): for each
+// l != K ascending, G(m_l; K) = (rho/2) kbar_l(v_K) d^c_l v_K, G(b_l; K) = - kbar_l(b_K) d^c_l b_K,
+// G(e; K) = sum_l v_l G(m_l; K) + b_l G(b_l; K) (c-11).  kmA / kmB: the kappa arrays of directions l1 < l2.
+template <int K, bool HD>
+__global__ void __launch_bounds__(128) cflux3_kernel(Grid3 g, Params3 prm, CV8 w, CV4 der, CV4 kmA, CV4 kmB, V7 cf) {
+  constexpr int L1 = K == 0 ? 1 : 0, L2 = K == 2 ? 1 : 2;
+  int c[3];
+  c[0] = (int)(blockIdx.x * blockDim.x + threadIdx.x) + (K == 0 ? -2 : 0);
+  c[1] = (int)blockIdx.y + (K == 1 ? -2 : 0);
+  c[2] = (int)blockIdx.z + (K == 2 ? -2 : 0);
+  if (c[0] >= (K == 0 ? g.n[0] + 2 : g.n[0])) return;
+  const long long q = addr3(g, c[0], c[1], c[2]);
+  const double rho = w.p[F_RHO][q];
+  const double m[3] = {w.p[F_MX][q], w.p[F_MY][q], w.p[F_MZ][q]};
+  const double b[3] = {w.p[F_BX][q], w.p[F_BY][q], w.p[F_BZ][q]};
+  const double v[3] = {der.p[0][q], der.p[1][q], der.p[2][q]};
+  const double eps = der.p[3][q];
+  const double b2h = 0.5 * fma(b[2], b[2], fma(b[1], b[1], b[0] * b[0]));
+  const double ptt = fma(prm.gamma - 1.0, eps, b2h);
+  const double bv = fma(b[2], v[2], fma(b[1], v[1], b[0] * v[0]));
+  const double h = w.p[F_E][q] + ptt;
+  double F[NPHI];
+  F[0] = rho * v[K];
+#pragma unroll
+  for (int l = 0; l < 3; ++l) {
+    const double f = fma(m[l], v[K], -(b[l] * b[K]));
+    F[1 + l] = l == K ? f + ptt : f;
+  }
+  F[4] = fma(v[K], h, -(b[K] * bv));
+  F[5] = fma(v[K], b[L1], -(b[K] * v[L1]));
+  F[6] = fma(v[K], b[L2], -(b[K] * v[L2]));
+  if (HD) {
+    // position of component K among the stored kappa components of direction l: K - (K > l)
+    constexpr int P1 = K - (K > L1 ? 1 : 0), P2 = K - (K > L2 ? 1 : 0);
+    const long long s1 = stride3(g, L1), s2 = stride3(g, L2);
+    const double kbv1 = 0.5 * (kmA.p[P1][q - s1] + kmA.p[P1][q]);
+    const double kbb1 = 0.5 * (kmA.p[2 + P1][q - s1] + kmA.p[2 + P1][q]);
+    const double dv1 = cd12p(der.p[K] + q, s1) * (1.0 / 12.0);
+    const double db1 = cd12p(w.p[F_BX + K] + q, s1) * (1.0 / 12.0);
+    const double gm1 = ((0.5 * rho) * kbv1) * dv1;
+    const double gb1 = -(kbb1 * db1);
+    const double kbv2 = 0.5 * (kmB.p[P2][q - s2] + kmB.p[P2][q]);
+    const double kbb2 = 0.5 * (kmB.p[2 + P2][q - s2] + kmB.p[2 + P2][q]);
+    const double dv2 = cd12p(der.p[K] + q, s2) * (1.0 / 12.0);
+    const double db2 = cd12p(w.p[F_BX + K] + q, s2) * (1.0 / 12.0);
+    const double gm2 = ((0.5 * rho) * kbv2) * dv2;
+    const double gb2 = -(kbb2 * db2);
+    double ge = fma(v[L1], gm1, b[L1] * gb1);
+    ge = fma(b[L2], gb2, fma(v[L2], gm2, ge));
+    F[1 + L1] = F[1 + L1] - gm1;
+    F[1 + L2] = F[1 + L2] - gm2;
+    F[4] = F[4] - ge;
+    F[5] = F[5] - gb1;
+    F[6] = F[6] - gb2;
+  }
+#pragma unroll
+  for (int f = 0; f < NPHI; ++f) cf.p[f][q] = F[f];
+}
+
+// ------------------------------------------------------------------------------------------------ assembly
+struct AsmArgs {
+  Grid3 g;
+  Params3 prm;
+  CV7 cf[3], phi[3];
+  CV4 der;
+  CV8 in, base, acc_in;
+  V8 out, acc_out;
+  Scalars3* sc;
+  int red_out;
+  double c;
+};
+
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double t = __shfl_xor_sync(0xffffffffu, v, o);
+    v = t > v ? t : v;
+  }
+  return v;
+}
+
+// slot of field component `l` of b (or the marker -1 for l == d) inside the 7-component C_d / Phi_d arrays
+__host__ __device__ constexpr int bslot(int l, int d) { return l == d ? -1 : 5 + l - (l > d ? 1 : 0); }
+
+template <int COMBINE, int WS, bool HD>
+__global__ void __launch_bounds__(128) assemble3_kernel(const AsmArgs a) {
+  __shared__ double sh[5 * 4];
+  const Grid3& g = a.g;
+  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+  double wsm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (i < g.n[0]) {
+    const long long q = addr3(g, i, (int)blockIdx.y, (int)blockIdx.z);
+    const long long st[3] = {1, g.pitch, g.plane};
+    double R[NF];
+    // -(1/12) sum_d cd12(C_d) / Delta_d, nested x outermost: fma(cd_x, 1/dx, fma(cd_y, 1/dy, cd_z (1/dz)))
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      double cd[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const int slot = f < F_BX ? f : bslot(f - F_BX, d);
+        cd[d] = slot < 0 ? 0.0 : cd12p(a.cf[d].p[slot] + q, st[d]);
+      }
+      R[f] = fma(cd[0], a.prm.inv_d[0], fma(cd[1], a.prm.inv_d[1], cd[2] * a.prm.inv_d[2])) * (-1.0 / 12.0);
+    }
+    if (a.prm.grav_on) {
+      const double rt = a.in.p[F_RHO][q];
+      const double gv = fma(a.prm.g[2], a.der.p[2][q], fma(a.prm.g[1], a.der.p[1][q], a.prm.g[0] * a.der.p[0][q]));
+#pragma unroll
+      for (int l = 0; l < 3; ++l) R[F_MX + l] = fma(rt, a.prm.g[l], R[F_MX + l]);
+      R[F_E] = fma(rt, gv, R[F_E]);
+    }
+    if (HD) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          const int slot = f < F_BX ? f : bslot(f - F_BX, d);
+          const double diff = slot < 0 ? 0.0 : a.phi[d].p[slot][q] - a.phi[d].p[slot][q - st[d]];
+          R[f] = fma(diff, a.prm.inv_d[d], R[f]);
+        }
+      }
+    }
+    const double cdt = a.c * a.sc->dt;
+    double o[NF];
+    if (COMBINE == COMBINE_FINAL) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const double w3 = a.in.p[f][q];
+        o[f] = fma(cdt, R[f], fma(fma(-2.0, w3, a.acc_in.p[f][q]), 1.0 / 3.0, w3));
+      }
+    } else {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const double wb = a.base.p[f][q];
+        o[f] = fma(cdt, R[f], wb);
+        if (COMBINE == COMBINE_ACC) a.acc_out.p[f][q] = fma(2.0, o[f], a.in.p[f][q] - wb);
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < NF; ++f) a.out.p[f][q] = o[f];
+    // wave speeds of the written cell (c-4)
+    const double rr = drcp(o[F_RHO]);
+    const double vx = o[F_MX] * rr, vy = o[F_MY] * rr, vz = o[F_MZ] * rr;
+    const double B2 = fma(o[F_BZ], o[F_BZ], fma(o[F_BY], o[F_BY], o[F_BX] * o[F_BX]));
+    const double pk = (a.prm.gamma - 1.0) * ((o[F_E] - 0.5 * fma(o[F_MZ], vz, fma(o[F_MY], vy, o[F_MX] * vx))) - 0.5 * B2);
+    const double a2 = (a.prm.gamma * pk) * rr;
+    const double b2 = B2 * rr;
+    wsm[3] = a2 > 0.0 ? a2 : 0.0;
+    wsm[4] = b2 > 0.0 ? b2 : 0.0;
+    if (WS == WS_FULL) {
+      const double s = a2 + b2;
+      const double fa = (4.0 * a2) * rr;
+      const double vv[3] = {vx, vy, vz};
+      const double bb[3] = {o[F_BX], o[F_BY], o[F_BZ]};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        const double disc = fma(s, s, -(fa * (bb[d] * bb[d])));
+        const double cf2 = 0.5 * (s + sqrt(disc > 0.0 ? disc : 0.0));
+        const double cc = fabs(vv[d]) + sqrt(cf2);
+        wsm[d] = cc > 0.0 ? cc : 0.0;
+      }
+    }
+  }
+  // block maximum (warp shuffles), one atomicMax per value and CTA; NaNs never enter (x > 0 ? x : 0)
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  constexpr int FROM = WS == WS_FULL ? 0 : 3;
+#pragma unroll
+  for (int k = FROM; k < 5; ++k) {
+    const double m = warp_max(wsm[k]);
+    if (lane == 0) sh[k * 4 + wid] = m;
+  }
+  __syncthreads();
+  if (threadIdx.x < 5 && (int)threadIdx.x >= FROM) {
+    const int k = threadIdx.x;
+    double m = sh[k * 4];
+    for (int w2 = 1; w2 < 4; ++w2) m = sh[k * 4 + w2] > m ? sh[k * 4 + w2] : m;
+    atomicMax(&a.sc->red[a.red_out][k], (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+// standalone reduction of all five maxima over the interior (set_state)
+__global__ void __launch_bounds__(128) wavespeed3_kernel(Grid3 g, CV8 w, double gamma, Scalars3* sc, int set) {
+  __shared__ double sh[5 * 4];
+  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+  double wsm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (i < g.n[0]) {
+    const long long q = addr3(g, i, (int)blockIdx.y, (int)blockIdx.z);
+    const double rr = drcp(w.p[F_RHO][q]);
+    const double mx = w.p[F_MX][q], my = w.p[F_MY][q], mz = w.p[F_MZ][q];
+    const double vv[3] = {mx * rr, my * rr, mz * rr};
+    const double bb[3] = {w.p[F_BX][q], w.p[F_BY][q], w.p[F_BZ][q]};
+    const double B2 = fma(bb[2], bb[2], fma(bb[1], bb[1], bb[0] * bb[0]));
+    const double pk = (gamma - 1.0) * ((w.p[F_E][q] - 0.5 * fma(mz, vv[2], fma(my, vv[1], mx * vv[0]))) - 0.5 * B2);
+    const double a2 = (gamma * pk) * rr;
+    const double b2 = B2 * rr;
+    wsm[3] = a2 > 0.0 ? a2 : 0.0;
+    wsm[4] = b2 > 0.0 ? b2 : 0.0;
+    const double s = a2 + b2;
+    const double fa = (4.0 * a2) * rr;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double disc = fma(s, s, -(fa * (bb[d] * bb[d])));
+      const double cf2 = 0.5 * (s + sqrt(disc > 0.0 ? disc : 0.0));
+      const double cc = fabs(vv[d]) + sqrt(cf2);
+      wsm[d] = cc > 0.0 ? cc : 0.0;
+    }
+  }
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const double m = warp_max(wsm[k]);
+    if (lane == 0) sh[k * 4 + wid] = m;
+  }
+  __syncthreads();
+  if (threadIdx.x < 5) {
+    const int k = threadIdx.x;
+    double m = sh[k * 4];
+    for (int w2 = 1; w2 < 4; ++w2) m = sh[k * 4 + w2] > m ? sh[k * 4 + w2] : m;
+    atomicMax(&sc->red[set][k], (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+// dt = cfl min_d (Delta_d / cmax_d) over the axes with n > 1 (c-7), t += dt, status, and the reduction sets of the coming
+// step cleared; one thread
+__global__ void dt3_kernel(Scalars3* s, int state_set, unsigned clear_sets, double cfl, double fixed_dt, double dx, double dy,
+                           double dz, int nx, int ny, int nz) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double dt = fixed_dt;
+  if (!(fixed_dt > 0.0)) {
+    double m = __longlong_as_double(0x7ff0000000000000LL);
+    if (nx > 1) m = fmin(m, dx / __longlong_as_double((long long)s->red[state_set][0]));
+    if (ny > 1) m = fmin(m, dy / __longlong_as_double((long long)s->red[state_set][1]));
+    if (nz > 1) m = fmin(m, dz / __longlong_as_double((long long)s->red[state_set][2]));
+    dt = cfl * m;
+  }
+  if (!(dt > 0.0) || isinf(dt) || isnan(dt)) s->status = 1;
+  s->dt = dt;
+  s->t += dt;
+  for (int k = 0; k < NRED; ++k)
+    if (clear_sets & (1u << k))
+      for (int v = 0; v < 5; ++v) s->red[k][v] = 0ULL;
+}
+
+// flat [8][nz][ny][nx] <-> padded interior
+__global__ void __launch_bounds__(128) pack3_kernel(Grid3 g, const double* flat, V8 w, int to_flat, double* flat_out) {
+  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+  if (i >= g.n[0]) return;
+  const int j = blockIdx.y, k = blockIdx.z;
+  const long long q = addr3(g, i, j, k);
+  const long long nvol = (long long)g.n[0] * g.n[1] * g.n[2];
+  const long long o = ((long long)k * g.n[1] + j) * g.n[0] + i;
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    if (to_flat) flat_out[f * nvol + o] = w.p[f][q];
+    else w.p[f][q] = flat[f * nvol + o];
+  }
+}
+
+// ================================================================================================ host side
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+#define CUDA_TRY(x)                                                                                  \
+  do {                                                                                               \
+    cudaError_t e_ = (x);                                                                            \
+    if (e_ != cudaSuccess) return fail(SMAUG3_ECUDA, std::string(#x) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+struct Ctx {
+  Grid3 g;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  double gamma = 0;
+  double L[3] = {1.0, 1.0, 1.0};
+  int hd_on = 1, rk_order = 4;
+  double c_rho = 0.02, c_mom = 0.4, c_e = 0.02, c_b = 0.02, fixed_dt = 0.0;
+  double grav[3] = {0.0, 0.0, 0.0};
+  double* mem = nullptr;        // one allocation: all volumes
+  V8 buf[4];                    // w^n / state, w1 -> w3, w2, accumulator
+  V4 der;
+  V7 phi[3], cf[3];
+  V4 km[3];
+  Scalars3* sc = nullptr;
+  int cur = 0;                  // reduction set holding the maxima of the state (0 or 4)
+  long long launches = 0;
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;
+  std::vector<int> ev_kind;
+  size_t ev_used = 0;
+  double ms[5] = {0, 0, 0, 0, 0};
+  long long nk[5] = {0, 0, 0, 0, 0};
+};
+
+constexpr int NVOL = 4 * NF + NDER + 3 * (NPHI + NPHI + NKM);      // 32 + 4 + 54 = 90 padded volumes
+
+int make_grid(int nx, int ny, int nz, const int bc[6], Grid3& g) {
+  g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+  g.pitch = (XOFF + nx + NG + 15) / 16 * 16;
+  g.rows = ny + 2 * NG;
+  g.plane = (long long)g.pitch * g.rows;
+  g.vol = g.plane * (nz + 2 * NG);
+  for (int s = 0; s < 6; ++s) g.bc[s] = bc ? bc[s] : 0;
+  return 0;
+}
+
+template <class T>
+CV8 cv8(const T& v) { CV8 c; for (int f = 0; f < NF; ++f) c.p[f] = v.p[f]; return c; }
+CV7 cv7(const V7& v) { CV7 c; for (int f = 0; f < NPHI; ++f) c.p[f] = v.p[f]; return c; }
+CV4 cv4(const V4& v) { CV4 c; for (int f = 0; f < 4; ++f) c.p[f] = v.p[f]; return c; }
+
+Params3 params(const Ctx& c) {
+  Params3 p;
+  p.gamma = c.gamma;
+  for (int d = 0; d < 3; ++d) { p.inv_d[d] = c.g.n[d] / c.L[d]; p.g[d] = c.grav[d]; }
+  p.c_rho = c.c_rho; p.c_mom = c.c_mom; p.c_e = c.c_e; p.c_b = c.c_b;
+  p.grav_on = c.grav[0] != 0.0 || c.grav[1] != 0.0 || c.grav[2] != 0.0;
+  return p;
+}
+
+// event bracket around one launch when timing is on
+struct Timed {
+  Ctx& c;
+  int kind;
+  Timed(Ctx& c_, int kind_) : c(c_), kind(kind_) {
+    ++c.launches;
+    if (c.timing) mark();
+  }
+  ~Timed() {
+    if (c.timing) mark();
+  }
+  void mark() {
+    if (c.ev_used == c.ev.size()) {
+      cudaEvent_t e;
+      cudaEventCreate(&e);
+      c.ev.push_back(e);
+      c.ev_kind.push_back(kind);
+    }
+    c.ev_kind[c.ev_used] = kind;
+    cudaEventRecord(c.ev[c.ev_used++], c.stream);
+  }
+};
+
+dim3 grid_for(int nxr, int nyr, int nzr) { return dim3((unsigned)((nxr + 127) / 128), (unsigned)nyr, (unsigned)nzr); }
+
+void launch_ghost(Ctx& c, V8 w, int freeze) {
+  Timed t(c, 0);
+  const Grid3& g = c.g;
+  ghost3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, w, freeze);
+}
+
+template <int D>
+void launch_kappa(Ctx& c, const Params3& p, const V8& in, int red_in) {
+  Timed t(c, 2);
+  const Grid3& g = c.g;
+  const int r[3] = {D == 0 ? g.n[0] + 1 : g.n[0] + 4, D == 1 ? g.n[1] + 1 : g.n[1] + 4, D == 2 ? g.n[2] + 1 : g.n[2] + 4};
+  kappa3_kernel<D><<<grid_for(r[0], r[1], r[2]), 128, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), c.sc, red_in, c.phi[D], c.km[D]);
+}
+
+template <int K>
+void launch_cflux(Ctx& c, const Params3& p, const V8& in) {
+  Timed t(c, 3);
+  const Grid3& g = c.g;
+  constexpr int L1 = K == 0 ? 1 : 0, L2 = K == 2 ? 1 : 2;
+  const int r[3] = {K == 0 ? g.n[0] + 4 : g.n[0], K == 1 ? g.n[1] + 4 : g.n[1], K == 2 ? g.n[2] + 4 : g.n[2]};
+  if (c.hd_on)
+    cflux3_kernel<K, true><<<grid_for(r[0], r[1], r[2]), 128, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), cv4(c.km[L1]), cv4(c.km[L2]), c.cf[K]);
+  else
+    cflux3_kernel<K, false><<<grid_for(r[0], r[1], r[2]), 128, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), cv4(c.km[L1]), cv4(c.km[L2]), c.cf[K]);
+}
+
+template <int COMBINE, int WS>
+void launch_assemble(Ctx& c, const AsmArgs& a) {
+  Timed t(c, 4);
+  const Grid3& g = c.g;
+  const dim3 gr = grid_for(g.n[0], g.n[1], g.n[2]);
+  if (c.hd_on) assemble3_kernel<COMBINE, WS, true><<<gr, 128, 0, c.stream>>>(a);
+  else assemble3_kernel<COMBINE, WS, false><<<gr, 128, 0, c.stream>>>(a);
+}
+
+// one RK stage: out = combine(in, R(in)); the maxima of `in` are in set red_in, those of `out` go to red_out
+void stage(Ctx& c, int in, int base, int out, int combine, int ws, double coef, int red_in, int red_out) {
+  const Params3 p = params(c);
+  launch_ghost(c, c.buf[in], 0);
+  {
+    Timed t(c, 1);
+    const Grid3& g = c.g;
+    derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[in]), c.der);
+  }
+  if (c.hd_on) {
+    launch_kappa<0>(c, p, c.buf[in], red_in);
+    launch_kappa<1>(c, p, c.buf[in], red_in);
+    launch_kappa<2>(c, p, c.buf[in], red_in);
+  }
+  launch_cflux<0>(c, p, c.buf[in]);
+  launch_cflux<1>(c, p, c.buf[in]);
+  launch_cflux<2>(c, p, c.buf[in]);
+  AsmArgs a;
+  a.g = c.g;
+  a.prm = p;
+  for (int d = 0; d < 3; ++d) { a.cf[d] = cv7(c.cf[d]); a.phi[d] = cv7(c.phi[d]); }
+  a.der = cv4(c.der);
+  a.in = cv8(c.buf[in]);
+  a.base = cv8(c.buf[base]);
+  a.acc_in = cv8(c.buf[3]);
+  a.out = c.buf[out];
+  a.acc_out = c.buf[3];
+  a.sc = c.sc;
+  a.red_out = red_out;
+  a.c = coef;
+  if (combine == COMBINE_BASE && ws == WS_VT) launch_assemble<COMBINE_BASE, WS_VT>(c, a);
+  else if (combine == COMBINE_BASE) launch_assemble<COMBINE_BASE, WS_FULL>(c, a);
+  else if (combine == COMBINE_ACC) launch_assemble<COMBINE_ACC, WS_VT>(c, a);
+  else launch_assemble<COMBINE_FINAL, WS_FULL>(c, a);
+}
+
+void enqueue_step(Ctx& c, double cfl) {
+  const int cur = c.cur, nxt = cur == 0 ? 4 : 0;
+  {
+    Timed t(c, 0);
+    dt3_kernel<<<1, 32, 0, c.stream>>>(c.sc, cur, (1u << 1) | (1u << 2) | (1u << 3) | (1u << nxt), cfl, c.fixed_dt,
+                                       c.L[0] / c.g.n[0], c.L[1] / c.g.n[1], c.L[2] / c.g.n[2], c.g.n[0], c.g.n[1], c.g.n[2]);
+  }
+  if (c.rk_order == 1) {
+    // Euler: w^{n+1} = w^n + dt R(w^n) written into buffer 1, then the buffers swap roles
+    stage(c, 0, 0, 1, COMBINE_BASE, WS_FULL, 1.0, cur, nxt);
+    std::swap(c.buf[0], c.buf[1]);
+  } else if (c.rk_order == 2) {
+    stage(c, 0, 0, 1, COMBINE_BASE, WS_VT, 0.5, cur, 1);
+    stage(c, 1, 0, 2, COMBINE_BASE, WS_FULL, 1.0, 1, nxt);
+    std::swap(c.buf[0], c.buf[2]);
+  } else {
+    stage(c, 0, 0, 1, COMBINE_BASE, WS_VT, 0.5, cur, 1);
+    stage(c, 1, 0, 2, COMBINE_ACC, WS_VT, 0.5, 1, 2);
+    stage(c, 2, 0, 1, COMBINE_BASE, WS_VT, 1.0, 2, 3);
+    stage(c, 1, 0, 0, COMBINE_FINAL, WS_FULL, 1.0 / 6.0, 3, nxt);
+  }
+  c.cur = nxt;
+}
+
+}  // namespace smaug3
+
+using namespace smaug3;
+#define CTX(p) (reinterpret_cast<smaug3::Ctx*>(p))
+
+extern "C" {
+
+const char* smaug3_last_error(void) { return g_err.c_str(); }
+
+size_t smaug3_workspace_bytes(int nx, int ny, int nz) {
+  if (nx < 1 || ny < 1 || nz < 1) return 0;
+  Grid3 g;
+  make_grid(nx, ny, nz, nullptr, g);
+  return (size_t)g.vol * NVOL * sizeof(double) + 4096;
+}
+
+int smaug3_create(int nx, int ny, int nz, double gamma, const int bc[6], void* stream, smaug3_ctx** out) {
+  if (!out || !bc) return fail(SMAUG3_EINVAL, "NULL argument");
+  *out = nullptr;
+  if (nx < 1 || ny < 1 || nz < 1) return fail(SMAUG3_EINVAL, "nx, ny, nz must be >= 1");
+  if (!(gamma > 1.0)) return fail(SMAUG3_EINVAL, "gamma must be > 1");
+  for (int s = 0; s < 6; ++s)
+    if (bc[s] < 0 || bc[s] > 2) return fail(SMAUG3_EINVAL, "unknown boundary kind");
+  for (int a = 0; a < 3; ++a)
+    if ((bc[2 * a] == BC_PERIODIC) != (bc[2 * a + 1] == BC_PERIODIC))
+      return fail(SMAUG3_EINVAL, "periodic must be set on both sides of an axis");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(SMAUG3_ECUDA, "no CUDA device: libsmaug has no CPU fallback");
+  }
+  Ctx* c = new Ctx();
+  make_grid(nx, ny, nz, bc, c->g);
+  if (c->g.vol >= (1LL << 31)) { delete c; return fail(SMAUG3_EINVAL, "a padded volume must have fewer than 2^31 elements"); }
+  if (nz + 6 > 65535 || ny + 6 > 65535) { delete c; return fail(SMAUG3_EINVAL, "ny, nz must be below 65529"); }
+  c->gamma = gamma;
+  c->stream = (cudaStream_t)stream;
+  if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return fail(SMAUG3_ECUDA, "cudaGetDevice failed"); }
+  const size_t bytes = (size_t)c->g.vol * NVOL * sizeof(double) + 4096;
+  if (cudaMalloc(&c->mem, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    delete c;
+    return fail(SMAUG3_ENOMEM, "device allocation of " + std::to_string(bytes) + " bytes failed");
+  }
+  cudaMemsetAsync(c->mem, 0, bytes, c->stream);
+  double* p = c->mem;
+  auto take = [&]() { double* r = p; p += c->g.vol; return r; };
+  for (int b = 0; b < 4; ++b)
+    for (int f = 0; f < NF; ++f) c->buf[b].p[f] = take();
+  for (int f = 0; f < NDER; ++f) c->der.p[f] = take();
+  for (int d = 0; d < 3; ++d) {
+    for (int f = 0; f < NPHI; ++f) c->phi[d].p[f] = take();
+    for (int f = 0; f < NPHI; ++f) c->cf[d].p[f] = take();
+    for (int f = 0; f < NKM; ++f) c->km[d].p[f] = take();
+  }
+  c->sc = reinterpret_cast<Scalars3*>(p);
+  *out = reinterpret_cast<smaug3_ctx*>(c);
+  return SMAUG3_OK;
+}
+
+void smaug3_destroy(smaug3_ctx* ctx) {
+  if (!ctx) return;
+  Ctx* c = CTX(ctx);
+  DeviceGuard guard_(c->device);
+  cudaStreamSynchronize(c->stream);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  cudaFree(c->mem);
+  delete c;
+}
+
+int smaug3_set_param(smaug3_ctx* ctx, int key, double v) {
+  if (!ctx) return fail(SMAUG3_EINVAL, "NULL ctx");
+  Ctx& c = *CTX(ctx);
+  switch (key) {
+    case SMAUG3_PARAM_LX: if (!(v > 0)) break; c.L[0] = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_LY: if (!(v > 0)) break; c.L[1] = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_LZ: if (!(v > 0)) break; c.L[2] = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_HD_ON: c.hd_on = v != 0.0; return SMAUG3_OK;
+    case SMAUG3_PARAM_C_RHO: if (!(v >= 0)) break; c.c_rho = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_C_MOM: if (!(v >= 0)) break; c.c_mom = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_C_E: if (!(v >= 0)) break; c.c_e = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_C_B: if (!(v >= 0)) break; c.c_b = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_RK_ORDER: if (v != 1 && v != 2 && v != 4) break; c.rk_order = (int)v; return SMAUG3_OK;
+    case SMAUG3_PARAM_FIXED_DT: if (!(v >= 0)) break; c.fixed_dt = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_GX: if (!std::isfinite(v)) break; c.grav[0] = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_GY: if (!std::isfinite(v)) break; c.grav[1] = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_GZ: if (!std::isfinite(v)) break; c.grav[2] = v; return SMAUG3_OK;
+    default: return fail(SMAUG3_EINVAL, "unknown parameter key");
+  }
+  return fail(SMAUG3_EINVAL, "parameter value out of range");
+}
+
+int smaug3_set_state(smaug3_ctx* ctx, const void* w) {
+  if (!ctx || !w) return fail(SMAUG3_EINVAL, "NULL argument");
+  Ctx& c = *CTX(ctx);
+  DeviceGuard guard_(c.device);
+  const Grid3& g = c.g;
+  const size_t nflat = (size_t)NF * g.n[0] * g.n[1] * g.n[2];
+  double* staging = c.cf[0].p[0];        // the C_d volumes (21 of them, contiguous with Phi / kappa) are free between steps
+  // the staging area must hold 8 flat volumes: cf[0] .. are contiguous allocations of padded volumes >= flat ones
+  CUDA_TRY(cudaMemcpyAsync(staging, w, nflat * sizeof(double), cudaMemcpyDefault, c.stream));
+  const dim3 gi = grid_for(g.n[0], g.n[1], g.n[2]);
+  pack3_kernel<<<gi, 128, 0, c.stream>>>(g, staging, c.buf[0], 0, nullptr);
+  ++c.launches;
+  launch_ghost(c, c.buf[0], 1);
+  // the other two buffers that are read with a halo get the same frozen ghosts (fixed sides are never rewritten)
+  for (int b = 1; b <= 2; ++b)
+    for (int f = 0; f < NF; ++f)
+      CUDA_TRY(cudaMemcpyAsync(c.buf[b].p[f], c.buf[0].p[f], (size_t)g.vol * sizeof(double), cudaMemcpyDeviceToDevice, c.stream));
+  CUDA_TRY(cudaMemsetAsync(c.sc, 0, sizeof(Scalars3), c.stream));
+  c.cur = 0;
+  wavespeed3_kernel<<<gi, 128, 0, c.stream>>>(g, cv8(c.buf[0]), c.gamma, c.sc, 0);
+  ++c.launches;
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaStreamSynchronize(c.stream));
+  return SMAUG3_OK;
+}
+
+int smaug3_step(smaug3_ctx* ctx, int n_steps, double cfl) {
+  if (!ctx || n_steps < 0) return fail(SMAUG3_EINVAL, "bad argument");
+  Ctx& c = *CTX(ctx);
+  if (c.fixed_dt <= 0.0 && !(cfl > 0.0)) return fail(SMAUG3_EINVAL, "cfl must be > 0");
+  DeviceGuard guard_(c.device);
+  for (int s = 0; s < n_steps; ++s) enqueue_step(c, cfl);
+  CUDA_TRY(cudaGetLastError());
+  Scalars3 h;
+  CUDA_TRY(cudaMemcpyAsync(&h, c.sc, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+  CUDA_TRY(cudaStreamSynchronize(c.stream));
+  if (h.status) return fail(SMAUG3_ENONFINITE, "non-finite or non-positive dt");
+  return SMAUG3_OK;
+}
+
+int smaug3_get_state(smaug3_ctx* ctx, void* w) {
+  if (!ctx || !w) return fail(SMAUG3_EINVAL, "NULL argument");
+  Ctx& c = *CTX(ctx);
+  DeviceGuard guard_(c.device);
+  const Grid3& g = c.g;
+  const size_t nflat = (size_t)NF * g.n[0] * g.n[1] * g.n[2];
+  double* staging = c.cf[0].p[0];
+  pack3_kernel<<<grid_for(g.n[0], g.n[1], g.n[2]), 128, 0, c.stream>>>(g, nullptr, c.buf[0], 1, staging);
+  ++c.launches;
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaMemcpyAsync(w, staging, nflat * sizeof(double), cudaMemcpyDefault, c.stream));
+  CUDA_TRY(cudaStreamSynchronize(c.stream));
+  return SMAUG3_OK;
+}
+
+int smaug3_get_time(smaug3_ctx* ctx, double* t, double* last_dt) {
+  if (!ctx) return fail(SMAUG3_EINVAL, "NULL ctx");
+  Ctx& c = *CTX(ctx);
+  DeviceGuard guard_(c.device);
+  Scalars3 h;
+  CUDA_TRY(cudaMemcpyAsync(&h, c.sc, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+  CUDA_TRY(cudaStreamSynchronize(c.stream));
+  if (t) *t = h.t;
+  if (last_dt) *last_dt = h.dt;
+  return SMAUG3_OK;
+}
+
+int smaug3_get_wavespeeds(smaug3_ctx* ctx, double out[5]) {
+  if (!ctx || !out) return fail(SMAUG3_EINVAL, "NULL argument");
+  Ctx& c = *CTX(ctx);
+  DeviceGuard guard_(c.device);
+  Scalars3 h;
+  CUDA_TRY(cudaMemcpyAsync(&h, c.sc, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+  CUDA_TRY(cudaStreamSynchronize(c.stream));
+  for (int k = 0; k < 5; ++k) {
+    const unsigned long long u = h.red[c.cur][k];
+    double d;
+    memcpy(&d, &u, sizeof(d));
+    out[k] = d;
+  }
+  return SMAUG3_OK;
+}
+
+int smaug3_get_launch_count(smaug3_ctx* ctx, long long* n) {
+  if (!ctx || !n) return fail(SMAUG3_EINVAL, "NULL argument");
+  *n = CTX(ctx)->launches;
+  return SMAUG3_OK;
+}
+
+int smaug3_set_kernel_timing(smaug3_ctx* ctx, int on) {
+  if (!ctx) return fail(SMAUG3_EINVAL, "NULL ctx");
+  Ctx& c = *CTX(ctx);
+  c.timing = on != 0;
+  c.ev_used = 0;
+  for (int k = 0; k < 5; ++k) { c.ms[k] = 0; c.nk[k] = 0; }
+  return SMAUG3_OK;
+}
+
+int smaug3_get_kernel_timing(smaug3_ctx* ctx, double ms[5], long long n[5]) {
+  if (!ctx || !ms || !n) return fail(SMAUG3_EINVAL, "NULL argument");
+  Ctx& c = *CTX(ctx);
+  DeviceGuard guard_(c.device);
+  CUDA_TRY(cudaStreamSynchronize(c.stream));
+  for (size_t e = 0; e + 1 < c.ev_used; e += 2) {
+    float t = 0;
+    CUDA_TRY(cudaEventElapsedTime(&t, c.ev[e], c.ev[e + 1]));
+    c.ms[c.ev_kind[e]] += t;
+    c.nk[c.ev_kind[e]] += 1;
+  }
+  c.ev_used = 0;
+  for (int k = 0; k < 5; ++k) { ms[k] = c.ms[k]; n[k] = c.nk[k]; }
+  return SMAUG3_OK;
+}
+
+}  // extern "C"

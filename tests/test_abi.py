@@ -26,6 +26,31 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(L, s), s
 
 
+def test_library_exports_every_symbol_of_the_3d_header():
+    src = open(os.path.join(ROOT, "include", "smaug3d.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    syms = sorted(set(re.findall(r"\b(smaug3_[a-z_]+)\s*\(", src)))
+    L = C.CDLL(pkg.build())
+    assert len(syms) >= 12 and "smaug3_step" in syms
+    for s in syms:
+        assert hasattr(L, s), s
+    L = pkg.lib()
+    h = C.c_void_p()
+    bc = (C.c_int * 6)(0, 0, 0, 0, 0, 0)
+    assert L.smaug3_workspace_bytes(0, 4, 4) == 0
+    assert 14e9 < L.smaug3_workspace_bytes(256, 256, 256) < 14.5e9          # 90 padded volumes of 288 x 262 x 262 doubles
+    assert L.smaug3_create(0, 4, 4, 1.4, bc, None, C.byref(h)) == pkg.EINVAL
+    assert L.smaug3_create(4, 4, 4, 1.0, bc, None, C.byref(h)) == pkg.EINVAL
+    assert L.smaug3_create(4, 4, 4, 1.4, (C.c_int * 6)(0, 0, 0, 0, 0, 1), None, C.byref(h)) == pkg.EINVAL
+    assert L.smaug3_create(4, 4, 4, 1.4, bc, None, None) == pkg.EINVAL
+    assert L.smaug3_step(None, 1, 0.3) == pkg.EINVAL and b"bad" in L.smaug3_last_error()
+    L.smaug3_destroy(None)
+    import torch
+    if not torch.cuda.is_available():
+        assert L.smaug3_create(8, 8, 8, 1.4, bc, None, C.byref(h)) == pkg.ECUDA and not h.value
+        assert b"no CPU fallback" in L.smaug3_last_error()
+
+
 def test_workspace_bytes_and_argument_validation():
     L = pkg.lib()
     assert L.smaug_workspace_bytes(0, 4, 0) == 0
