@@ -43,6 +43,11 @@ WORKLOADS = {
     # SURVEY 8(d) extra row: the 8000^2 Orszag-Tang state as a perturbation on a uniform non-zero background
     # (exercises the background loads and the energy source) -- split_kernel<128, .., BG>
     "orszag_tang_8000_bg": (8000, 8000, "otbg"),
+    # the three-dimensional form (include/smaug3d.h): a 3-D Orszag-Tang-like vortex, eight fields,
+    # periodic, hyperdiffusion on, RK4 (smaug_inputs.orszag_tang_3d; the paper prints no 3-D configuration)
+    "orszag_tang_3d_128": (128, 128, "ot3d"),
+    "orszag_tang_3d_256": (256, 256, "ot3d"),
+    "orszag_tang_3d_384": (384, 384, "ot3d"),
 }
 # Algorithmic HBM bytes per cell-update of the fused step as built: per stage the
 # kernel reads the 6 input planes once and writes 6; stages 2-3 also read w^n; stage 2 also writes the
@@ -330,6 +335,94 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_3d(args):
+    """A 3-D workload: same JSON line; a step = dt + 4 x {ghost fill, derived quantities, kappa /
+    interface fluxes along x, y, z, cell-centred fluxes along x, y, z, assembly + RK combine + reduction}.  The roofline
+    entry is taken over the whole stage (the nine launches together) against what a fully fused stage must move:
+    8 fields x 8 B x (4 reads with halo + 4 writes + 2 x w^n + accumulator written once and read once) = 768 B per
+    cell-update, 192 B per cell and stage."""
+    import torch
+    import paper_1710_06423_b200 as pkg
+    pkg.lib()
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py: the 3-D rows are single-GPU rows")
+    torch.cuda.set_device(0)
+    name = args.workload
+    n = WORKLOADS[name][0]
+    w_np, bc, gamma = si.orszag_tang_3d(n)
+    w_host = torch.from_numpy(w_np).pin_memory()
+    out_host = torch.empty_like(w_host).pin_memory()
+    del w_np
+    sim = pkg.Smaug3D(n, n, n, gamma, bc, hd_on=0 if args.no_hd else 1, rk_order=args.rk_order)
+    sim.set_state(w_host)
+    K, W = args.steps, args.warmup
+    sim.step(W, 0.3)
+    sim.set_kernel_timing(True)
+    sampler = ClockSampler(0)
+    launches0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    sim.step(K, 0.3)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launch_count() - launches0
+    kinds = sim.kernel_timing()
+    sim.set_kernel_timing(False)
+    t_sim, dt_last = sim.time()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    sim.set_state(w_host)
+    sim.step(K, 0.3)
+    sim.get_state(out_host)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    finite = bool(torch.isfinite(out_host[:, ::7, ::5, ::3]).all())
+    cells = float(n) ** 3
+    stages = {4: 4, 2: 2}[args.rk_order]
+    bpcu = {4: 768.0, 2: 320.0}[args.rk_order]
+    peak, peak_src = peaks()
+    stage_ms = sum(v[0] for v in kinds.values()) / (K * stages)
+    achieved = bpcu / stages * cells / (stage_ms * 1e-3) / 1e9
+    top = max(kinds, key=lambda k: kinds[k][0])
+    line = {
+        "metric": METRIC, "value": cells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": name, "nx": n, "ny": n, "nz": n, "fields": 8, "cfl": 0.3, "hd": not args.no_hd,
+                   "rk_order": args.rk_order, "background": "zero", "parallelism": "1 gpu",
+                   "l2": "working set >> L2, no flush needed" if cells * 64 > 4e8 else "working set comparable to L2 (126 MB)"},
+        "hbm_gbs_algorithmic": cells * K / (ms * 1e-3) * bpcu / 1e9,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src,
+                     "kernel": "smaug3 RK stage (9 launches: ghost3, derive3, 3 x kappa3, 3 x cflux3, assemble3); "
+                               f"largest share: {top}",
+                     "bytes_per_launch": bpcu / stages * cells, "avg_launch_ms": stage_ms,
+                     "launches_timed": int(sum(v[1] for v in kinds.values())),
+                     "stage_kernel_share_of_step": sum(v[0] for v in kinds.values()) / ms,
+                     "ms_per_stage_by_kind": {k: v[0] / (K * stages) for k, v in kinds.items()}},
+        "e2e": {"value": cells * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 64 * cells / K, "d2h_bytes_per_step": 64 * cells / K,
+                "note": "smaug3_set_state(host) + smaug3_step(K) + smaug3_get_state(host), pinned host memory"},
+        "gpu_launches": launches, "clocks": clocks, "sim": {"t": t_sim, "last_dt": dt_last, "finite": finite},
+    }
+    if not args.no_cpu_baseline:
+        import oracle
+        ns, steps_s = 64, 3
+        w, bc, gamma = si.orszag_tang_3d(ns)
+        o = oracle.Oracle3D(ns, ns, ns, gamma, bc, hd_on=0 if args.no_hd else 1, rk_order=args.rk_order)
+        o.set_state(w)
+        t0 = time.perf_counter()
+        o.step(steps_s, 0.3)
+        el = time.perf_counter() - t0
+        o.close()
+        line["cpu_baseline"] = {"value": ns ** 3 * steps_s / el, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"3-D oracle on the same vortex at {ns}^3, {steps_s} steps, {el:.1f} s, 1 of {os.cpu_count()} host cores"}
+    print(json.dumps(line), flush=True)
+    sim.close()
+
+
 def run_decomp(args):
     """--decomp PXxPY: the decomposed run of the workload on one device beside the unsplit run of the same steps
     (the decomposition's own cost: exchange kernels, barriers between the members' streams, smaller launches)."""
@@ -400,6 +493,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif WORKLOADS[args.workload][2] == "ot3d":
+        run_3d(args)
     elif args.decomp:
         run_decomp(args)
     else:
