@@ -154,6 +154,13 @@ int smaug_get_kernel_timing(smaug_ctx* ctx, double* stage_ms, long long* stage_l
  * kappa_ratio (or its fast path, taken only when every M1 of the warp is >= 2^-923).  Runs on the current device. */
 int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, long long draws, unsigned long long out[5]);
 
+/* fp64-pipe micro-benchmark on the current device (the measurement behind DESIGN.md section 5's "one fp64 warp instruction
+ * per two cycles and SM sub-partition, dependent latency 9 cycles"): every warp of a grid of one CTA per SM with
+ * 128 * warps_per_subpartition threads runs `iters` trips of `ilp` (1, 2, 4 or 8) independent dependent-DFMA chains.
+ * out[0] = clock cycles per warp instruction and sub-partition, out[1] = cycles per trip (the chain latency while the
+ * pipe is not saturated).  Errors: EINVAL, ECUDA.  tests/test_gpu_division.py prints and bounds both. */
+int smaug_selftest_fp64_pipe(int ilp, int warps_per_subpartition, int iters, double out[2]);
+
 void smaug_destroy(smaug_ctx* ctx); /* NULL is a no-op */
 
 /* ---- Domain decomposition (SURVEY.md 8(f) NEXT-1; PAPER.md:25 Fig. 1, :55-59 "the full domain is divided into

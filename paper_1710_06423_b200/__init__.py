@@ -81,6 +81,7 @@ def lib() -> C.CDLL:
         L.smaug_get_kernel_timing.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
         L.smaug_selftest_division.argtypes = [C.c_int, C.c_int, C.c_ulonglong, C.c_longlong,
                                               C.POINTER(C.c_ulonglong)]
+        L.smaug_selftest_fp64_pipe.argtypes = [C.c_int, C.c_int, C.c_int, dp]
         L.smaug_destroy.argtypes = [vp]
         L.smaug_destroy.restype = None
         ip = C.POINTER(C.c_int)
@@ -142,6 +143,13 @@ def selftest_division(exp_lo: int, exp_hi: int, seed: int = 1, draws: int = 1 <<
     o = (C.c_ulonglong * 5)()
     _check(lib().smaug_selftest_division(int(exp_lo), int(exp_hi), int(seed), int(draws), o))
     return dict(ddiv=o[0], drcp=o[1], ratio_div=o[2], kappa_ratio=o[3], draws=o[4])
+
+
+def selftest_fp64_pipe(ilp: int, warps_per_subpartition: int, iters: int = 2048):
+    """smaug_selftest_fp64_pipe: (cycles per fp64 warp instruction and sub-partition, cycles per trip of the chains)."""
+    o = (C.c_double * 2)()
+    _check(lib().smaug_selftest_fp64_pipe(int(ilp), int(warps_per_subpartition), int(iters), o))
+    return o[0], o[1]
 
 
 class Smaug:

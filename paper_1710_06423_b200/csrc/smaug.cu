@@ -975,6 +975,40 @@ int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, lon
   return SMAUG_OK;
 }
 
+int smaug_selftest_fp64_pipe(int ilp, int warps_per_subpartition, int iters, double out[2]) {
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  if ((ilp != 1 && ilp != 2 && ilp != 4 && ilp != 8) || warps_per_subpartition < 1 || warps_per_subpartition > 8 || iters < 1)
+    return fail(SMAUG_EINVAL, "ilp must be 1, 2, 4 or 8; warps per sub-partition 1..8; iters >= 1");
+  int ndev = 0, dev = 0, n_sm = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(SMAUG_ECUDA, "no CUDA device: libsmaug has no CPU fallback");
+  }
+  CU(cudaGetDevice(&dev));
+  CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  long long* d = nullptr;
+  CU(cudaMalloc((void**)&d, 2 * sizeof(long long)));
+  cudaError_t e = cudaMemset(d, 0, 2 * sizeof(long long));
+  const int threads = 128 * warps_per_subpartition;
+  for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) {      // the second launch is the measurement
+    switch (ilp) {
+      case 1: fp64_pipe_selftest_kernel<1><<<n_sm, threads>>>(iters, 1.25, d); break;
+      case 2: fp64_pipe_selftest_kernel<2><<<n_sm, threads>>>(iters, 1.25, d); break;
+      case 4: fp64_pipe_selftest_kernel<4><<<n_sm, threads>>>(iters, 1.25, d); break;
+      default: fp64_pipe_selftest_kernel<8><<<n_sm, threads>>>(iters, 1.25, d); break;
+    }
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  }
+  long long h[2] = {0, 0};
+  if (e == cudaSuccess) e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(SMAUG_ECUDA, std::string("fp64 pipe self-test: ") + cudaGetErrorString(e));
+  out[0] = (double)h[0] / ((double)iters * ilp * warps_per_subpartition);   // cycles per warp instruction and sub-partition
+  out[1] = (double)h[0] / (double)iters;                                    // cycles per trip (= chain latency when not pipe-bound)
+  return SMAUG_OK;
+}
+
 }  // extern "C"
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -53,4 +53,26 @@ __global__ void division_selftest_kernel(int exp_lo, int exp_hi, unsigned long l
   if (blockIdx.x == 0 && threadIdx.x == 0) counts[4] = (unsigned long long)gridDim.x * blockDim.x * (unsigned long long)draws_per_thread;
 }
 
+// fp64-pipe micro-benchmark behind the numbers DESIGN.md section 5 quotes ("one fp64 warp instruction per two cycles and
+// sub-partition, dependent latency 9 cycles"): every warp runs `iters` trips of ILP independent dependent-DFMA chains;
+// out[0] = clock64 cycles of warp 0 of CTA 0.  The grid is one CTA of 128 * warps_per_subpartition threads per SM.
+template <int ILP>
+__global__ void fp64_pipe_selftest_kernel(int iters, double seed, long long* out) {
+  double x[ILP];
+#pragma unroll
+  for (int i = 0; i < ILP; ++i) x[i] = seed + i + threadIdx.x;
+  __syncthreads();
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < ILP; ++i) x[i] = fma(x[i], 1.0000001, 0.5);
+  }
+  const long long t1 = clock64();
+  double sum = 0.0;
+#pragma unroll
+  for (int i = 0; i < ILP; ++i) sum += x[i];
+  if (threadIdx.x == 0 && blockIdx.x == 0) out[0] = t1 - t0;
+  if (sum == 12345.678) out[1] = 1;      // keeps the chains alive
+}
+
 }  // namespace smaug

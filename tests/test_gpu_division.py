@@ -40,3 +40,21 @@ def test_unguarded_division_is_wrong_below_2_to_minus_960(pkg):
     r = pkg.selftest_division(-1020, -900, seed=3, draws=DRAWS)
     assert r["ddiv"] > 0, r
     assert (r["ratio_div"], r["kappa_ratio"]) == (0, 0), r
+
+
+def test_fp64_pipe_throughput_and_latency(pkg, capsys):
+    """The micro-benchmark behind DESIGN.md section 5 (smaug_selftest_fp64_pipe): a dependent DFMA costs ~9 cycles, the
+    fp64 pipe of an SM sub-partition takes one warp instruction per two cycles (64 lanes per SM), and three warps per
+    scheduler -- what the hot kernel has -- need two independent chains each to fill it."""
+    rows = {}
+    for ilp in (1, 2, 4, 8):
+        for warps in (1, 2, 3, 4):
+            rows[(ilp, warps)] = pkg.selftest_fp64_pipe(ilp, warps)
+    with capsys.disabled():
+        print("\nfp64 pipe: cycles per warp instruction and sub-partition (cycles per trip)")
+        for ilp in (1, 2, 4, 8):
+            print(f"  ILP {ilp}: " + "  ".join(f"{w} warps {rows[(ilp, w)][0]:.2f} ({rows[(ilp, w)][1]:.1f})" for w in (1, 2, 3, 4)))
+    lat = rows[(1, 1)][1]
+    assert 7.0 <= lat <= 11.0, lat                               # dependent-issue latency of DFMA
+    assert 1.9 <= rows[(8, 4)][0] <= 2.2, rows[(8, 4)]           # saturated: one per two cycles
+    assert rows[(1, 3)][0] >= 2.7 and rows[(2, 3)][0] <= 2.4     # three warps: one chain each is not enough, two are
