@@ -42,7 +42,14 @@ enum { WS_VT = 1, WS_FULL = 2 };
 constexpr int NRED = 5;       // reduction sets
 constexpr int NDER = 4;       // vx, vy, vz, eps
 constexpr int NPHI = 7;       // Phi_d / C_d components: rho, mx, my, mz, e, b_l1, b_l2 (l1 < l2, both != d)
-constexpr int NKM = 4;        // kappa_d(v_k1), kappa_d(v_k2), kappa_d(b_k1), kappa_d(b_k2), k1 < k2, both != d
+constexpr int NKM = 4;
+#ifndef SMAUG3_BX
+#define SMAUG3_BX 32      // thread-block shape of the stencil kernels (kappa3, cflux3, assemble3): BX x BY x BZ = 128 threads;
+#define SMAUG3_BY 4       // a block that is several cells thick across x finds part of its y- and z-neighbours in L1
+#define SMAUG3_BZ 1
+#endif
+constexpr int BX = SMAUG3_BX, BY = SMAUG3_BY, BZ = SMAUG3_BZ;
+static_assert(BX * BY * BZ == 128 && BX % 32 == 0, "stencil kernels run 128 threads, whole warps along x");        // kappa_d(v_k1), kappa_d(v_k2), kappa_d(b_k1), kappa_d(b_k2), k1 < k2, both != d
 
 // Padded volume: (nz + 6) planes of (ny + 6) rows of `pitch` doubles; interior cell (i, j, k) at
 // ((k + 3)(ny + 6) + (j + 3)) pitch + i + 16 (interior column 0 is 128-byte aligned).
@@ -109,12 +116,8 @@ __device__ __forceinline__ int wrap_idx(int i, int n) {
 // side is never rewritten -- if the outermost out-of-range axis (z before y before x) is fixed the cell is skipped,
 // and a fixed axis met later stops the mapping (the source is then a frozen ghost).  freeze: fixed acts like open
 // (set_state).  Reads interior cells or frozen ghosts, writes other ghosts: no race within the launch.
-__global__ void __launch_bounds__(128) ghost3_kernel(Grid3 g, V8 w, int freeze) {
-  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - NG;
-  const int j = (int)blockIdx.y - NG, k = (int)blockIdx.z - NG;
-  if (i >= g.n[0] + NG) return;
+__device__ __forceinline__ void ghost_cell(const Grid3& g, const V8& w, int freeze, int i, int j, int k) {
   int c[3] = {i, j, k};
-  if (c[0] >= 0 && c[0] < g.n[0] && c[1] >= 0 && c[1] < g.n[1] && c[2] >= 0 && c[2] < g.n[2]) return;
   bool first = true;
 #pragma unroll
   for (int a = 2; a >= 0; --a) {
@@ -130,6 +133,33 @@ __global__ void __launch_bounds__(128) ghost3_kernel(Grid3 g, V8 w, int freeze) 
   const long long dst = addr3(g, i, j, k), src = addr3(g, c[0], c[1], c[2]);
 #pragma unroll
   for (int f = 0; f < NF; ++f) w.p[f][dst] = w.p[f][src];
+}
+// ghost index 0..5 -> -3, -2, -1, n, n+1, n+2
+__device__ __forceinline__ int ghost_coord(int s, int n) { return s < NG ? s - NG : n + (s - NG); }
+
+// The ghost shell in three launches (only ghost cells get a thread): SLAB 2: the six ghost planes (all i, j);
+// SLAB 1: the six ghost rows of every interior plane (all i); SLAB 0: the six ghost columns of every interior row.
+template <int SLAB>
+__global__ void __launch_bounds__(128) ghost3_kernel(Grid3 g, V8 w, int freeze) {
+  int i, j, k;
+  if (SLAB == 2) {
+    i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - NG;
+    j = (int)blockIdx.y - NG;
+    k = ghost_coord((int)blockIdx.z, g.n[2]);
+    if (i >= g.n[0] + NG) return;
+  } else if (SLAB == 1) {
+    i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - NG;
+    j = ghost_coord((int)blockIdx.y, g.n[1]);
+    k = (int)blockIdx.z;
+    if (i >= g.n[0] + NG) return;
+  } else {
+    const int t = (int)(blockIdx.x * blockDim.x + threadIdx.x);      // 6 ghost columns x ny interior rows of plane k
+    if (t >= 2 * NG * g.n[1]) return;
+    j = t / (2 * NG);
+    i = ghost_coord(t - j * 2 * NG, g.n[0]);
+    k = (int)blockIdx.y;
+  }
+  ghost_cell(g, w, freeze, i, j, k);
 }
 
 // ------------------------------------------------------------------------------------------------ derived (c-2)
@@ -151,30 +181,22 @@ __global__ void __launch_bounds__(128) derive3_kernel(Grid3 g, CV8 w, V4 der) {
 // One thread per interface (cell q | cell q + stride(D)); interfaces -1 .. n-1 along D, cells [-2, n+2) across it
 // (the mixed terms read kappa there).  Phi = g kappa (q_b - q_a); energy: Phi(eps) + sum_l vbar_l Phi(m_l)
 // + sum_{l != D} Bbar_l Phi(b_l), l ascending, v before B (c-11).
+struct KappaCv { double rho, mom, e, b; };
 template <int D>
-__global__ void __launch_bounds__(128) kappa3_kernel(Grid3 g, Params3 prm, CV8 w, CV4 der, const Scalars3* sc, int red_in,
-                                                     V7 phi, V4 km) {
+__device__ __forceinline__ void kappa_dir(const Grid3& g, const KappaCv& cv, const CV8& w, const CV4& der, long long q,
+                                          const V7& phi, const V4& km) {
   constexpr int A1 = D == 0 ? 1 : 0, A2 = D == 2 ? 1 : 2;          // the two axes across D, ascending
-  int c[3];
-  c[0] = (int)(blockIdx.x * blockDim.x + threadIdx.x) + (D == 0 ? -1 : -2);
-  c[1] = (int)blockIdx.y + (D == 1 ? -1 : -2);
-  c[2] = (int)blockIdx.z + (D == 2 ? -1 : -2);
-  if (c[0] >= (D == 0 ? g.n[0] : g.n[0] + 2)) return;
-  const long long q = addr3(g, c[0], c[1], c[2]);
   const long long s = stride3(g, D);
-  const double vt = sqrt(__longlong_as_double((long long)sc->red[red_in][3])) +
-                    sqrt(__longlong_as_double((long long)sc->red[red_in][4]));
-  const double cv_rho = prm.c_rho * vt, cv_mom = prm.c_mom * vt, cv_e = prm.c_e * vt, cv_b = prm.c_b * vt;
   double d, lo, hi;
-  const double k_rho = kappa_at(w.p[F_RHO] + q, s, cv_rho, d, lo, hi);
+  const double k_rho = kappa_at(w.p[F_RHO] + q, s, cv.rho, d, lo, hi);
   const double rbar = 0.5 * (lo + hi);
   phi.p[0][q] = k_rho * d;
-  const double k_e = kappa_at(der.p[3] + q, s, cv_e, d, lo, hi);
+  const double k_e = kappa_at(der.p[3] + q, s, cv.e, d, lo, hi);
   double e = k_e * d;
   double kv[3];
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
-    kv[l] = kappa_at(der.p[l] + q, s, cv_mom, d, lo, hi);
+    kv[l] = kappa_at(der.p[l] + q, s, cv.mom, d, lo, hi);
     const double gl = l == D ? rbar : 0.5 * rbar;
     const double pm = (gl * kv[l]) * d;
     phi.p[1 + l][q] = pm;
@@ -183,14 +205,14 @@ __global__ void __launch_bounds__(128) kappa3_kernel(Grid3 g, Params3 prm, CV8 w
   km.p[0][q] = kv[A1];
   km.p[1][q] = kv[A2];
   {
-    const double kb = kappa_at(w.p[F_BX + A1] + q, s, cv_b, d, lo, hi);
+    const double kb = kappa_at(w.p[F_BX + A1] + q, s, cv.b, d, lo, hi);
     const double pb = kb * d;
     phi.p[5][q] = pb;
     km.p[2][q] = kb;
     e = fma(0.5 * (lo + hi), pb, e);
   }
   {
-    const double kb = kappa_at(w.p[F_BX + A2] + q, s, cv_b, d, lo, hi);
+    const double kb = kappa_at(w.p[F_BX + A2] + q, s, cv.b, d, lo, hi);
     const double pb = kb * d;
     phi.p[6][q] = pb;
     km.p[3][q] = kb;
@@ -199,36 +221,43 @@ __global__ void __launch_bounds__(128) kappa3_kernel(Grid3 g, Params3 prm, CV8 w
   phi.p[4][q] = e;
 }
 
+// One launch for the three axes: a thread owns cell c in [-2, n+2)^3 and evaluates the interface (c | c + e_d) for every
+// axis d with -1 <= c_d <= n_d - 1 (the windows of the three axes share their centre cells; the y- and z-windows of
+// neighbouring cells are L1 / L2 hits, so the eight input volumes are read from DRAM once instead of three times).
+struct KappaOut { V7 phi[3]; V4 km[3]; };
+__global__ void __launch_bounds__(128) kappa3_kernel(Grid3 g, Params3 prm, CV8 w, CV4 der, const Scalars3* sc, int red_in,
+                                                     KappaOut o) {
+  const int c0 = (int)(blockIdx.x * BX + threadIdx.x) - 2;
+  const int c1 = (int)(blockIdx.y * BY + threadIdx.y) - 2, c2 = (int)(blockIdx.z * BZ + threadIdx.z) - 2;
+  if (c0 >= g.n[0] + 2 || c1 >= g.n[1] + 2 || c2 >= g.n[2] + 2) return;
+  const long long q = addr3(g, c0, c1, c2);
+  const double vt = sqrt(__longlong_as_double((long long)sc->red[red_in][3])) +
+                    sqrt(__longlong_as_double((long long)sc->red[red_in][4]));
+  const KappaCv cv = {prm.c_rho * vt, prm.c_mom * vt, prm.c_e * vt, prm.c_b * vt};
+  if (c0 >= -1 && c0 <= g.n[0] - 1) kappa_dir<0>(g, cv, w, der, q, o.phi[0], o.km[0]);
+  if (c1 >= -1 && c1 <= g.n[1] - 1) kappa_dir<1>(g, cv, w, der, q, o.phi[1], o.km[1]);
+  if (c2 >= -1 && c2 <= g.n[2] - 1) kappa_dir<2>(g, cv, w, der, q, o.phi[2], o.km[2]);
+}
+
 // ------------------------------------------------------------------------------------------------ C_k = F_k - G_k
 // One thread per cell, [-2, n+2) along K, interior across it.  F: c-2.  G (hyperdiffusion on): for each
 // l != K ascending, G(m_l; K) = (rho/2) kbar_l(v_K) d^c_l v_K, G(b_l; K) = - kbar_l(b_K) d^c_l b_K,
 // G(e; K) = sum_l v_l G(m_l; K) + b_l G(b_l; K) (c-11).  kmA / kmB: the kappa arrays of directions l1 < l2.
+struct CellVals { double rho, e, eps, ptt, bv, m[3], b[3], v[3]; };
 template <int K, bool HD>
-__global__ void __launch_bounds__(128) cflux3_kernel(Grid3 g, Params3 prm, CV8 w, CV4 der, CV4 kmA, CV4 kmB, V7 cf) {
+__device__ __forceinline__ void cflux_dir(const Grid3& g, const CellVals& u, const CV8& w, const CV4& der, const CV4& kmA,
+                                          const CV4& kmB, long long q, const V7& cf) {
   constexpr int L1 = K == 0 ? 1 : 0, L2 = K == 2 ? 1 : 2;
-  int c[3];
-  c[0] = (int)(blockIdx.x * blockDim.x + threadIdx.x) + (K == 0 ? -2 : 0);
-  c[1] = (int)blockIdx.y + (K == 1 ? -2 : 0);
-  c[2] = (int)blockIdx.z + (K == 2 ? -2 : 0);
-  if (c[0] >= (K == 0 ? g.n[0] + 2 : g.n[0])) return;
-  const long long q = addr3(g, c[0], c[1], c[2]);
-  const double rho = w.p[F_RHO][q];
-  const double m[3] = {w.p[F_MX][q], w.p[F_MY][q], w.p[F_MZ][q]};
-  const double b[3] = {w.p[F_BX][q], w.p[F_BY][q], w.p[F_BZ][q]};
-  const double v[3] = {der.p[0][q], der.p[1][q], der.p[2][q]};
-  const double eps = der.p[3][q];
-  const double b2h = 0.5 * fma(b[2], b[2], fma(b[1], b[1], b[0] * b[0]));
-  const double ptt = fma(prm.gamma - 1.0, eps, b2h);
-  const double bv = fma(b[2], v[2], fma(b[1], v[1], b[0] * v[0]));
-  const double h = w.p[F_E][q] + ptt;
+  const double* m = u.m; const double* b = u.b; const double* v = u.v;
+  const double h = u.e + u.ptt;
   double F[NPHI];
-  F[0] = rho * v[K];
+  F[0] = u.rho * v[K];
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
     const double f = fma(m[l], v[K], -(b[l] * b[K]));
-    F[1 + l] = l == K ? f + ptt : f;
+    F[1 + l] = l == K ? f + u.ptt : f;
   }
-  F[4] = fma(v[K], h, -(b[K] * bv));
+  F[4] = fma(v[K], h, -(b[K] * u.bv));
   F[5] = fma(v[K], b[L1], -(b[K] * v[L1]));
   F[6] = fma(v[K], b[L2], -(b[K] * v[L2]));
   if (HD) {
@@ -239,13 +268,13 @@ __global__ void __launch_bounds__(128) cflux3_kernel(Grid3 g, Params3 prm, CV8 w
     const double kbb1 = 0.5 * (kmA.p[2 + P1][q - s1] + kmA.p[2 + P1][q]);
     const double dv1 = cd12p(der.p[K] + q, s1) * (1.0 / 12.0);
     const double db1 = cd12p(w.p[F_BX + K] + q, s1) * (1.0 / 12.0);
-    const double gm1 = ((0.5 * rho) * kbv1) * dv1;
+    const double gm1 = ((0.5 * u.rho) * kbv1) * dv1;
     const double gb1 = -(kbb1 * db1);
     const double kbv2 = 0.5 * (kmB.p[P2][q - s2] + kmB.p[P2][q]);
     const double kbb2 = 0.5 * (kmB.p[2 + P2][q - s2] + kmB.p[2 + P2][q]);
     const double dv2 = cd12p(der.p[K] + q, s2) * (1.0 / 12.0);
     const double db2 = cd12p(w.p[F_BX + K] + q, s2) * (1.0 / 12.0);
-    const double gm2 = ((0.5 * rho) * kbv2) * dv2;
+    const double gm2 = ((0.5 * u.rho) * kbv2) * dv2;
     const double gb2 = -(kbb2 * db2);
     double ge = fma(v[L1], gm1, b[L1] * gb1);
     ge = fma(b[L2], gb2, fma(v[L2], gm2, ge));
@@ -257,6 +286,32 @@ __global__ void __launch_bounds__(128) cflux3_kernel(Grid3 g, Params3 prm, CV8 w
   }
 #pragma unroll
   for (int f = 0; f < NPHI; ++f) cf.p[f][q] = F[f];
+}
+
+// One launch for the three flux directions: a thread owns cell c in [-2, n+2)^3; C_k is needed on [-2, n_k + 2) along k and
+// on interior cells across it, so an interior cell evaluates all three and a halo cell the one direction it extends.
+// The point values (12 loads, p_t, b.v) are shared by the three directions.
+struct CfluxIO { CV4 km[3]; V7 cf[3]; };
+template <bool HD>
+__global__ void __launch_bounds__(128) cflux3_kernel(Grid3 g, Params3 prm, CV8 w, CV4 der, CfluxIO io) {
+  const int c0 = (int)(blockIdx.x * BX + threadIdx.x) - 2;
+  const int c1 = (int)(blockIdx.y * BY + threadIdx.y) - 2, c2 = (int)(blockIdx.z * BZ + threadIdx.z) - 2;
+  if (c0 >= g.n[0] + 2 || c1 >= g.n[1] + 2 || c2 >= g.n[2] + 2) return;
+  const bool in0 = c0 >= 0 && c0 < g.n[0], in1 = c1 >= 0 && c1 < g.n[1], in2 = c2 >= 0 && c2 < g.n[2];
+  if ((int)in0 + (int)in1 + (int)in2 < 2) return;            // an edge or corner of the extended box: no direction needs it
+  const long long q = addr3(g, c0, c1, c2);
+  CellVals u;
+  u.rho = w.p[F_RHO][q];
+  u.e = w.p[F_E][q];
+#pragma unroll
+  for (int l = 0; l < 3; ++l) { u.m[l] = w.p[F_MX + l][q]; u.b[l] = w.p[F_BX + l][q]; u.v[l] = der.p[l][q]; }
+  u.eps = der.p[3][q];
+  const double b2h = 0.5 * fma(u.b[2], u.b[2], fma(u.b[1], u.b[1], u.b[0] * u.b[0]));
+  u.ptt = fma(prm.gamma - 1.0, u.eps, b2h);
+  u.bv = fma(u.b[2], u.v[2], fma(u.b[1], u.v[1], u.b[0] * u.v[0]));
+  if (in1 && in2) cflux_dir<0, HD>(g, u, w, der, io.km[1], io.km[2], q, io.cf[0]);
+  if (in0 && in2) cflux_dir<1, HD>(g, u, w, der, io.km[0], io.km[2], q, io.cf[1]);
+  if (in0 && in1) cflux_dir<2, HD>(g, u, w, der, io.km[0], io.km[1], q, io.cf[2]);
 }
 
 // ------------------------------------------------------------------------------------------------ assembly
@@ -288,10 +343,12 @@ template <int COMBINE, int WS, bool HD>
 __global__ void __launch_bounds__(128) assemble3_kernel(const AsmArgs a) {
   __shared__ double sh[5 * 4];
   const Grid3& g = a.g;
-  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+  const int i = (int)(blockIdx.x * BX + threadIdx.x);
+  const int j = (int)(blockIdx.y * BY + threadIdx.y), k = (int)(blockIdx.z * BZ + threadIdx.z);
+  const int tid = (int)((threadIdx.z * BY + threadIdx.y) * BX + threadIdx.x);
   double wsm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  if (i < g.n[0]) {
-    const long long q = addr3(g, i, (int)blockIdx.y, (int)blockIdx.z);
+  if (i < g.n[0] && j < g.n[1] && k < g.n[2]) {
+    const long long q = addr3(g, i, j, k);
     const long long st[3] = {1, g.pitch, g.plane};
     double R[NF];
     // -(1/12) sum_d cd12(C_d) / Delta_d, nested x outermost: fma(cd_x, 1/dx, fma(cd_y, 1/dy, cd_z (1/dz)))
@@ -365,19 +422,18 @@ __global__ void __launch_bounds__(128) assemble3_kernel(const AsmArgs a) {
     }
   }
   // block maximum (warp shuffles), one atomicMax per value and CTA; NaNs never enter (x > 0 ? x : 0)
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int lane = tid & 31, wid = tid >> 5;
   constexpr int FROM = WS == WS_FULL ? 0 : 3;
 #pragma unroll
-  for (int k = FROM; k < 5; ++k) {
-    const double m = warp_max(wsm[k]);
-    if (lane == 0) sh[k * 4 + wid] = m;
+  for (int v = FROM; v < 5; ++v) {
+    const double m = warp_max(wsm[v]);
+    if (lane == 0) sh[v * 4 + wid] = m;
   }
   __syncthreads();
-  if (threadIdx.x < 5 && (int)threadIdx.x >= FROM) {
-    const int k = threadIdx.x;
-    double m = sh[k * 4];
-    for (int w2 = 1; w2 < 4; ++w2) m = sh[k * 4 + w2] > m ? sh[k * 4 + w2] : m;
-    atomicMax(&a.sc->red[a.red_out][k], (unsigned long long)__double_as_longlong(m));
+  if (tid < 5 && tid >= FROM) {
+    double m = sh[tid * 4];
+    for (int w2 = 1; w2 < 4; ++w2) m = sh[tid * 4 + w2] > m ? sh[tid * 4 + w2] : m;
+    atomicMax(&a.sc->red[a.red_out][tid], (unsigned long long)__double_as_longlong(m));
   }
 }
 
@@ -558,40 +614,44 @@ struct Timed {
 };
 
 dim3 grid_for(int nxr, int nyr, int nzr) { return dim3((unsigned)((nxr + 127) / 128), (unsigned)nyr, (unsigned)nzr); }
+// grid / block of the stencil kernels (BX x BY x BZ threads)
+dim3 sgrid_for(int nxr, int nyr, int nzr) { return dim3((unsigned)((nxr + BX - 1) / BX), (unsigned)((nyr + BY - 1) / BY), (unsigned)((nzr + BZ - 1) / BZ)); }
+const dim3 SBLOCK(BX, BY, BZ);
 
 void launch_ghost(Ctx& c, V8 w, int freeze) {
   Timed t(c, 0);
   const Grid3& g = c.g;
-  ghost3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, w, freeze);
+  ghost3_kernel<2><<<grid_for(g.n[0] + 6, g.n[1] + 6, 6), 128, 0, c.stream>>>(g, w, freeze);
+  ghost3_kernel<1><<<grid_for(g.n[0] + 6, 6, g.n[2]), 128, 0, c.stream>>>(g, w, freeze);
+  ghost3_kernel<0><<<dim3((unsigned)((6 * g.n[1] + 127) / 128), (unsigned)g.n[2], 1), 128, 0, c.stream>>>(g, w, freeze);
+  c.launches += 2;
 }
 
-template <int D>
 void launch_kappa(Ctx& c, const Params3& p, const V8& in, int red_in) {
   Timed t(c, 2);
   const Grid3& g = c.g;
-  const int r[3] = {D == 0 ? g.n[0] + 1 : g.n[0] + 4, D == 1 ? g.n[1] + 1 : g.n[1] + 4, D == 2 ? g.n[2] + 1 : g.n[2] + 4};
-  kappa3_kernel<D><<<grid_for(r[0], r[1], r[2]), 128, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), c.sc, red_in, c.phi[D], c.km[D]);
+  KappaOut o;
+  for (int d = 0; d < 3; ++d) { o.phi[d] = c.phi[d]; o.km[d] = c.km[d]; }
+  kappa3_kernel<<<sgrid_for(g.n[0] + 4, g.n[1] + 4, g.n[2] + 4), SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), c.sc, red_in, o);
 }
 
-template <int K>
 void launch_cflux(Ctx& c, const Params3& p, const V8& in) {
   Timed t(c, 3);
   const Grid3& g = c.g;
-  constexpr int L1 = K == 0 ? 1 : 0, L2 = K == 2 ? 1 : 2;
-  const int r[3] = {K == 0 ? g.n[0] + 4 : g.n[0], K == 1 ? g.n[1] + 4 : g.n[1], K == 2 ? g.n[2] + 4 : g.n[2]};
-  if (c.hd_on)
-    cflux3_kernel<K, true><<<grid_for(r[0], r[1], r[2]), 128, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), cv4(c.km[L1]), cv4(c.km[L2]), c.cf[K]);
-  else
-    cflux3_kernel<K, false><<<grid_for(r[0], r[1], r[2]), 128, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), cv4(c.km[L1]), cv4(c.km[L2]), c.cf[K]);
+  CfluxIO io;
+  for (int d = 0; d < 3; ++d) { io.km[d] = cv4(c.km[d]); io.cf[d] = c.cf[d]; }
+  const dim3 gr = sgrid_for(g.n[0] + 4, g.n[1] + 4, g.n[2] + 4);
+  if (c.hd_on) cflux3_kernel<true><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), io);
+  else cflux3_kernel<false><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), io);
 }
 
 template <int COMBINE, int WS>
 void launch_assemble(Ctx& c, const AsmArgs& a) {
   Timed t(c, 4);
   const Grid3& g = c.g;
-  const dim3 gr = grid_for(g.n[0], g.n[1], g.n[2]);
-  if (c.hd_on) assemble3_kernel<COMBINE, WS, true><<<gr, 128, 0, c.stream>>>(a);
-  else assemble3_kernel<COMBINE, WS, false><<<gr, 128, 0, c.stream>>>(a);
+  const dim3 gr = sgrid_for(g.n[0], g.n[1], g.n[2]);
+  if (c.hd_on) assemble3_kernel<COMBINE, WS, true><<<gr, SBLOCK, 0, c.stream>>>(a);
+  else assemble3_kernel<COMBINE, WS, false><<<gr, SBLOCK, 0, c.stream>>>(a);
 }
 
 // one RK stage: out = combine(in, R(in)); the maxima of `in` are in set red_in, those of `out` go to red_out
@@ -603,14 +663,8 @@ void stage(Ctx& c, int in, int base, int out, int combine, int ws, double coef, 
     const Grid3& g = c.g;
     derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[in]), c.der);
   }
-  if (c.hd_on) {
-    launch_kappa<0>(c, p, c.buf[in], red_in);
-    launch_kappa<1>(c, p, c.buf[in], red_in);
-    launch_kappa<2>(c, p, c.buf[in], red_in);
-  }
-  launch_cflux<0>(c, p, c.buf[in]);
-  launch_cflux<1>(c, p, c.buf[in]);
-  launch_cflux<2>(c, p, c.buf[in]);
+  if (c.hd_on) launch_kappa(c, p, c.buf[in], red_in);
+  launch_cflux(c, p, c.buf[in]);
   AsmArgs a;
   a.g = c.g;
   a.prm = p;
