@@ -337,8 +337,8 @@ def run_ours(args):
 
 def run_3d(args):
     """A 3-D workload: same JSON line; a step = dt + 4 x {ghost fill, derived quantities, kappa /
-    interface fluxes along x, y, z, cell-centred fluxes along x, y, z, assembly + RK combine + reduction}.  The roofline
-    entry is taken over the whole stage (the nine launches together) against what a fully fused stage must move:
+    interface fluxes, cell-centred fluxes, assembly + RK combine + reduction}.  The roofline
+    entry is taken over the whole stage (its kernels together) against what a fully fused stage must move:
     8 fields x 8 B x (4 reads with halo + 4 writes + 2 x w^n + accumulator written once and read once) = 768 B per
     cell-update, 192 B per cell and stage."""
     import torch
@@ -397,7 +397,7 @@ def run_3d(args):
         "hbm_gbs_algorithmic": cells * K / (ms * 1e-3) * bpcu / 1e9,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": None, "peak_source": peak_src,
-                     "kernel": "smaug3 RK stage (9 launches: ghost3, derive3, 3 x kappa3, 3 x cflux3, assemble3); "
+                     "kernel": "smaug3 RK stage (ghost3, derive3, kappa3, cflux3, assemble3); "
                                f"largest share: {top}",
                      "bytes_per_launch": bpcu / stages * cells, "avg_launch_ms": stage_ms,
                      "launches_timed": int(sum(v[1] for v in kinds.values())),

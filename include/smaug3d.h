@@ -74,7 +74,7 @@ int smaug3_set_state(smaug3_ctx* ctx, const void* w);
 
 /* Advance n_steps time steps with dt = cfl min_d(Delta_d / cmax_d) (or the fixed dt): per step one dt launch and,
  * per RK stage, ghost fill -> derived quantities -> kappa / interface fluxes along x, y, z -> cell-centred fluxes
- * C_d = F_d - G_d -> assembly, RK combine and wave-speed reduction.  dt and the maxima stay on the device.
+ * C_d = F_d - G_d -> assembly, RK combine and wave-speed reduction (five kernels).  dt and the maxima stay on the device.
  * ENONFINITE if a time step was non-finite or <= 0. */
 int smaug3_step(smaug3_ctx* ctx, int n_steps, double cfl);
 

@@ -6,9 +6,9 @@
 // First 3-D form: an RK stage is a short sequence of streaming kernels over padded volumes in HBM,
 //   ghost3_kernel     ghost cells of the stage input, six sides, edges and corners by composing the three maps (c-8)
 //   derive3_kernel    v = m (1/rho), eps on every padded cell (c-2)
-//   kappa3_kernel<d>  per interface along d: the seven hyperviscosity ratios (c-5) and the interface fluxes Phi_d of
-//                     all fields; keeps kappa_d(v_k), kappa_d(b_k), k != d, for the mixed terms
-//   cflux3_kernel<k>  per cell: C_k = F_k - G_k (c-2 fluxes minus the mixed fluxes of c-5 / c-11)
+//   kappa3_kernel     per interface along each axis d: the seven hyperviscosity ratios (c-5) and the interface fluxes
+//                     Phi_d of all fields; keeps kappa_d(v_k), kappa_d(b_k), k != d, for the mixed terms
+//   cflux3_kernel     per cell and direction k: C_k = F_k - G_k (c-2 fluxes minus the mixed fluxes of c-5 / c-11)
 //   assemble3_kernel  per cell: R = -sum_k d^c_k C_k + gravity + sum_d (Phi_d+ - Phi_d-)/Delta_d, the RK combine in
 //                     the epilogue, the store, and the wave-speed maxima of the written state (warp shuffles, one
 //                     atomicMax pass per CTA)
