@@ -5,7 +5,8 @@
 //
 // First 3-D form: an RK stage is a short sequence of streaming kernels over padded volumes in HBM,
 //   ghost3_kernel     ghost cells of the stage input, six sides, edges and corners by composing the three maps (c-8)
-//   derive3_kernel    v = m (1/rho), eps on every padded cell (c-2)
+//   derive3_kernel    v = m (1/rho), eps on every padded cell (c-2): at set_state only; afterwards the assembly epilogue
+//                     writes them for the state it produces and the ghost fill carries them into the ghost cells
 //   kappa3_kernel     per interface along each axis d: the seven hyperviscosity ratios (c-5) and the interface fluxes
 //                     Phi_d of all fields; keeps kappa_d(v_k), kappa_d(b_k), k != d, for the mixed terms
 //   cflux3_kernel     per cell and direction k: C_k = F_k - G_k (c-2 fluxes minus the mixed fluxes of c-5 / c-11)
@@ -69,6 +70,7 @@ struct CV8 { const double* p[NF]; };
 struct V7 { double* p[NPHI]; };
 struct CV7 { const double* p[NPHI]; };
 struct V4 { double* p[4]; };
+struct V12 { double* p[NF + 4]; };     // the state and its derived quantities (ghost fill)
 struct CV4 { const double* p[4]; };
 
 struct Scalars3 {
@@ -115,8 +117,9 @@ __device__ __forceinline__ int wrap_idx(int i, int n) {
 // Composed: a ghost cell takes the cell reached by mapping z, then y, then x (periodic: wrap, open: clamp); a FIXED
 // side is never rewritten -- if the outermost out-of-range axis (z before y before x) is fixed the cell is skipped,
 // and a fixed axis met later stops the mapping (the source is then a frozen ghost).  freeze: fixed acts like open
-// (set_state).  Reads interior cells or frozen ghosts, writes other ghosts: no race within the launch.
-__device__ __forceinline__ void ghost_cell(const Grid3& g, const V8& w, int freeze, int i, int j, int k) {
+// (set_state).  Reads interior cells or frozen ghosts, writes other ghosts: no race within the launch.  The derived
+// quantities (v, eps) ride along: a ghost cell's derived values are those of its source cell, bit for bit.
+__device__ __forceinline__ void ghost_cell(const Grid3& g, const V12& w, int freeze, int i, int j, int k) {
   int c[3] = {i, j, k};
   bool first = true;
 #pragma unroll
@@ -132,7 +135,7 @@ __device__ __forceinline__ void ghost_cell(const Grid3& g, const V8& w, int free
   }
   const long long dst = addr3(g, i, j, k), src = addr3(g, c[0], c[1], c[2]);
 #pragma unroll
-  for (int f = 0; f < NF; ++f) w.p[f][dst] = w.p[f][src];
+  for (int f = 0; f < NF + 4; ++f) w.p[f][dst] = w.p[f][src];
 }
 // ghost index 0..5 -> -3, -2, -1, n, n+1, n+2
 __device__ __forceinline__ int ghost_coord(int s, int n) { return s < NG ? s - NG : n + (s - NG); }
@@ -140,7 +143,7 @@ __device__ __forceinline__ int ghost_coord(int s, int n) { return s < NG ? s - N
 // The ghost shell in three launches (only ghost cells get a thread): SLAB 2: the six ghost planes (all i, j);
 // SLAB 1: the six ghost rows of every interior plane (all i); SLAB 0: the six ghost columns of every interior row.
 template <int SLAB>
-__global__ void __launch_bounds__(128) ghost3_kernel(Grid3 g, V8 w, int freeze) {
+__global__ void __launch_bounds__(128) ghost3_kernel(Grid3 g, V12 w, int freeze) {
   int i, j, k;
   if (SLAB == 2) {
     i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - NG;
@@ -319,7 +322,7 @@ struct AsmArgs {
   Grid3 g;
   Params3 prm;
   CV7 cf[3], phi[3];
-  CV4 der;
+  V4 der;             // derived quantities of the stage input (read: gravity); overwritten with those of the output
   CV8 in, base, acc_in;
   V8 out, acc_out;
   Scalars3* sc;
@@ -398,11 +401,14 @@ __global__ void __launch_bounds__(128) assemble3_kernel(const AsmArgs a) {
     }
 #pragma unroll
     for (int f = 0; f < NF; ++f) a.out.p[f][q] = o[f];
-    // wave speeds of the written cell (c-4)
+    // derived quantities of the written cell (c-2) -- the next stage's input: derive3_kernel's operations -- and its
+    // wave speeds (c-4), which share every sub-expression with them
     const double rr = drcp(o[F_RHO]);
     const double vx = o[F_MX] * rr, vy = o[F_MY] * rr, vz = o[F_MZ] * rr;
     const double B2 = fma(o[F_BZ], o[F_BZ], fma(o[F_BY], o[F_BY], o[F_BX] * o[F_BX]));
-    const double pk = (a.prm.gamma - 1.0) * ((o[F_E] - 0.5 * fma(o[F_MZ], vz, fma(o[F_MY], vy, o[F_MX] * vx))) - 0.5 * B2);
+    const double eps = (o[F_E] - 0.5 * fma(o[F_MZ], vz, fma(o[F_MY], vy, o[F_MX] * vx))) - 0.5 * B2;
+    a.der.p[0][q] = vx; a.der.p[1][q] = vy; a.der.p[2][q] = vz; a.der.p[3][q] = eps;
+    const double pk = (a.prm.gamma - 1.0) * eps;
     const double a2 = (a.prm.gamma * pk) * rr;
     const double b2 = B2 * rr;
     wsm[3] = a2 > 0.0 ? a2 : 0.0;
@@ -618,9 +624,12 @@ dim3 grid_for(int nxr, int nyr, int nzr) { return dim3((unsigned)((nxr + 127) / 
 dim3 sgrid_for(int nxr, int nyr, int nzr) { return dim3((unsigned)((nxr + BX - 1) / BX), (unsigned)((nyr + BY - 1) / BY), (unsigned)((nzr + BZ - 1) / BZ)); }
 const dim3 SBLOCK(BX, BY, BZ);
 
-void launch_ghost(Ctx& c, V8 w, int freeze) {
+void launch_ghost(Ctx& c, const V8& w8, int freeze) {
   Timed t(c, 0);
   const Grid3& g = c.g;
+  V12 w;
+  for (int f = 0; f < NF; ++f) w.p[f] = w8.p[f];
+  for (int f = 0; f < 4; ++f) w.p[NF + f] = c.der.p[f];
   ghost3_kernel<2><<<grid_for(g.n[0] + 6, g.n[1] + 6, 6), 128, 0, c.stream>>>(g, w, freeze);
   ghost3_kernel<1><<<grid_for(g.n[0] + 6, 6, g.n[2]), 128, 0, c.stream>>>(g, w, freeze);
   ghost3_kernel<0><<<dim3((unsigned)((6 * g.n[1] + 127) / 128), (unsigned)g.n[2], 1), 128, 0, c.stream>>>(g, w, freeze);
@@ -657,19 +666,14 @@ void launch_assemble(Ctx& c, const AsmArgs& a) {
 // one RK stage: out = combine(in, R(in)); the maxima of `in` are in set red_in, those of `out` go to red_out
 void stage(Ctx& c, int in, int base, int out, int combine, int ws, double coef, int red_in, int red_out) {
   const Params3 p = params(c);
-  launch_ghost(c, c.buf[in], 0);
-  {
-    Timed t(c, 1);
-    const Grid3& g = c.g;
-    derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[in]), c.der);
-  }
+  launch_ghost(c, c.buf[in], 0);        // (the derived quantities of `in` were written by the stage that produced it)
   if (c.hd_on) launch_kappa(c, p, c.buf[in], red_in);
   launch_cflux(c, p, c.buf[in]);
   AsmArgs a;
   a.g = c.g;
   a.prm = p;
   for (int d = 0; d < 3; ++d) { a.cf[d] = cv7(c.cf[d]); a.phi[d] = cv7(c.phi[d]); }
-  a.der = cv4(c.der);
+  a.der = c.der;
   a.in = cv8(c.buf[in]);
   a.base = cv8(c.buf[base]);
   a.acc_in = cv8(c.buf[3]);
@@ -813,6 +817,10 @@ int smaug3_set_state(smaug3_ctx* ctx, const void* w) {
   pack3_kernel<<<gi, 128, 0, c.stream>>>(g, staging, c.buf[0], 0, nullptr);
   ++c.launches;
   launch_ghost(c, c.buf[0], 1);
+  {
+    Timed t(c, 1);     // derived quantities on every padded cell, once (afterwards the stage epilogues keep them current)
+    derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[0]), c.der);
+  }
   // the other two buffers that are read with a halo get the same frozen ghosts (fixed sides are never rewritten)
   for (int b = 1; b <= 2; ++b)
     for (int f = 0; f < NF; ++f)
