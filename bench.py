@@ -398,7 +398,7 @@ def run_3d(args):
         "hbm_gbs_algorithmic": cells * K / (ms * 1e-3) * bpcu / 1e9,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "frac_of_nominal_8TBs": achieved / 8000.0, "traffic": None, "peak_source": peak_src,
-                     "kernel": "smaug3 RK stage (ghost3, derive3, kappa3, cflux3, assemble3); "
+                     "kernel": "smaug3 RK stage (ghost3, kappa3, stage3); "
                                f"largest share: {top}",
                      "bytes_per_launch": bpcu / stages * cells, "avg_launch_ms": stage_ms,
                      "launches_timed": int(sum(v[1] for v in kinds.values())),

@@ -17,7 +17,7 @@
  *   - bc[6] = x_lo, x_hi, y_lo, y_hi, z_lo, z_hi, each SMAUG3_BC_*; periodic must be set on both sides of an axis.
  *   - cell centres x_i = (i + 1/2) Lx / nx, likewise y, z; Lx = Ly = Lz = 1 by default; ghost width 3.
  *   - a context lives on the device current at smaug3_create and owns its device memory (cudaMalloc; about
- *     91 padded volumes of (nx + 19 rounded up to 16) x (ny + 6) x (nz + 6) doubles -- smaug3_workspace_bytes tells);
+ *     94 padded volumes of (nx + 19 rounded up to 16) x (ny + 6) x (nz + 6) doubles -- smaug3_workspace_bytes tells);
  *     every entry point makes that device current for the call and restores the caller's.
  *   - all work is enqueued on the stream given at creation (0 = the legacy default stream); smaug3_step,
  *     smaug3_get_state, smaug3_get_time and smaug3_get_wavespeeds synchronise it before returning.
@@ -48,7 +48,9 @@ enum { /* keys of smaug3_set_param: 0..11 mean what they mean in smaug.h */
   SMAUG3_PARAM_FIXED_DT = 8, /* > 0: this dt instead of the CFL step */
   SMAUG3_PARAM_GX = 10, SMAUG3_PARAM_GY = 11,
   SMAUG3_PARAM_LZ = 13,      /* domain length in z, > 0 (default 1) */
-  SMAUG3_PARAM_GZ = 14       /* third component of the uniform gravitational acceleration */
+  SMAUG3_PARAM_GZ = 14,      /* third component of the uniform gravitational acceleration */
+  SMAUG3_PARAM_KERNEL = 15   /* 1 (default): cell-centred fluxes and assembly fused in one kernel (C_d in shared memory);
+                                0: two kernels with the C_d volumes in HBM.  Same bits; the switch is for tests / profiling */
 };
 
 /* Thread-local message of the last failed call (never NULL). */

@@ -317,7 +317,7 @@ class SmaugGroup:
             pass
 
 
-PARAMS3 = dict(lx=0, ly=1, hd_on=2, c_rho=3, c_mom=4, c_e=5, c_b=6, rk_order=7, fixed_dt=8, gx=10, gy=11, lz=13, gz=14)
+PARAMS3 = dict(lx=0, ly=1, hd_on=2, c_rho=3, c_mom=4, c_e=5, c_b=6, rk_order=7, fixed_dt=8, gx=10, gy=11, lz=13, gz=14, kernel=15)
 KERNEL_KINDS3 = ("ghost fill + dt", "derived quantities", "kappa / interface fluxes", "cell-centred fluxes", "assembly")
 
 

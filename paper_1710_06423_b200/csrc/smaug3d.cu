@@ -3,19 +3,18 @@
 // formula is the explicit IEEE operation sequence the 3-D oracle documents; results are bit-identical to it).
 // Product code: shares nothing with oracle/.
 //
-// First 3-D form: an RK stage is a short sequence of streaming kernels over padded volumes in HBM,
-//   ghost3_kernel     ghost cells of the stage input, six sides, edges and corners by composing the three maps (c-8)
-//   derive3_kernel    v = m (1/rho), eps on every padded cell (c-2): at set_state only; afterwards the assembly epilogue
-//                     writes them for the state it produces and the ghost fill carries them into the ghost cells
+// First 3-D form: an RK stage is three kernels over padded volumes in HBM,
+//   ghost3_kernel     ghost cells of the stage input and of its derived quantities, six sides, edges and corners by composing
+//                     the three maps (c-8); only the ghost shell gets threads
 //   kappa3_kernel     per interface along each axis d: the seven hyperviscosity ratios (c-5) and the interface fluxes
 //                     Phi_d of all fields; keeps kappa_d(v_k), kappa_d(b_k), k != d, for the mixed terms
-//   cflux3_kernel     per cell and direction k: C_k = F_k - G_k (c-2 fluxes minus the mixed fluxes of c-5 / c-11)
-//   assemble3_kernel  per cell: R = -sum_k d^c_k C_k + gravity + sum_d (Phi_d+ - Phi_d-)/Delta_d, the RK combine in
-//                     the epilogue, the store, and the wave-speed maxima of the written state (warp shuffles, one
-//                     atomicMax pass per CTA)
-// thread per cell, x fastest (coalesced), stencil neighbours through L1/L2.  dt, t and the maxima stay on the
-// device; one host synchronisation per smaug3_step call.  DESIGN.md section 5 has the byte counts and what a fused
-// 2.5-D march (the 2-D kernel's design carried to 3-D) would save.
+//   stage3_kernel     per 32 x 4 x 4 tile: C_k = F_k - G_k (c-2 fluxes minus the mixed fluxes of c-5 / c-11) through shared
+//                     memory, one direction at a time; R = -sum_k d^c_k C_k + gravity + sum_d (Phi_d+ - Phi_d-)/Delta_d; the RK
+//                     combine in the epilogue, the store, the derived quantities v, eps of the written state (c-2) and its
+//                     wave-speed maxima (warp shuffles, one atomicMax pass per CTA)
+// (SMAUG3_PARAM_KERNEL = 0: cflux3_kernel + assemble3_kernel, the same with the C_k volumes in HBM; derive3_kernel: v, eps on
+// every padded cell, at set_state).  dt, t and the maxima stay on the device; one host synchronisation per smaug3_step call.
+// DESIGN.md section 5 has the byte counts and what taking kappa / Phi out of HBM as well would need.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -249,11 +248,10 @@ __global__ void __launch_bounds__(128) kappa3_kernel(Grid3 g, Params3 prm, CV8 w
 struct CellVals { double rho, e, eps, ptt, bv, m[3], b[3], v[3]; };
 template <int K, bool HD>
 __device__ __forceinline__ void cflux_dir(const Grid3& g, const CellVals& u, const CV8& w, const CV4& der, const CV4& kmA,
-                                          const CV4& kmB, long long q, const V7& cf) {
+                                          const CV4& kmB, long long q, double (&F)[NPHI]) {
   constexpr int L1 = K == 0 ? 1 : 0, L2 = K == 2 ? 1 : 2;
   const double* m = u.m; const double* b = u.b; const double* v = u.v;
   const double h = u.e + u.ptt;
-  double F[NPHI];
   F[0] = u.rho * v[K];
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
@@ -287,8 +285,18 @@ __device__ __forceinline__ void cflux_dir(const Grid3& g, const CellVals& u, con
     F[5] = F[5] - gb1;
     F[6] = F[6] - gb2;
   }
+}
+
+// the point values of cell q that the three flux directions share (12 loads, p_t, b.v)
+__device__ __forceinline__ void load_cell(const Params3& prm, const CV8& w, const CV4& der, long long q, CellVals& u) {
+  u.rho = w.p[F_RHO][q];
+  u.e = w.p[F_E][q];
 #pragma unroll
-  for (int f = 0; f < NPHI; ++f) cf.p[f][q] = F[f];
+  for (int l = 0; l < 3; ++l) { u.m[l] = w.p[F_MX + l][q]; u.b[l] = w.p[F_BX + l][q]; u.v[l] = der.p[l][q]; }
+  u.eps = der.p[3][q];
+  const double b2h = 0.5 * fma(u.b[2], u.b[2], fma(u.b[1], u.b[1], u.b[0] * u.b[0]));
+  u.ptt = fma(prm.gamma - 1.0, u.eps, b2h);
+  u.bv = fma(u.b[2], u.v[2], fma(u.b[1], u.v[1], u.b[0] * u.v[0]));
 }
 
 // One launch for the three flux directions: a thread owns cell c in [-2, n+2)^3; C_k is needed on [-2, n_k + 2) along k and
@@ -304,17 +312,23 @@ __global__ void __launch_bounds__(128) cflux3_kernel(Grid3 g, Params3 prm, CV8 w
   if ((int)in0 + (int)in1 + (int)in2 < 2) return;            // an edge or corner of the extended box: no direction needs it
   const long long q = addr3(g, c0, c1, c2);
   CellVals u;
-  u.rho = w.p[F_RHO][q];
-  u.e = w.p[F_E][q];
+  load_cell(prm, w, der, q, u);
+  double F[NPHI];
+  if (in1 && in2) {
+    cflux_dir<0, HD>(g, u, w, der, io.km[1], io.km[2], q, F);
 #pragma unroll
-  for (int l = 0; l < 3; ++l) { u.m[l] = w.p[F_MX + l][q]; u.b[l] = w.p[F_BX + l][q]; u.v[l] = der.p[l][q]; }
-  u.eps = der.p[3][q];
-  const double b2h = 0.5 * fma(u.b[2], u.b[2], fma(u.b[1], u.b[1], u.b[0] * u.b[0]));
-  u.ptt = fma(prm.gamma - 1.0, u.eps, b2h);
-  u.bv = fma(u.b[2], u.v[2], fma(u.b[1], u.v[1], u.b[0] * u.v[0]));
-  if (in1 && in2) cflux_dir<0, HD>(g, u, w, der, io.km[1], io.km[2], q, io.cf[0]);
-  if (in0 && in2) cflux_dir<1, HD>(g, u, w, der, io.km[0], io.km[2], q, io.cf[1]);
-  if (in0 && in1) cflux_dir<2, HD>(g, u, w, der, io.km[0], io.km[1], q, io.cf[2]);
+    for (int f = 0; f < NPHI; ++f) io.cf[0].p[f][q] = F[f];
+  }
+  if (in0 && in2) {
+    cflux_dir<1, HD>(g, u, w, der, io.km[0], io.km[2], q, F);
+#pragma unroll
+    for (int f = 0; f < NPHI; ++f) io.cf[1].p[f][q] = F[f];
+  }
+  if (in0 && in1) {
+    cflux_dir<2, HD>(g, u, w, der, io.km[0], io.km[1], q, F);
+#pragma unroll
+    for (int f = 0; f < NPHI; ++f) io.cf[2].p[f][q] = F[f];
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ assembly
@@ -322,7 +336,9 @@ struct AsmArgs {
   Grid3 g;
   Params3 prm;
   CV7 cf[3], phi[3];
-  V4 der;             // derived quantities of the stage input (read: gravity); overwritten with those of the output
+  CV4 der;            // derived quantities of the stage input
+  V4 der_out;         // ... of the stage output, written by the epilogue (another set of volumes: neighbouring CTAs of the
+                      // fused kernel may still be reading `der` when this one writes)
   CV8 in, base, acc_in;
   V8 out, acc_out;
   Scalars3* sc;
@@ -342,6 +358,93 @@ __device__ __forceinline__ double warp_max(double v) {
 // slot of field component `l` of b (or the marker -1 for l == d) inside the 7-component C_d / Phi_d arrays
 __host__ __device__ constexpr int bslot(int l, int d) { return l == d ? -1 : 5 + l - (l > d ? 1 : 0); }
 
+// Everything after the central flux divergence of one interior cell: gravity (c-10), the interface-flux differences along
+// x, y, z (c-5), the RK combine (c-6), the stores, the derived quantities of the written cell (the next stage's input:
+// derive3_kernel's operations) and its wave speeds (c-4), which share every sub-expression with them.
+template <int COMBINE, int WS, bool HD>
+__device__ __forceinline__ void finish_cell(const AsmArgs& a, long long q, double (&R)[NF], double (&wsm)[5]) {
+  const long long st[3] = {1, a.g.pitch, a.g.plane};
+  if (a.prm.grav_on) {
+    const double rt = a.in.p[F_RHO][q];
+    const double gv = fma(a.prm.g[2], a.der.p[2][q], fma(a.prm.g[1], a.der.p[1][q], a.prm.g[0] * a.der.p[0][q]));
+#pragma unroll
+    for (int l = 0; l < 3; ++l) R[F_MX + l] = fma(rt, a.prm.g[l], R[F_MX + l]);
+    R[F_E] = fma(rt, gv, R[F_E]);
+  }
+  if (HD) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const int slot = f < F_BX ? f : bslot(f - F_BX, d);
+        const double diff = slot < 0 ? 0.0 : a.phi[d].p[slot][q] - a.phi[d].p[slot][q - st[d]];
+        R[f] = fma(diff, a.prm.inv_d[d], R[f]);
+      }
+    }
+  }
+  const double cdt = a.c * a.sc->dt;
+  double o[NF];
+  if (COMBINE == COMBINE_FINAL) {
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const double w3 = a.in.p[f][q];
+      o[f] = fma(cdt, R[f], fma(fma(-2.0, w3, a.acc_in.p[f][q]), 1.0 / 3.0, w3));
+    }
+  } else {
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const double wb = a.base.p[f][q];
+      o[f] = fma(cdt, R[f], wb);
+      if (COMBINE == COMBINE_ACC) a.acc_out.p[f][q] = fma(2.0, o[f], a.in.p[f][q] - wb);
+    }
+  }
+#pragma unroll
+  for (int f = 0; f < NF; ++f) a.out.p[f][q] = o[f];
+  const double rr = drcp(o[F_RHO]);
+  const double vx = o[F_MX] * rr, vy = o[F_MY] * rr, vz = o[F_MZ] * rr;
+  const double B2 = fma(o[F_BZ], o[F_BZ], fma(o[F_BY], o[F_BY], o[F_BX] * o[F_BX]));
+  const double eps = (o[F_E] - 0.5 * fma(o[F_MZ], vz, fma(o[F_MY], vy, o[F_MX] * vx))) - 0.5 * B2;
+  a.der_out.p[0][q] = vx; a.der_out.p[1][q] = vy; a.der_out.p[2][q] = vz; a.der_out.p[3][q] = eps;
+  const double pk = (a.prm.gamma - 1.0) * eps;
+  const double a2 = (a.prm.gamma * pk) * rr;
+  const double b2 = B2 * rr;
+  wsm[3] = a2 > 0.0 ? a2 : 0.0;
+  wsm[4] = b2 > 0.0 ? b2 : 0.0;
+  if (WS == WS_FULL) {
+    const double s = a2 + b2;
+    const double fa = (4.0 * a2) * rr;
+    const double vv[3] = {vx, vy, vz};
+    const double bb[3] = {o[F_BX], o[F_BY], o[F_BZ]};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double disc = fma(s, s, -(fa * (bb[d] * bb[d])));
+      const double cf2 = 0.5 * (s + sqrt(disc > 0.0 ? disc : 0.0));
+      const double cc = fabs(vv[d]) + sqrt(cf2);
+      wsm[d] = cc > 0.0 ? cc : 0.0;
+    }
+  }
+}
+
+// block maximum of the five candidates (warp shuffles), one atomicMax per value and CTA; NaNs never enter (x > 0 ? x : 0).
+// sh: 5 * NW doubles of shared memory; every thread of the CTA calls.
+template <int WS, int NW>
+__device__ __forceinline__ void block_max5_atomic(const double (&wsm)[5], double* sh, int tid, unsigned long long* slots) {
+  const int lane = tid & 31, wid = tid >> 5;
+  constexpr int FROM = WS == WS_FULL ? 0 : 3;
+#pragma unroll
+  for (int v = FROM; v < 5; ++v) {
+    const double m = warp_max(wsm[v]);
+    if (lane == 0) sh[v * NW + wid] = m;
+  }
+  __syncthreads();
+  if (tid < 5 && tid >= FROM) {
+    double m = sh[tid * NW];
+    for (int w2 = 1; w2 < NW; ++w2) m = sh[tid * NW + w2] > m ? sh[tid * NW + w2] : m;
+    atomicMax(&slots[tid], (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+// multi-pass form: C_d from the volumes cflux3_kernel wrote
 template <int COMBINE, int WS, bool HD>
 __global__ void __launch_bounds__(128) assemble3_kernel(const AsmArgs a) {
   __shared__ double sh[5 * 4];
@@ -365,82 +468,110 @@ __global__ void __launch_bounds__(128) assemble3_kernel(const AsmArgs a) {
       }
       R[f] = fma(cd[0], a.prm.inv_d[0], fma(cd[1], a.prm.inv_d[1], cd[2] * a.prm.inv_d[2])) * (-1.0 / 12.0);
     }
-    if (a.prm.grav_on) {
-      const double rt = a.in.p[F_RHO][q];
-      const double gv = fma(a.prm.g[2], a.der.p[2][q], fma(a.prm.g[1], a.der.p[1][q], a.prm.g[0] * a.der.p[0][q]));
-#pragma unroll
-      for (int l = 0; l < 3; ++l) R[F_MX + l] = fma(rt, a.prm.g[l], R[F_MX + l]);
-      R[F_E] = fma(rt, gv, R[F_E]);
-    }
-    if (HD) {
-#pragma unroll
-      for (int d = 0; d < 3; ++d) {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-          const int slot = f < F_BX ? f : bslot(f - F_BX, d);
-          const double diff = slot < 0 ? 0.0 : a.phi[d].p[slot][q] - a.phi[d].p[slot][q - st[d]];
-          R[f] = fma(diff, a.prm.inv_d[d], R[f]);
-        }
-      }
-    }
-    const double cdt = a.c * a.sc->dt;
-    double o[NF];
-    if (COMBINE == COMBINE_FINAL) {
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        const double w3 = a.in.p[f][q];
-        o[f] = fma(cdt, R[f], fma(fma(-2.0, w3, a.acc_in.p[f][q]), 1.0 / 3.0, w3));
-      }
-    } else {
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        const double wb = a.base.p[f][q];
-        o[f] = fma(cdt, R[f], wb);
-        if (COMBINE == COMBINE_ACC) a.acc_out.p[f][q] = fma(2.0, o[f], a.in.p[f][q] - wb);
-      }
-    }
-#pragma unroll
-    for (int f = 0; f < NF; ++f) a.out.p[f][q] = o[f];
-    // derived quantities of the written cell (c-2) -- the next stage's input: derive3_kernel's operations -- and its
-    // wave speeds (c-4), which share every sub-expression with them
-    const double rr = drcp(o[F_RHO]);
-    const double vx = o[F_MX] * rr, vy = o[F_MY] * rr, vz = o[F_MZ] * rr;
-    const double B2 = fma(o[F_BZ], o[F_BZ], fma(o[F_BY], o[F_BY], o[F_BX] * o[F_BX]));
-    const double eps = (o[F_E] - 0.5 * fma(o[F_MZ], vz, fma(o[F_MY], vy, o[F_MX] * vx))) - 0.5 * B2;
-    a.der.p[0][q] = vx; a.der.p[1][q] = vy; a.der.p[2][q] = vz; a.der.p[3][q] = eps;
-    const double pk = (a.prm.gamma - 1.0) * eps;
-    const double a2 = (a.prm.gamma * pk) * rr;
-    const double b2 = B2 * rr;
-    wsm[3] = a2 > 0.0 ? a2 : 0.0;
-    wsm[4] = b2 > 0.0 ? b2 : 0.0;
-    if (WS == WS_FULL) {
-      const double s = a2 + b2;
-      const double fa = (4.0 * a2) * rr;
-      const double vv[3] = {vx, vy, vz};
-      const double bb[3] = {o[F_BX], o[F_BY], o[F_BZ]};
-#pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        const double disc = fma(s, s, -(fa * (bb[d] * bb[d])));
-        const double cf2 = 0.5 * (s + sqrt(disc > 0.0 ? disc : 0.0));
-        const double cc = fabs(vv[d]) + sqrt(cf2);
-        wsm[d] = cc > 0.0 ? cc : 0.0;
-      }
-    }
+    finish_cell<COMBINE, WS, HD>(a, q, R, wsm);
   }
-  // block maximum (warp shuffles), one atomicMax per value and CTA; NaNs never enter (x > 0 ? x : 0)
-  const int lane = tid & 31, wid = tid >> 5;
-  constexpr int FROM = WS == WS_FULL ? 0 : 3;
+  block_max5_atomic<WS, 4>(wsm, sh, tid, a.sc->red[a.red_out]);
+}
+
+// Fused form of the two kernels above (SMAUG3_PARAM_KERNEL = 1, the default): a CTA owns a tile of TX x TY x TZ cells and,
+// one direction at a time (z, y, x: the nesting order of the sum), evaluates C_d = F_d - G_d on the tile extended by two
+// cells along d into shared memory, takes the central difference from there and folds it into R -- the 21 C_d volumes
+// never exist in HBM.  The halo cells repeat (TX+4)/TX, (TY+4)/TY, (TZ+4)/TZ of the flux evaluations (1.7x for
+// 32 x 4 x 4), which are cheap; their loads are L1 / L2 hits.
+#ifndef SMAUG3_TY
+#define SMAUG3_TY 4
+#define SMAUG3_TZ 4
+#endif
+#ifndef SMAUG3_ZFAST
+#define SMAUG3_ZFAST 0      // 1: blockIdx.x runs over the z-tiles (then y, then x), so that CTAs resident at the same time are
+#endif                      //    neighbours along z and y (measured: 3.21 vs 3.11 ms per stage at 256^3 -- no gain; off)
+constexpr int TX = 32, TY = SMAUG3_TY, TZ = SMAUG3_TZ, TT = TX * TY * TZ;
+constexpr int cmax3(int a, int b, int c) { return a > b ? (a > c ? a : c) : (b > c ? b : c); }
+constexpr int TEXT = cmax3((TX + 4) * TY * TZ, TX * (TY + 4) * TZ, TX * TY * (TZ + 4));      // cells of the largest extended tile
+constexpr size_t STAGE3_SMEM = (size_t)(NPHI * TEXT + 5 * (TT / 32)) * sizeof(double);
+
+template <int D, bool HD>
+__device__ __forceinline__ void tile_cflux(const AsmArgs& a, const CV4 (&km)[3], int x0, int y0, int z0, int tid, double* sC) {
+  constexpr int L1 = D == 0 ? 1 : 0, L2 = D == 2 ? 1 : 2;
+  constexpr int NE = D == 0 ? (TX + 4) * TY * TZ : (D == 1 ? TX * (TY + 4) * TZ : TX * TY * (TZ + 4));
+  const Grid3& g = a.g;
+  for (int e = tid; e < NE; e += TT) {
+    int i, j, k;
+    if (D == 0) { i = e % (TX + 4) - 2; j = (e / (TX + 4)) % TY; k = e / ((TX + 4) * TY); }
+    else if (D == 1) { i = e % TX; j = (e / TX) % (TY + 4) - 2; k = e / (TX * (TY + 4)); }
+    else { i = e % TX; j = (e / TX) % TY; k = e / (TX * TY) - 2; }
+    const int c[3] = {x0 + i, y0 + j, z0 + k};
+    bool ok = true;
 #pragma unroll
-  for (int v = FROM; v < 5; ++v) {
-    const double m = warp_max(wsm[v]);
-    if (lane == 0) sh[v * 4 + wid] = m;
+    for (int ax = 0; ax < 3; ++ax) ok = ok && (ax == D ? (c[ax] >= -2 && c[ax] < g.n[ax] + 2) : (c[ax] >= 0 && c[ax] < g.n[ax]));
+    if (!ok) continue;
+    const long long q = addr3(g, c[0], c[1], c[2]);
+    CellVals u;
+    load_cell(a.prm, a.in, a.der, q, u);
+    double F[NPHI];
+    cflux_dir<D, HD>(g, u, a.in, a.der, km[L1], km[L2], q, F);
+#pragma unroll
+    for (int f = 0; f < NPHI; ++f) sC[f * TEXT + e] = F[f];
+  }
+}
+
+struct KmIn { CV4 km[3]; };
+
+template <int COMBINE, int WS, bool HD>
+__global__ void __launch_bounds__(TT, 1024 / TT) stage3_kernel(const AsmArgs a, const KmIn kin) {
+  extern __shared__ __align__(16) double sm3[];
+  double* const sC = sm3;
+  double* const sh = sm3 + NPHI * TEXT;
+  const Grid3& g = a.g;
+  const int tx = threadIdx.x, ty = threadIdx.y, tz = threadIdx.z;
+  const int tid = (tz * TY + ty) * TX + tx;
+  const int x0 = (SMAUG3_ZFAST ? blockIdx.z : blockIdx.x) * TX, y0 = blockIdx.y * TY, z0 = (SMAUG3_ZFAST ? blockIdx.x : blockIdx.z) * TZ;
+  const int i = x0 + tx, j = y0 + ty, k = z0 + tz;
+  const bool cell = i < g.n[0] && j < g.n[1] && k < g.n[2];
+  double R[NF];
+  // z: T = cd_z (1/dz)
+  tile_cflux<2, HD>(a, kin.km, x0, y0, z0, tid, sC);
+  __syncthreads();
+  {
+    const double* p = sC + ((tz + 2) * TY + ty) * TX + tx;
+    constexpr int S = TX * TY;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int slot = f < F_BX ? f : bslot(f - F_BX, 2);
+      const double cd = slot < 0 ? 0.0 : cd12v(p[slot * TEXT - 2 * S], p[slot * TEXT - S], p[slot * TEXT + S], p[slot * TEXT + 2 * S]);
+      R[f] = cd * a.prm.inv_d[2];
+    }
   }
   __syncthreads();
-  if (tid < 5 && tid >= FROM) {
-    double m = sh[tid * 4];
-    for (int w2 = 1; w2 < 4; ++w2) m = sh[tid * 4 + w2] > m ? sh[tid * 4 + w2] : m;
-    atomicMax(&a.sc->red[a.red_out][tid], (unsigned long long)__double_as_longlong(m));
+  // y: T = fma(cd_y, 1/dy, T)
+  tile_cflux<1, HD>(a, kin.km, x0, y0, z0, tid, sC);
+  __syncthreads();
+  {
+    const double* p = sC + (tz * (TY + 4) + ty + 2) * TX + tx;
+    constexpr int S = TX;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int slot = f < F_BX ? f : bslot(f - F_BX, 1);
+      const double cd = slot < 0 ? 0.0 : cd12v(p[slot * TEXT - 2 * S], p[slot * TEXT - S], p[slot * TEXT + S], p[slot * TEXT + 2 * S]);
+      R[f] = fma(cd, a.prm.inv_d[1], R[f]);
+    }
   }
+  __syncthreads();
+  // x: R = fma(cd_x, 1/dx, T) (-1/12)
+  tile_cflux<0, HD>(a, kin.km, x0, y0, z0, tid, sC);
+  __syncthreads();
+  double wsm[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (cell) {
+    const double* p = sC + (tz * TY + ty) * (TX + 4) + tx + 2;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int slot = f < F_BX ? f : bslot(f - F_BX, 0);
+      const double cd = slot < 0 ? 0.0 : cd12v(p[slot * TEXT - 2], p[slot * TEXT - 1], p[slot * TEXT + 1], p[slot * TEXT + 2]);
+      R[f] = fma(cd, a.prm.inv_d[0], R[f]) * (-1.0 / 12.0);
+    }
+    finish_cell<COMBINE, WS, HD>(a, addr3(g, i, j, k), R, wsm);
+  }
+  block_max5_atomic<WS, TT / 32>(wsm, sh, tid, a.sc->red[a.red_out]);
 }
 
 // standalone reduction of all five maxima over the interior (set_state)
@@ -556,7 +687,9 @@ struct Ctx {
   double grav[3] = {0.0, 0.0, 0.0};
   double* mem = nullptr;        // one allocation: all volumes
   V8 buf[4];                    // w^n / state, w1 -> w3, w2, accumulator
-  V4 der;
+  V4 der[2];                    // derived quantities: of the current stage input (dcur) and of its output
+  int dcur = 0;
+  int fused = 1;                // SMAUG3_PARAM_KERNEL: 1 fused cflux + assembly (stage3_kernel), 0 multi-pass
   V7 phi[3], cf[3];
   V4 km[3];
   Scalars3* sc = nullptr;
@@ -570,7 +703,7 @@ struct Ctx {
   long long nk[5] = {0, 0, 0, 0, 0};
 };
 
-constexpr int NVOL = 4 * NF + NDER + 3 * (NPHI + NPHI + NKM);      // 32 + 4 + 54 = 90 padded volumes
+constexpr int NVOL = 4 * NF + 2 * NDER + 3 * (NPHI + NPHI + NKM);      // 32 + 8 + 54 = 94 padded volumes
 
 int make_grid(int nx, int ny, int nz, const int bc[6], Grid3& g) {
   g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
@@ -629,7 +762,7 @@ void launch_ghost(Ctx& c, const V8& w8, int freeze) {
   const Grid3& g = c.g;
   V12 w;
   for (int f = 0; f < NF; ++f) w.p[f] = w8.p[f];
-  for (int f = 0; f < 4; ++f) w.p[NF + f] = c.der.p[f];
+  for (int f = 0; f < 4; ++f) w.p[NF + f] = c.der[c.dcur].p[f];
   ghost3_kernel<2><<<grid_for(g.n[0] + 6, g.n[1] + 6, 6), 128, 0, c.stream>>>(g, w, freeze);
   ghost3_kernel<1><<<grid_for(g.n[0] + 6, 6, g.n[2]), 128, 0, c.stream>>>(g, w, freeze);
   ghost3_kernel<0><<<dim3((unsigned)((6 * g.n[1] + 127) / 128), (unsigned)g.n[2], 1), 128, 0, c.stream>>>(g, w, freeze);
@@ -641,7 +774,7 @@ void launch_kappa(Ctx& c, const Params3& p, const V8& in, int red_in) {
   const Grid3& g = c.g;
   KappaOut o;
   for (int d = 0; d < 3; ++d) { o.phi[d] = c.phi[d]; o.km[d] = c.km[d]; }
-  kappa3_kernel<<<sgrid_for(g.n[0] + 4, g.n[1] + 4, g.n[2] + 4), SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), c.sc, red_in, o);
+  kappa3_kernel<<<sgrid_for(g.n[0] + 4, g.n[1] + 4, g.n[2] + 4), SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der[c.dcur]), c.sc, red_in, o);
 }
 
 void launch_cflux(Ctx& c, const Params3& p, const V8& in) {
@@ -650,14 +783,29 @@ void launch_cflux(Ctx& c, const Params3& p, const V8& in) {
   CfluxIO io;
   for (int d = 0; d < 3; ++d) { io.km[d] = cv4(c.km[d]); io.cf[d] = c.cf[d]; }
   const dim3 gr = sgrid_for(g.n[0] + 4, g.n[1] + 4, g.n[2] + 4);
-  if (c.hd_on) cflux3_kernel<true><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), io);
-  else cflux3_kernel<false><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der), io);
+  if (c.hd_on) cflux3_kernel<true><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der[c.dcur]), io);
+  else cflux3_kernel<false><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der[c.dcur]), io);
 }
 
 template <int COMBINE, int WS>
 void launch_assemble(Ctx& c, const AsmArgs& a) {
   Timed t(c, 4);
   const Grid3& g = c.g;
+  if (c.fused) {
+    KmIn kin;
+    for (int d = 0; d < 3; ++d) kin.km[d] = cv4(c.km[d]);
+    const unsigned gx = (unsigned)((g.n[0] + TX - 1) / TX), gz = (unsigned)((g.n[2] + TZ - 1) / TZ);
+    const dim3 gr(SMAUG3_ZFAST ? gz : gx, (unsigned)((g.n[1] + TY - 1) / TY), SMAUG3_ZFAST ? gx : gz);
+    const dim3 bl(TX, TY, TZ);
+    if (c.hd_on) {
+      cudaFuncSetAttribute(stage3_kernel<COMBINE, WS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE3_SMEM);
+      stage3_kernel<COMBINE, WS, true><<<gr, bl, STAGE3_SMEM, c.stream>>>(a, kin);
+    } else {
+      cudaFuncSetAttribute(stage3_kernel<COMBINE, WS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE3_SMEM);
+      stage3_kernel<COMBINE, WS, false><<<gr, bl, STAGE3_SMEM, c.stream>>>(a, kin);
+    }
+    return;
+  }
   const dim3 gr = sgrid_for(g.n[0], g.n[1], g.n[2]);
   if (c.hd_on) assemble3_kernel<COMBINE, WS, true><<<gr, SBLOCK, 0, c.stream>>>(a);
   else assemble3_kernel<COMBINE, WS, false><<<gr, SBLOCK, 0, c.stream>>>(a);
@@ -668,12 +816,13 @@ void stage(Ctx& c, int in, int base, int out, int combine, int ws, double coef, 
   const Params3 p = params(c);
   launch_ghost(c, c.buf[in], 0);        // (the derived quantities of `in` were written by the stage that produced it)
   if (c.hd_on) launch_kappa(c, p, c.buf[in], red_in);
-  launch_cflux(c, p, c.buf[in]);
+  if (!c.fused) launch_cflux(c, p, c.buf[in]);
   AsmArgs a;
   a.g = c.g;
   a.prm = p;
   for (int d = 0; d < 3; ++d) { a.cf[d] = cv7(c.cf[d]); a.phi[d] = cv7(c.phi[d]); }
-  a.der = c.der;
+  a.der = cv4(c.der[c.dcur]);
+  a.der_out = c.der[c.dcur ^ 1];
   a.in = cv8(c.buf[in]);
   a.base = cv8(c.buf[base]);
   a.acc_in = cv8(c.buf[3]);
@@ -686,6 +835,7 @@ void stage(Ctx& c, int in, int base, int out, int combine, int ws, double coef, 
   else if (combine == COMBINE_BASE) launch_assemble<COMBINE_BASE, WS_FULL>(c, a);
   else if (combine == COMBINE_ACC) launch_assemble<COMBINE_ACC, WS_VT>(c, a);
   else launch_assemble<COMBINE_FINAL, WS_FULL>(c, a);
+  c.dcur ^= 1;        // the derived quantities of `out` are now the current ones
 }
 
 void enqueue_step(Ctx& c, double cfl) {
@@ -761,7 +911,8 @@ int smaug3_create(int nx, int ny, int nz, double gamma, const int bc[6], void* s
   auto take = [&]() { double* r = p; p += c->g.vol; return r; };
   for (int b = 0; b < 4; ++b)
     for (int f = 0; f < NF; ++f) c->buf[b].p[f] = take();
-  for (int f = 0; f < NDER; ++f) c->der.p[f] = take();
+  for (int b = 0; b < 2; ++b)
+    for (int f = 0; f < NDER; ++f) c->der[b].p[f] = take();
   for (int d = 0; d < 3; ++d) {
     for (int f = 0; f < NPHI; ++f) c->phi[d].p[f] = take();
     for (int f = 0; f < NPHI; ++f) c->cf[d].p[f] = take();
@@ -799,6 +950,7 @@ int smaug3_set_param(smaug3_ctx* ctx, int key, double v) {
     case SMAUG3_PARAM_GX: if (!std::isfinite(v)) break; c.grav[0] = v; return SMAUG3_OK;
     case SMAUG3_PARAM_GY: if (!std::isfinite(v)) break; c.grav[1] = v; return SMAUG3_OK;
     case SMAUG3_PARAM_GZ: if (!std::isfinite(v)) break; c.grav[2] = v; return SMAUG3_OK;
+    case SMAUG3_PARAM_KERNEL: if (v != 0 && v != 1) break; c.fused = (int)v; return SMAUG3_OK;
     default: return fail(SMAUG3_EINVAL, "unknown parameter key");
   }
   return fail(SMAUG3_EINVAL, "parameter value out of range");
@@ -819,7 +971,10 @@ int smaug3_set_state(smaug3_ctx* ctx, const void* w) {
   launch_ghost(c, c.buf[0], 1);
   {
     Timed t(c, 1);     // derived quantities on every padded cell, once (afterwards the stage epilogues keep them current)
-    derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[0]), c.der);
+    // (both sets: the frozen ghosts of fixed sides are never written again)
+    derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[0]), c.der[0]);
+    derive3_kernel<<<grid_for(g.n[0] + 6, g.n[1] + 6, g.n[2] + 6), 128, 0, c.stream>>>(g, cv8(c.buf[0]), c.der[1]);
+    ++c.launches;
   }
   // the other two buffers that are read with a halo get the same frozen ghosts (fixed sides are never rewritten)
   for (int b = 1; b <= 2; ++b)

@@ -55,29 +55,35 @@ def check(a, ta, wsa, b, tb, wsb):
 
 @pytest.mark.parametrize("shape,steps", [((24, 20, 150), 6), ((9, 130, 33), 5), ((40, 7, 5), 5), ((64, 64, 64), 10)])
 def test_orszag_tang_3d_parity(gpu, oracle_mod, shape, steps):
-    """several 128-thread blocks along x plus a ragged tail; thin and thick axes; the bench workload's shape family"""
+    """several thread blocks / tiles along every axis plus ragged tails; thin and thick axes; both kernel forms"""
     nz, ny, nx = shape
     w, bc, gamma = si.orszag_tang_3d(nx, ny, nz)
-    check(*gpu_run(gpu, w, bc, gamma, steps), *cpu_run(oracle_mod, w, bc, gamma, steps))
+    ref = cpu_run(oracle_mod, w, bc, gamma, steps)
+    check(*gpu_run(gpu, w, bc, gamma, steps), *ref)
+    check(*gpu_run(gpu, w, bc, gamma, steps, kernel=0), *ref)
 
 
+@pytest.mark.parametrize("kernel", [1, 0])
 @pytest.mark.parametrize("bc", [(P, P, O, O, F, F), (O, F, P, P, O, O), (F, F, F, F, F, F), (O, O, O, O, P, P)])
-def test_boundary_kinds_3d(gpu, oracle_mod, bc):
+def test_boundary_kinds_3d(gpu, oracle_mod, bc, kernel):
     """open / fixed / periodic mixes on six sides, edges and corners included (a smooth state is not periodic-compatible
     with them, so the boundaries are active from the first step)"""
     L = (1.0, 0.8, 0.6)
     w, _, gamma = si.smooth_random_3d(37, 22, 14, seed=5, amp=4e-2, lengths=L)
     kw = dict(lx=L[0], ly=L[1], lz=L[2])
-    check(*gpu_run(gpu, w, bc, gamma, 8, **kw), *cpu_run(oracle_mod, w, bc, gamma, 8, **kw))
+    check(*gpu_run(gpu, w, bc, gamma, 8, kernel=kernel, **kw), *cpu_run(oracle_mod, w, bc, gamma, 8, **kw))
 
 
 @pytest.mark.parametrize("params", [dict(hd_on=0), dict(rk_order=2), dict(rk_order=1), dict(gx=0.3, gy=-0.2, gz=0.5),
                                     dict(c_rho=0.05, c_mom=0.2, c_e=0.01, c_b=0.08), dict(fixed_dt=2e-4),
                                     dict(hd_on=0, rk_order=2, gz=-1.0)])
 def test_parameters_3d(gpu, oracle_mod, params):
+    """every parameter in both kernel forms (SMAUG3_PARAM_KERNEL: 1 = fused tile kernel, 0 = C_d volumes in HBM)"""
     w, bc, gamma = si.smooth_random_3d(30, 18, 12, seed=17, amp=5e-2)
     bc = (P, P, O, O, P, P) if "gz" in params else bc
-    check(*gpu_run(gpu, w, bc, gamma, 7, **params), *cpu_run(oracle_mod, w, bc, gamma, 7, **params))
+    ref = cpu_run(oracle_mod, w, bc, gamma, 7, **params)
+    for kernel in (1, 0):
+        check(*gpu_run(gpu, w, bc, gamma, 7, kernel=kernel, **params), *ref)
 
 
 @pytest.mark.parametrize("shape", [(1, 40, 60), (1, 1, 200), (3, 1, 50), (50, 1, 1), (2, 2, 2)])
