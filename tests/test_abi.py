@@ -38,7 +38,7 @@ def test_library_exports_every_symbol_of_the_3d_header():
     h = C.c_void_p()
     bc = (C.c_int * 6)(0, 0, 0, 0, 0, 0)
     assert L.smaug3_workspace_bytes(0, 4, 4) == 0
-    assert 14e9 < L.smaug3_workspace_bytes(256, 256, 256) < 14.5e9          # 90 padded volumes of 288 x 262 x 262 doubles
+    assert 14.5e9 < L.smaug3_workspace_bytes(256, 256, 256) < 15.2e9        # 94 padded volumes of 288 x 262 x 262 doubles
     assert L.smaug3_create(0, 4, 4, 1.4, bc, None, C.byref(h)) == pkg.EINVAL
     assert L.smaug3_create(4, 4, 4, 1.0, bc, None, C.byref(h)) == pkg.EINVAL
     assert L.smaug3_create(4, 4, 4, 1.4, (C.c_int * 6)(0, 0, 0, 0, 0, 1), None, C.byref(h)) == pkg.EINVAL
