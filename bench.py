@@ -388,6 +388,7 @@ def run_3d(args):
     stage_ms = sum(v[0] for v in kinds.values()) / (K * stages)
     achieved = bpcu / stages * cells / (stage_ms * 1e-3) / 1e9
     top = max(kinds, key=lambda k: kinds[k][0])
+    cap = ncu_capture(name + ("_nohd" if args.no_hd else "") + ("_rk%d" % args.rk_order if args.rk_order != 4 else ""))
     line = {
         "metric": METRIC, "value": cells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -397,7 +398,8 @@ def run_3d(args):
                    "l2": "working set >> L2, no flush needed" if cells * 64 > 4e8 else "working set comparable to L2 (126 MB)"},
         "hbm_gbs_algorithmic": cells * K / (ms * 1e-3) * bpcu / 1e9,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "frac_of_nominal_8TBs": achieved / 8000.0, "traffic": None, "peak_source": peak_src,
+                     "frac_of_nominal_8TBs": achieved / 8000.0, "traffic": cap.get("dram_bytes"),
+                     "traffic_source": cap.get("capture"), "peak_source": peak_src,
                      "kernel": "smaug3 RK stage (ghost3, kappa3, stage3); "
                                f"largest share: {top}",
                      "bytes_per_launch": bpcu / stages * cells, "avg_launch_ms": stage_ms,
