@@ -75,8 +75,9 @@ int smaug3_set_param(smaug3_ctx* ctx, int key, double value);
 int smaug3_set_state(smaug3_ctx* ctx, const void* w);
 
 /* Advance n_steps time steps with dt = cfl min_d(Delta_d / cmax_d) (or the fixed dt): per step one dt launch and,
- * per RK stage, ghost fill -> derived quantities -> kappa / interface fluxes along x, y, z -> cell-centred fluxes
- * C_d = F_d - G_d -> assembly, RK combine and wave-speed reduction (five kernels).  dt and the maxima stay on the device.
+ * per RK stage, ghost fill (state and derived quantities) -> kappa / interface fluxes along x, y, z -> cell-centred
+ * fluxes C_d = F_d - G_d, assembly, RK combine, derived quantities of the result and wave-speed reduction (one tile
+ * kernel; SMAUG3_PARAM_KERNEL = 0: two kernels).  dt and the maxima stay on the device.
  * ENONFINITE if a time step was non-finite or <= 0. */
 int smaug3_step(smaug3_ctx* ctx, int n_steps, double cfl);
 
