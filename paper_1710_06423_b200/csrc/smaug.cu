@@ -343,21 +343,20 @@ int launch_split(smaug_ctx* c, const StageArgs& a) {
 }
 
 #ifndef SMAUG_FLUX_NT
-#define SMAUG_FLUX_NT 128
+#define SMAUG_FLUX_NT 0        // 0: strip width picked per grid (flux_strip_threads); 128 / 256: forced (tuning builds)
 #endif
-constexpr int FLUX_NT = SMAUG_FLUX_NT;
 
 // Streaming form without hyperdiffusion (smaug_flux_kernel.cuh): HD off, with (BG) or without a background.
-template <bool BG, bool GRAV = false>
+template <int NT, bool BG, bool GRAV>
 int launch_flux_t(smaug_ctx* c, const StageArgs& a) {
   static unsigned long long configured = 0;     // devices on which this instantiation has its smem limit raised
-  constexpr size_t smem = FluxSmem<FLUX_NT, BG>::BYTES;
-  auto kern = flux_kernel<FLUX_NT, BG, GRAV>;
+  constexpr size_t smem = FluxSmem<NT, BG>::BYTES;
+  auto kern = flux_kernel<NT, BG, GRAV>;
   CU(configure_smem(kern, smem, c->device, configured));
-  const int W = FLUX_NT - 4;
+  const int W = NT - 4;
   const int strips = (c->g.nx + W - 1) / W;
   MarchGeom mg;
-  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * FluxSmem<FLUX_NT, BG>::CTAS_PER_SM, 4);
+  mg.rows_per_cta = pick_rows_per_cta(c->g.ny, strips, c->n_sm * FluxSmem<NT, BG>::CTAS_PER_SM, 4);
   const int nchunks = (c->g.ny + mg.rows_per_cta - 1) / mg.rows_per_cta;
   dim3 grid(strips, nchunks);
   c->last_ctas = strips * nchunks;
@@ -367,16 +366,37 @@ int launch_flux_t(smaug_ctx* c, const StageArgs& a) {
     e1 = c->ev[c->ev_used++];
     CU(cudaEventRecord(e0, c->stream));
   }
-  kern<<<grid, FLUX_NT, smem, c->stream>>>(a, mg);
+  kern<<<grid, NT, smem, c->stream>>>(a, mg);
   if (e1) CU(cudaEventRecord(e1, c->stream));
   c->launches++;
   CU(cudaGetLastError());
   return SMAUG_OK;
 }
 
+// Strip width of the streaming kernel without HD: 256 threads (two CTAs per SM) or 128 (four; three with a background).
+// Modelled efficiency of a width = useful columns of its strips x useful rows of its chunks x filled CTA slots of its
+// waves; the wide strip gets the 5 % it measures better at equal geometry (fewer halo columns, longer coalesced rows).
+// Measured, HD off, ms per stage (128 / 256): 8000^2 1.70 / 1.66, 4000^2 0.451 / 0.435, 2044^2 0.126 / 0.175, 1000^2 0.0439 / 0.0396.
+double flux_geometry_efficiency(const smaug_ctx* c, int nt, int ctas_per_sm) {
+  const int W = nt - 4, strips = (c->g.nx + W - 1) / W, slots = c->n_sm * ctas_per_sm;
+  const int rows = pick_rows_per_cta(c->g.ny, strips, slots, 4);
+  const int nchunks = (c->g.ny + rows - 1) / rows;
+  const long long ctas = (long long)strips * nchunks, waves = (ctas + slots - 1) / slots;
+  return ((double)c->g.nx / ((double)strips * W)) * ((double)rows / (rows + 4)) * ((double)ctas / ((double)waves * slots));
+}
+int flux_strip_threads(const smaug_ctx* c) {
+  if (SMAUG_FLUX_NT != 0) return SMAUG_FLUX_NT;
+  const double e128 = flux_geometry_efficiency(c, 128, c->has_bg ? 3 : 4), e256 = 1.05 * flux_geometry_efficiency(c, 256, 2);
+  return e256 >= e128 ? 256 : 128;
+}
+
 int launch_flux(smaug_ctx* c, const StageArgs& a) {
-  if (c->has_bg) return launch_flux_t<true>(c, a);
-  return a.prm.grav_on ? launch_flux_t<false, true>(c, a) : launch_flux_t<false>(c, a);
+  if (flux_strip_threads(c) == 256) {
+    if (c->has_bg) return launch_flux_t<256, true, false>(c, a);
+    return a.prm.grav_on ? launch_flux_t<256, false, true>(c, a) : launch_flux_t<256, false, false>(c, a);
+  }
+  if (c->has_bg) return launch_flux_t<128, true, false>(c, a);
+  return a.prm.grav_on ? launch_flux_t<128, false, true>(c, a) : launch_flux_t<128, false, false>(c, a);
 }
 
 // The streaming kernels cover every configuration; the tiled kernel runs when SMAUG_PARAM_KERNEL = 0 (tests), and
@@ -898,8 +918,10 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
   if (uses_line(c)) {                                      // small-grid path: one cluster of tiles, whole steps per launch
     out[0] = LINE_W; out[1] = 1; out[2] = LINE_NT; out[3] = (int)LineSmem::BYTES;
   } else if (uses_flux(c)) {                               // streaming kernel without HD: a strip of NT-4 columns
-    out[0] = FLUX_NT - 4; out[1] = 1; out[2] = FLUX_NT;
-    out[3] = (int)(c->has_bg ? FluxSmem<FLUX_NT, true>::BYTES : FluxSmem<FLUX_NT>::BYTES);
+    const int nt = flux_strip_threads(c);
+    out[0] = nt - 4; out[1] = 1; out[2] = nt;
+    out[3] = nt == 256 ? (int)(c->has_bg ? FluxSmem<256, true>::BYTES : FluxSmem<256>::BYTES)
+                       : (int)(c->has_bg ? FluxSmem<128, true>::BYTES : FluxSmem<128>::BYTES);
   } else if (uses_split(c)) {   // role-split streaming kernel: a strip of NC-8 columns
     out[0] = SPLIT_NC - 8; out[1] = 1; out[2] = SPLIT_NC + SPLIT_NC / 2;
     out[3] = (int)(c->has_bg ? SplitSmem<SPLIT_NC, true>::BYTES : SplitSmem<SPLIT_NC>::BYTES);
@@ -920,7 +942,7 @@ int smaug_get_kernel_info(smaug_ctx* c, int out[5]) {
 const char* smaug_get_kernel_name(smaug_ctx* c) {
   if (!c) return "?";
   if (uses_line(c)) return "line_step_kernel<128>";
-  if (uses_flux(c)) return FLUX_NT == 128 ? "flux_kernel<128>" : "flux_kernel";
+  if (uses_flux(c)) return flux_strip_threads(c) == 256 ? "flux_kernel<256>" : "flux_kernel<128>";
   if (uses_split(c)) return SPLIT_NC == 128 ? "split_kernel<128>" : "split_kernel";
   if (uses_march(c)) return "march_kernel<256>";
   return TW == 32 && TH == 8 && NT == 512 ? "stage_kernel<32,8,512>" : "stage_kernel";

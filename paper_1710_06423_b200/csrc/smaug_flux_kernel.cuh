@@ -10,13 +10,19 @@
 //   -- one __syncthreads per row --
 //   tail: central x-difference of F_x(j) from the ring (neighbour columns), central y-difference of F_y from
 //         the history, R, RK combine, coalesced store, wave-speed maxima.
-// Input rows arrive DEPTH - 1 rows ahead through cp.async into a thread-private ring (no registers held, about
-// 3 x 48 bytes per thread in flight); the RK operands of the tail row are plain loads issued at the top of the
+// Input rows arrive DEPTH - 1 rows ahead through cp.async into a thread-private ring (no registers held, 48 bytes
+// per thread and row in flight); the RK operands of the tail row are plain loads issued at the top of the
 // step.  The 4 halo columns of a strip and the 4 warm-up rows of a chunk hit L2; the pointwise re-read of the stage
 // input at the tail row (stages 2 and 4) misses it in part (DRAM traffic 1.08 x the algorithmic bytes, see L2HINT).
 #pragma once
 #include "smaug_split_kernel.cuh"
 
+#ifndef SMAUG_FLUX_DEPTH
+#define SMAUG_FLUX_DEPTH 2      // landing-ring rows.  Measured at 8000^2, HD off, ms per stage (NT = strip threads x CTAs per SM):
+#endif                          // 128 x 4: depth 4 1.83, 3 1.74, 2 1.70;  256 x 2: depth 3 1.68, 2 1.66 (chosen);  512 x 1: 1.72.
+                                // The shallow ring wins: what the kernel gains is shared memory handed back to L1 (the halo
+                                // columns, the warm-up rows and the pointwise re-read of the tail row hit there), not bytes in
+                                // flight.  Background form (stratified 4000^2): 128 x 3, depth 4 0.906 -> 256 x 2, depth 2 0.661.
 #ifndef SMAUG_FLUX_L2HINT
 #define SMAUG_FLUX_L2HINT 0     // 1: L2 eviction priorities -- in stages 2 and 4 the stage-input rows (read with their halo by the
 #endif                          // cp.async ring and once more pointwise two rows later) are fetched with evict_last, RK operands and
@@ -56,7 +62,7 @@ __device__ __forceinline__ void st_hint(double* p, double v, unsigned long long 
 // the energy source S_e (their y-derivatives come from a five-row register history), gravity is three fmas (c-10).
 template <int NT, bool BG = false>
 struct FluxSmem {
-  static constexpr int DEPTH = 4;                         // input rows in the landing ring
+  static constexpr int DEPTH = SMAUG_FLUX_DEPTH;           // input rows in the landing ring (DEPTH - 1 rows in flight)
   static constexpr int NIN = BG ? NF + NBG : NF;          // fields per landing row
   static constexpr int OFF_FXR = 0;                       // ring 4 rows x 5 planes: F_x
   static constexpr int OFF_VXR = OFF_FXR + 4 * 5 * NT;    // BG: ring 4 rows x 2 planes: vx, vy
