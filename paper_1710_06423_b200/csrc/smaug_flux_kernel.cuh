@@ -294,14 +294,18 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
           for (int f = 0; f < NF; ++f) ST_ONCE(a.acc_out.p[f] + gj, fma(2.0, o[f], jin[f] - jbase[f]));
         }
         if (ws_mode != WS_NONE) {
-          double w4[4];
-          if constexpr (BG)
-            cell_wavespeeds(jrb + o[F_RHO], o[F_MX], o[F_MY], jeb + o[F_E], jBbx + o[F_BX], jBby + o[F_BY], gamma,
-                            ws_mode == WS_FULL, w4);
-          else
-            cell_wavespeeds(o[F_RHO], o[F_MX], o[F_MY], o[F_E], o[F_BX], o[F_BY], gamma, ws_mode == WS_FULL, w4);
+          // split_wavespeeds (smaug_split_kernel.cuh): the same maxima, candidates entering with `c > m ? c : m`, and in
+          // the last stage the two fast speeds only where they can still raise the thread's running maximum
+          double ot[NF];
+          if constexpr (BG) {
+            ot[F_RHO] = jrb + o[F_RHO]; ot[F_MX] = o[F_MX]; ot[F_MY] = o[F_MY]; ot[F_E] = jeb + o[F_E];
+            ot[F_BX] = jBbx + o[F_BX]; ot[F_BY] = jBby + o[F_BY];
+          } else {
 #pragma unroll
-          for (int k = 0; k < 4; ++k) wsmax[k] = dmax(wsmax[k], w4[k]);
+            for (int f = 0; f < NF; ++f) ot[f] = o[f];
+          }
+          if (ws_mode == WS_FULL) split_wavespeeds<WS_FULL>(ot, gamma, wsmax, wsmax[0], wsmax[1]);
+          else split_wavespeeds<WS_VT>(ot, gamma, wsmax, 0.0, 0.0);
         }
       }
       gj += upitch;
