@@ -301,6 +301,8 @@ def run_ours(args):
                          "frac": (achieved / peak) if achieved else None,
                          "frac_of_nominal_8TBs": (achieved / 8000.0) if achieved else None, "traffic": cap.get("dram_bytes"),
                          "traffic_source": cap.get("capture"),
+                         "traffic_bytes_per_cell_update": (cap["dram_bytes"] * stages / cells) if cap.get("dram_bytes") else None,
+                         "algorithmic_bytes_per_cell_update": bpcu,
                          "peak_source": peak_src, "kernel": f"smaug::{sim.kernel_name()} (fused RK stage)",
                          "bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_launch_ms,
                          "launches_timed": stage_n, "stage_kernel_share_of_step": stage_ms / ms,
