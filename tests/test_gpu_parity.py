@@ -138,6 +138,29 @@ def test_no_hyperdiffusion_streaming_kernel(gpu, oracle_mod, nx, ny, steps, para
     check(*a, *b)
 
 
+@pytest.mark.parametrize("nx,ny,want", [(250, 70, "flux_kernel<256>"), (300, 3000, "flux_kernel<128>"), (1100, 70, None)])
+@pytest.mark.parametrize("form", ["plain", "gravity", "background"])
+def test_no_hyperdiffusion_both_strip_widths(gpu, oracle_mod, nx, ny, want, form):
+    """flux_kernel picks its strip width per grid (256 threads x 2 CTAs per SM or 128 x 4, smaug.cu flux_strip_threads):
+    both widths, in the plain, gravity and background forms, against the oracle; a one-strip grid of 250 columns takes the
+    wide strip, 300 columns on a grid tall enough to fill the GPU (two wide strips would be 60 % full) the narrow one."""
+    import torch
+    if form == "background":
+        w, bc, gamma, bg, (gx, gy) = si.stratified_atmosphere(nx, ny)
+        params = dict(hd_on=0, gx=gx, gy=gy)
+    else:
+        w, bc, gamma = si.orszag_tang(nx, ny)
+        bg, params = None, dict(hd_on=0)
+        if form == "gravity":
+            bc, params = (0, 0, 1, 1), dict(hd_on=0, gx=0.2, gy=-0.6)
+    if want is not None and (form != "background" or ny >= 1000):      # (an under-filled GPU has no preferred width)
+        s = gpu.Smaug(nx, ny, gamma, bc, bg=None if bg is None else torch.from_numpy(bg), **params)
+        assert s.kernel_name() == want, s.kernel_name()
+        s.close()
+    steps = 9 if ny < 1000 else 4
+    check(*gpu_run(gpu, w, bc, gamma, steps, bg=bg, **params), *cpu_run(oracle_mod, w, bc, gamma, steps, bg=bg, threads=16, **params))
+
+
 def test_no_hyperdiffusion_open_and_fixed_boundaries(gpu, oracle_mod):
     w, bc, gamma = si.brio_wu(200, 12)
     a = gpu_run(gpu, w, bc, gamma, 40, hd_on=0, cfl=0.2)
