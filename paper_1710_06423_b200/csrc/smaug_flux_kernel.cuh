@@ -87,7 +87,10 @@ __global__ void __launch_bounds__(NT, FluxSmem<NT, BG>::CTAS_PER_SM) flux_kernel
   constexpr int W = NT - 4;
   const int x0 = blockIdx.x * W;
   const int ci = x0 - 2 + tid;                            // interior column of this thread (>= -2: a ghost)
-  const int cl = min(ci, g.nx + NG - 1);                  // clamped for loads
+  // column used for loads: lanes right of the padded plane (a partial last strip) produce nothing; they read the columns one
+  // strip width to their left -- distinct, coalesced addresses (hundreds of lanes clamped onto ONE address make cp.async
+  // crawl: 2044^2 with 256-thread strips 0.168 -> 0.126 ms per stage)
+  const int cl = ci <= g.nx + NG - 1 ? ci : max(ci - NT, -NG);
   const bool col_out = tid >= 2 && tid < NT - 2 && ci < g.nx;
   const int ystart = blockIdx.y * mg.rows_per_cta;
   const int yend = min(ystart + mg.rows_per_cta, g.ny);
