@@ -1,7 +1,7 @@
 // smaug_flux_kernel.cuh -- streaming fused stage kernel for the case WITHOUT hyperdiffusion ("Without HD" column of
 // the paper's Table 1): R = -(d^c_x F_x + d^c_y F_y) (+ the energy source and gravity in the BG / GRAV
 // forms, see FluxSmem below), RK combine, wave-speed maxima.  About 90 fp64 operations against 144 bytes per cell and stage: this case
-// sits on the memory side of the B200 ridge, so the kernel is built around bytes in flight, not arithmetic.
+// sits on the memory side of the B200 ridge: what counts is that every byte crosses HBM once (SMAUG_FLUX_DEPTH below).
 // Same arithmetic contract as every other stage kernel: bit-identical to the oracle.
 //
 // One CTA owns a strip of NT - 4 output columns (thread t <-> column x0 - 2 + t) and marches down a chunk of
@@ -12,8 +12,8 @@
 //         the history, R, RK combine, coalesced store, wave-speed maxima.
 // Input rows arrive DEPTH - 1 rows ahead through cp.async into a thread-private ring (no registers held, 48 bytes
 // per thread and row in flight); the RK operands of the tail row are plain loads issued at the top of the
-// step.  The 4 halo columns of a strip and the 4 warm-up rows of a chunk hit L2; the pointwise re-read of the stage
-// input at the tail row (stages 2 and 4) misses it in part (DRAM traffic 1.08 x the algorithmic bytes, see L2HINT).
+// step.  The 4 halo columns of a strip, the 4 warm-up rows of a chunk and the pointwise re-read of the stage input at the
+// tail row (stages 2 and 4) hit L1 / L2: DRAM traffic 1.01 - 1.03 x the algorithmic bytes per stage.
 #pragma once
 #include "smaug_split_kernel.cuh"
 
