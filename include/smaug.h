@@ -161,6 +161,35 @@ int smaug_selftest_division(int exp_lo, int exp_hi, unsigned long long seed, lon
  * pipe is not saturated).  Errors: EINVAL, ECUDA.  tests/test_gpu_division.py prints and bounds both. */
 int smaug_selftest_fp64_pipe(int ilp, int warps_per_subpartition, int iters, double out[2]);
 
+/* ---- Wave-speed maxima without any device allocation --------------------------------------------------------------
+ * out = { max(|vx|+c_fx), max(|vy|+c_fy), max a^2, max b^2 } (c-4; "maximum wave speed") of a state the
+ * caller already holds on the device -- the numbers a CFL monitor or an output routine wants -- bit for bit what
+ * smaug_set_state + smaug_get_wavespeeds return for the same arrays.
+ *
+ * Who this is for: a caller that cannot call cudaMalloc, directly or through this library.  The usual cases are a
+ * process whose GPU memory belongs to somebody else's allocator (a framework's caching pool or a job-wide arena has
+ * reserved the device, so a raw cudaMalloc fails or breaks the memory budget) and a time-critical loop that must not
+ * take cudaMalloc / cudaFree's device-wide synchronisation.  The context route needs a workspace of some 24 padded
+ * planes (over 12 GB at 8000 x 8000) just to own four reduction slots; this call needs none: its working memory is a
+ * 524,544-byte array inside the library image, which every GPU that loads libsmaug.so holds until the process exits.
+ * It calls neither cudaMalloc nor cudaFree nor any routine that allocates.
+ *
+ * Arguments: w [6][ny][nx] and bg [4][ny][nx] (NULL = zero background) are DEVICE pointers in the layout above,
+ * out is a DEVICE pointer to 4 doubles; all three stay the caller's.  Host pointers are refused (SMAUG_EINVAL): there
+ * is nowhere to stage them.  The work is enqueued on `stream` (a cudaStream_t, NULL = default stream) of the CURRENT
+ * device and the call returns without waiting: out is valid once that stream reaches the end of the kernel.
+ * Limit: nx * ny <= SMAUG_WAVESPEEDS_STATIC_MAX_CELLS (the array holds four partial maxima per block of 4096 cells);
+ * larger grids are refused with SMAUG_EINVAL and a message that names the limit.
+ * First call on each device: looks up the array's device address (cudaGetSymbolAddress), so make that first call
+ * outside any stream capture; later calls on that device reuse the address.
+ * Sharing: all calls in the process use the same array, which keeps the last call's contents.  The one word that
+ * must start at zero is cleared on `stream` before each launch, so calls that are ordered on the GPU (one stream, or
+ * streams joined by events) are independent of each other; calls that can OVERLAP on the GPU race on the array and
+ * give undefined results -- serialise them.  Not for use from several host threads at once on one device either.
+ * As in smaug_get_wavespeeds, NaN and negative candidates are skipped (maxima start at 0). */
+#define SMAUG_WAVESPEEDS_STATIC_MAX_CELLS 67108864LL /* 16384 blocks x 4096 cells; 8000 x 8000 fits, 8192 x 8193 does not */
+int smaug_wavespeeds_static(int nx, int ny, double gamma, const double* w, const double* bg, double* out, void* stream);
+
 void smaug_destroy(smaug_ctx* ctx); /* NULL is a no-op */
 
 /* ---- Domain decomposition (SURVEY.md 8(f) NEXT-1; PAPER.md:25 Fig. 1, :55-59 "the full domain is divided into

@@ -31,13 +31,14 @@ def _sources():
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/smaug.cu and csrc/smaug3d.cu for sm_100a into libsmaug.so (in-tree) if missing or stale."""
+    """Compile csrc/smaug.cu, csrc/smaug3d.cu and csrc/smaug_static.cu for sm_100a into libsmaug.so (in-tree) if missing or stale."""
     newest = max(os.path.getmtime(p) for p in _sources() + [os.path.join(INCLUDE, "smaug.h"), os.path.join(INCLUDE, "smaug3d.h")])
     if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         extra = os.environ.get("SMAUG_NVCC_EXTRA", "").split()     # e.g. -DSMAUG_TW=24 for tuning sweeps
         cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
-              ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu"), os.path.join(_CSRC, "smaug3d.cu")]
+              ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu"), os.path.join(_CSRC, "smaug3d.cu"),
+               os.path.join(_CSRC, "smaug_static.cu")]
         subprocess.run(cmd, check=True)
     return LIB_PATH
 
@@ -84,6 +85,7 @@ def lib() -> C.CDLL:
         L.smaug_selftest_fp64_pipe.argtypes = [C.c_int, C.c_int, C.c_int, dp]
         L.smaug_destroy.argtypes = [vp]
         L.smaug_destroy.restype = None
+        L.smaug_wavespeeds_static.argtypes = [C.c_int, C.c_int, C.c_double, vp, vp, vp, vp]
         ip = C.POINTER(C.c_int)
         L.smaug_group_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, ip, vp, ip, C.POINTER(vp)]
         L.smaug_group_size.argtypes = [vp, ip, ip]
@@ -150,6 +152,32 @@ def selftest_fp64_pipe(ilp: int, warps_per_subpartition: int, iters: int = 2048)
     o = (C.c_double * 2)()
     _check(lib().smaug_selftest_fp64_pipe(int(ilp), int(warps_per_subpartition), int(iters), o))
     return o[0], o[1]
+
+
+WAVESPEEDS_STATIC_MAX_CELLS = 16384 * 4096     # SMAUG_WAVESPEEDS_STATIC_MAX_CELLS of include/smaug.h
+
+
+def wavespeeds_static(w, gamma, bg=None, out=None):
+    """smaug_wavespeeds_static: the four wave-speed maxima (c-4) of a cuda state tensor ``w[6, ny, nx]`` (and optional
+    background ``bg[4, ny, nx]``) without a context and without any device allocation by the library -- for callers
+    whose GPU memory is owned by another allocator or who must avoid cudaMalloc's synchronisation.  The library's
+    scratch is a fixed array inside libsmaug.so, shared by all calls: do not let two calls overlap on the GPU.
+
+    ``out`` is a 4-element float64 cuda tensor that receives the maxima; pass one you already own to keep torch from
+    allocating either (default: a new one).  Enqueued on torch's current stream of ``w``'s device; read ``out`` after
+    that stream has caught up (``out.cpu()`` does).  At most WAVESPEEDS_STATIC_MAX_CELLS cells."""
+    import torch
+    assert w.is_cuda and w.dim() == 3 and w.shape[0] == 6
+    ny, nx = int(w.shape[1]), int(w.shape[2])
+    if bg is not None:
+        assert bg.is_cuda and tuple(bg.shape) == (4, ny, nx)
+    with torch.cuda.device(w.device):
+        if out is None:
+            out = torch.empty(4, dtype=torch.float64, device=w.device)
+        assert out.is_cuda and out.numel() == 4
+        stream = torch.cuda.current_stream(w.device).cuda_stream
+        _check(lib().smaug_wavespeeds_static(nx, ny, float(gamma), _ptr(w), _ptr(bg), _ptr(out), C.c_void_p(stream)))
+    return out
 
 
 class Smaug:

@@ -658,6 +658,11 @@ int sync_and_status(smaug_ctx* c) {
 
 }  // namespace
 
+// For the library's other translation units (smaug_static.cu): leave a message where smaug_last_error() finds it.
+namespace smaug {
+__attribute__((visibility("hidden"))) int set_last_error(int code, const char* msg) { return fail(code, msg ? msg : ""); }
+}  // namespace smaug
+
 extern "C" {
 
 const char* smaug_last_error(void) { return g_err.c_str(); }

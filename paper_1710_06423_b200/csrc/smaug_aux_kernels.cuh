@@ -1,5 +1,6 @@
 // smaug_aux_kernels.cuh -- the small kernels of the step: ghost fill (c-8), standalone wave-speed
-// reduction (c-4), device-resident dt (c-7).  sm_100a, fp64.
+// reduction (c-4), device-resident dt (c-7).  sm_100a, fp64.  The non-template kernels are `static`: smaug.cu and
+// smaug_static.cu both include this header.
 #pragma once
 #include "smaug_device.cuh"
 
@@ -129,7 +130,7 @@ __device__ __forceinline__ void ghost_fill_plane(const Grid& g, double* p, int f
   }
 }
 
-__global__ void __launch_bounds__(256) ghost_fill_kernel(Grid g, Planes6 pl, int freeze) {
+static __global__ void __launch_bounds__(256) ghost_fill_kernel(Grid g, Planes6 pl, int freeze) {
   ghost_fill_plane(g, pl.p[blockIdx.y], freeze, (long long)blockIdx.x * blockDim.x + threadIdx.x,
                    (long long)gridDim.x * blockDim.x);
 }
@@ -161,12 +162,12 @@ __device__ __forceinline__ void dt_body(DeviceScalars* s, int state_set, unsigne
   }
 }
 
-__global__ void dt_kernel(DeviceScalars* s, int state_set, unsigned clear_sets, double cfl, double fixed_dt,
+static __global__ void dt_kernel(DeviceScalars* s, int state_set, unsigned clear_sets, double cfl, double fixed_dt,
                           double dx, double dy, int nx, int ny) {
   if (threadIdx.x == 0 && blockIdx.x == 0) dt_body(s, state_set, clear_sets, cfl, fixed_dt, dx, dy, nx, ny);
 }
 
-__global__ void clear_red_kernel(DeviceScalars* s, unsigned clear_sets) {
+static __global__ void clear_red_kernel(DeviceScalars* s, unsigned clear_sets) {
   if (threadIdx.x == 0 && blockIdx.x == 0)
     for (int k = 0; k < NRED; ++k)
       if (clear_sets & (1u << k)) {
