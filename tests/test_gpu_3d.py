@@ -94,6 +94,17 @@ def test_degenerate_axes_3d(gpu, oracle_mod, shape):
     check(*gpu_run(gpu, w, bc, gamma, 6), *cpu_run(oracle_mod, w, bc, gamma, 6))
 
 
+@pytest.mark.parametrize("shape,lens", [((1, 40, 60), dict(lz=1e-3)), ((50, 1, 1), dict(lx=1e-3, ly=1e-3)), ((20, 1, 30), dict(ly=1e-3))])
+def test_one_cell_axes_are_left_out_of_dt_3d(gpu, oracle_mod, shape, lens):
+    """the n = 1 rule of c-7 where it decides dt: the one-cell axes are SHORT, so counting them would shrink dt 10x or more
+    (dt3_kernel against the oracle rule that tests/test_oracle_dt_pins.py pins)"""
+    nz, ny, nx = shape
+    w, bc, gamma = si.smooth_random_3d(nx, ny, nz, seed=5, amp=5e-2)
+    a = gpu_run(gpu, w, bc, gamma, 6, **lens)
+    check(*a, *cpu_run(oracle_mod, w, bc, gamma, 6, **lens))
+    assert a[1][1] > 0.3 * 2e-3                  # far above any cfl * 1e-3 / cmax a counted short axis would give
+
+
 def test_z_invariant_3d_equals_the_2d_cuda_path(gpu, oracle_mod):
     """the 3-D kernels on a z-invariant state against the 2-D CUDA path (and both against their oracles)"""
     import torch

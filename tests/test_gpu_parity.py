@@ -557,3 +557,21 @@ def test_line_kernel_does_not_apply_beyond_one_cluster(gpu):
     s = gpu.Smaug(64, 2, gamma, bc)
     assert s.kernel_name().startswith("split_kernel")
     s.close()
+
+
+# ----------------------------------------------------------------------------- the n = 1 rule of c-7 where it decides dt
+@pytest.mark.parametrize("nx,ny,kernel,extra", [
+    (64, 1, 2, {}), (64, 1, 3, {}), (1, 64, 2, {}), (1200, 1, 2, {}), (300, 1, 2, dict(rk_order=2)), (90, 1, 3, dict(hd_on=0))])
+def test_one_cell_axis_is_left_out_of_dt(gpu, oracle_mod, nx, ny, kernel, extra):
+    """A one-dimensional problem whose collapsed axis is SHORT (L = 1e-3 over one cell): Delta / cmax along it would be
+    the minimum by far if the axis were counted, so dt_kernel (kernel = 3, and the grids the small-grid path does not
+    take) and line_step_kernel (kernel = 2 at ny = 1, which forms dt itself) must leave it out exactly as the oracle
+    does (tests/test_oracle_dt_pins.py pins the oracle's rule).  Every cell, (t, dt) and the maxima are compared exactly,
+    and dt is checked to be the long axis' term."""
+    n = max(nx, ny)
+    w, bc, gamma = si.brio_wu(n, 1, transpose=(nx == 1))
+    lens = dict(lx=1e-3, ly=1.0) if nx == 1 else dict(lx=1.0, ly=1e-3)
+    a = gpu_run(gpu, w, bc, gamma, 12, kernel=kernel, **lens, **extra)
+    b = cpu_run(oracle_mod, w, bc, gamma, 12, threads=1, **lens, **extra)
+    check(*a, *b)
+    assert 0.3 * (1.0 / n) / 6.0 < a[1][1] < 0.3 * (1.0 / n) / 2.0        # cmax between 2 and 6: the long axis decided
