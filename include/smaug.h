@@ -134,7 +134,8 @@ int smaug_get_kernel_info(smaug_ctx* ctx, int out[5]);
 
 /* Name of the fused stage kernel the context's current parameters select (static string, never NULL;
  * "?" for a NULL context): "split_kernel<128>" (role-split streaming form), "march_kernel<256>"
- * (single-role streaming form), "flux_kernel<128>" (streaming form without hyperdiffusion),
+ * (single-role streaming form), "flux_kernel<128>" or "flux_kernel<256>" (streaming form without hyperdiffusion; the
+ * strip width is picked per grid),
  * "line_step_kernel<128>" (small-grid path) or "stage_kernel<32,8,512>" (tiled form: SMAUG_PARAM_KERNEL = 0). */
 const char* smaug_get_kernel_name(smaug_ctx* ctx);
 
@@ -205,6 +206,10 @@ void smaug_destroy(smaug_ctx* ctx); /* NULL is a no-op */
  * and v_t are global (the paper's implied MAX all-reduce).  Members step in lockstep: per stage, all exchanges run
  * after all members' previous stage (events between the members' streams), then all stage kernels.
  * Contract: a decomposed run is BIT-IDENTICAL to the single-context run of the same global problem.
+ * Status of the several-GPU form: EXPERIMENTAL.  With all members on one device the contract is tested (tests/
+ * test_gpu_group.py).  With distinct devices the same kernels run over peer mappings and the reduction uses system-scope
+ * atomics (atomicMax_system: a device-scope atomic is atomic among the threads of one GPU only), but that path has not
+ * run on hardware yet; its test is collected only where two GPUs are visible.
  * State / background arrays are the GLOBAL ones, [6][ny][nx] / [4][ny][nx], host or device; the group scatters and
  * gathers the blocks.  All group calls synchronise before returning.  Errors as for the context calls. */
 int smaug_group_create(int px, int py, int nx, int ny, double gamma, const int bc[4], const double* bg,

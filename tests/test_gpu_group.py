@@ -110,6 +110,15 @@ def test_brio_wu_1d_over_four_members(gpu, oracle_mod):
     same(grp, ref)
 
 
+def test_group_leaves_a_short_one_cell_axis_out_of_dt(gpu, oracle_mod):
+    """the n = 1 rule of c-7 through the group: the leader's dt_kernel gets the GLOBAL cell counts, and the collapsed y axis
+    is short (L_y = 1e-3), so it would decide dt if it were counted"""
+    w, bc, gamma = si.brio_wu(400, 1)
+    ref = oracle_run(oracle_mod, w, bc, gamma, 30, ly=1e-3)
+    grp, _ = split(gpu, 3, 1, w, bc, gamma, 30, ly=1e-3)
+    same(grp, ref)
+
+
 def test_tiny_blocks_narrower_than_the_halo(gpu, oracle_mod):
     """Blocks of 2 cells: a ghost cell's source lies two members away."""
     w, bc, gamma = si.orszag_tang(8, 6)
@@ -124,3 +133,28 @@ def test_member_cannot_be_stepped_alone_and_devices_are_validated(gpu):
     h = C.c_void_p()
     bc = (C.c_int * 4)(0, 0, 0, 0)
     assert L.smaug_group_create(2, 1, 64, 64, 1.4, bc, None, (C.c_int * 2)(0, 99), C.byref(h)) == gpu.EINVAL
+
+
+def _visible_gpus():
+    try:
+        import torch
+        return torch.cuda.device_count()
+    except Exception:  # noqa: BLE001
+        return 0
+
+
+# Defined -- hence collected -- only where two GPUs are visible: a skip on the one-GPU boxes would read as coverage.
+if _visible_gpus() >= 2:
+    def test_group_across_two_devices_equals_unsplit(gpu, oracle_mod):
+        """The several-GPU form (peer pointers over NVLink, system-scope atomic maxima into the leader's slots, events
+        across devices): members on devices 0 and 1 against the unsplit run and the oracle, bit for bit."""
+        w, bc, gamma = si.orszag_tang(200, 120)
+        ref = oracle_run(oracle_mod, w, bc, gamma, 12)
+        same(unsplit(gpu, w, bc, gamma, 12), ref)
+        import torch
+        g = gpu.SmaugGroup(2, 1, 200, 120, gamma, bc, devices=[0, 1])
+        g.set_state(torch.from_numpy(w))
+        g.step(12, 0.3)
+        out = g.get_state(torch.empty((6, 120, 200), dtype=torch.float64)).numpy(), g.time(), g.wavespeeds()
+        g.close()
+        same(out, ref)
