@@ -20,6 +20,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <new>
 #include <string>
 #include <vector>
 
@@ -697,6 +698,7 @@ struct Ctx {
   int cur = 0;                  // reduction set holding the maxima of the state (0 or 4)
   long long launches = 0;
   bool timing = false;
+  bool timing_broken = false;   // an event could not be created / recorded: timing was switched off, the totals are void
   std::vector<cudaEvent_t> ev;
   std::vector<int> ev_kind;
   size_t ev_used = 0;
@@ -741,15 +743,28 @@ struct Timed {
   ~Timed() {
     if (c.timing) mark();
   }
+  // Never throws and never fails the step: if the event pool cannot grow or an event cannot be recorded, timing is
+  // abandoned (smaug3_get_kernel_timing then reports it) and the launches go on untimed.
+  void give_up() {
+    cudaGetLastError();
+    c.timing = false;
+    c.timing_broken = true;
+  }
   void mark() {
     if (c.ev_used == c.ev.size()) {
-      cudaEvent_t e;
-      cudaEventCreate(&e);
-      c.ev.push_back(e);
-      c.ev_kind.push_back(kind);
+      cudaEvent_t e = nullptr;
+      if (cudaEventCreate(&e) != cudaSuccess) return give_up();
+      try {
+        c.ev_kind.push_back(kind);
+        c.ev.push_back(e);
+      } catch (...) {
+        cudaEventDestroy(e);
+        return give_up();
+      }
     }
     c.ev_kind[c.ev_used] = kind;
-    cudaEventRecord(c.ev[c.ev_used++], c.stream);
+    if (cudaEventRecord(c.ev[c.ev_used], c.stream) != cudaSuccess) return give_up();
+    ++c.ev_used;
   }
 };
 
@@ -788,6 +803,18 @@ void launch_cflux(Ctx& c, const Params3& p, const V8& in) {
   else cflux3_kernel<false><<<gr, SBLOCK, 0, c.stream>>>(g, p, cv8(in), cv4(c.der[c.dcur]), io);
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: raised once per (instantiation,
+// device).  A failure leaves the bit clear; the launch that follows then fails and the step reports it.
+template <typename K>
+void raise_smem_once(K kern, int device, unsigned long long& mask) {
+  if (device >= 0 && device < 64 && (mask >> device & 1ULL)) return;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE3_SMEM) == cudaSuccess) {
+    if (device >= 0 && device < 64) mask |= 1ULL << device;
+  } else {
+    cudaGetLastError();
+  }
+}
+
 template <int COMBINE, int WS>
 void launch_assemble(Ctx& c, const AsmArgs& a) {
   Timed t(c, 4);
@@ -798,11 +825,12 @@ void launch_assemble(Ctx& c, const AsmArgs& a) {
     const unsigned gx = (unsigned)((g.n[0] + TX - 1) / TX), gz = (unsigned)((g.n[2] + TZ - 1) / TZ);
     const dim3 gr(SMAUG3_ZFAST ? gz : gx, (unsigned)((g.n[1] + TY - 1) / TY), SMAUG3_ZFAST ? gx : gz);
     const dim3 bl(TX, TY, TZ);
+    static unsigned long long raised_hd = 0, raised_plain = 0;      // per instantiation: devices already configured
     if (c.hd_on) {
-      cudaFuncSetAttribute(stage3_kernel<COMBINE, WS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE3_SMEM);
+      raise_smem_once(stage3_kernel<COMBINE, WS, true>, c.device, raised_hd);
       stage3_kernel<COMBINE, WS, true><<<gr, bl, STAGE3_SMEM, c.stream>>>(a, kin);
     } else {
-      cudaFuncSetAttribute(stage3_kernel<COMBINE, WS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE3_SMEM);
+      raise_smem_once(stage3_kernel<COMBINE, WS, false>, c.device, raised_plain);
       stage3_kernel<COMBINE, WS, false><<<gr, bl, STAGE3_SMEM, c.stream>>>(a, kin);
     }
     return;
@@ -894,7 +922,8 @@ int smaug3_create(int nx, int ny, int nz, double gamma, const int bc[6], void* s
     cudaGetLastError();
     return fail(SMAUG3_ECUDA, "no CUDA device: libsmaug has no CPU fallback");
   }
-  Ctx* c = new Ctx();
+  Ctx* c = new (std::nothrow) Ctx();
+  if (!c) return fail(SMAUG3_ENOMEM, "host allocation failed");
   make_grid(nx, ny, nz, bc, c->g);
   if (c->g.vol >= (1LL << 31)) { delete c; return fail(SMAUG3_EINVAL, "a padded volume must have fewer than 2^31 elements"); }
   if (nz + 6 > 65535 || ny + 6 > 65535) { delete c; return fail(SMAUG3_EINVAL, "ny, nz must be below 65529"); }
@@ -907,7 +936,12 @@ int smaug3_create(int nx, int ny, int nz, double gamma, const int bc[6], void* s
     delete c;
     return fail(SMAUG3_ENOMEM, "device allocation of " + std::to_string(bytes) + " bytes failed");
   }
-  cudaMemsetAsync(c->mem, 0, bytes, c->stream);
+  if (cudaMemsetAsync(c->mem, 0, bytes, c->stream) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(c->mem);
+    delete c;
+    return fail(SMAUG3_ECUDA, "clearing the device memory failed");
+  }
   double* p = c->mem;
   auto take = [&]() { double* r = p; p += c->g.vol; return r; };
   for (int b = 0; b < 4; ++b)
@@ -1056,7 +1090,10 @@ int smaug3_get_launch_count(smaug3_ctx* ctx, long long* n) {
 int smaug3_set_kernel_timing(smaug3_ctx* ctx, int on) {
   if (!ctx) return fail(SMAUG3_EINVAL, "NULL ctx");
   Ctx& c = *CTX(ctx);
+  DeviceGuard guard_(c.device);
+  CUDA_TRY(cudaStreamSynchronize(c.stream));      // recorded events may still be pending: settle them before the pool is reused
   c.timing = on != 0;
+  c.timing_broken = false;
   c.ev_used = 0;
   for (int k = 0; k < 5; ++k) { c.ms[k] = 0; c.nk[k] = 0; }
   return SMAUG3_OK;
@@ -1067,6 +1104,7 @@ int smaug3_get_kernel_timing(smaug3_ctx* ctx, double ms[5], long long n[5]) {
   Ctx& c = *CTX(ctx);
   DeviceGuard guard_(c.device);
   CUDA_TRY(cudaStreamSynchronize(c.stream));
+  if (c.timing_broken) return fail(SMAUG3_ECUDA, "kernel timing was abandoned: a CUDA event could not be created or recorded");
   for (size_t e = 0; e + 1 < c.ev_used; e += 2) {
     float t = 0;
     CUDA_TRY(cudaEventElapsedTime(&t, c.ev[e], c.ev[e + 1]));
