@@ -161,6 +161,10 @@ __device__ __forceinline__ void kappa_family(const double (&m3)[N], const double
   for (int q = 1; q < N; ++q) lo = min(lo, __double2hiint(m1[q]));
 #pragma unroll
   for (int q = 0; q < N; ++q) k[q] = cv * ddiv(m3[q], m1[q]);
+  // Only a TINY M1 needs the redo.  A non-finite M1 (infinite or NaN: a blown-up state) passes this test, and rightly so:
+  // kappa_ratio would leave it as it is (it is not zero) and scale by 1.0 (it is not tiny), i.e. form the same
+  // cv * ddiv(m3, m1) from the same operands, so both forms return the same bits there too.  (An upper bound in the vote
+  // was measured: +2.4 % per stage at 8000^2 for no difference in any result.)
   if (__any_sync(0xffffffffu, lo < ORDINARY_HI)) {
 #pragma unroll
     for (int q = 0; q < N; ++q) k[q] = kappa_ratio(m3[q], m1[q], cv);
