@@ -12,12 +12,16 @@ Prints ONE JSON line (rank 0).  `value` = cell-updates/s with the state resident
 through the C ABI with HOST buffers (set_state H2D + steps + get_state D2H inside the timed region);
 `roofline` = algorithmic bytes of the fused stage kernel / its CUDA-event duration vs the measured HBM peak;
 `cpu_baseline` = the oracle, as it stands, timed on one host core on a bounded sample of the same workload.
+The default invocation (one GPU, no workload flags) also carries `rows`: compact entries (ms_per_step, roofline.frac,
+kernel, clocks; each timed for >= 0.5 s) for 8000 x 8000 without hyperdiffusion, BASELINE configs 1-4, 8000 x 8000 on a
+uniform background, the 256^3 three-dimensional form and the 2 x 2 decomposition group; `--no-rows` leaves them out.
 N > 1: the path does not shard ("replicas only") -- every rank runs an independent replica.
 """
 from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -188,6 +192,90 @@ def oracle_rate(sample_n, steps, warmup=0, threads=1, kind="ot"):
     return sample_n * sample_n * steps / el, el
 
 
+# Rows the default invocation adds beside the headline (BASELINE.json lists five configs, SURVEY 8(d):
+# "additionally report each OT size with HD_ON=0"): (workload, hyperdiffusion on, decomposition or None)
+ROWS = [("orszag_tang_8000", False, None), ("brio_wu_800", True, None), ("orszag_tang_1000", True, None),
+        ("orszag_tang_2044", True, None), ("orszag_tang_4000", True, None), ("orszag_tang_8000_bg", True, None),
+        ("orszag_tang_3d_256", True, None), ("orszag_tang_8000", True, (2, 2))]
+
+
+def compact_row(pkg, name, hd=True, decomp=None, min_ms=500.0, device=0, state=None):
+    """One entry of `rows`: the workload timed on the device for at least `min_ms` (step count calibrated from a short
+    untimed run that also serves as warm-up), once as the product runs it (CUDA-graph replay where the library uses
+    it) for ms_per_step, and -- for a single 2-D context -- once more with CUDA events around the stage kernels for
+    the roofline fraction of the fused stage kernel.  Clocks are sampled from before the calibration run to the end."""
+    import torch
+    nx, ny, kind = WORKLOADS[name]
+    sampler = ClockSampler(device)
+    three_d = kind == "ot3d"
+    if three_d:
+        w_np, bc, gamma = si.orszag_tang_3d(nx)
+        sim = pkg.Smaug3D(nx, nx, nx, gamma, bc, hd_on=1 if hd else 0)
+        cells, has_bg = float(nx) ** 3, False
+        sim.set_state(torch.from_numpy(w_np))
+    else:
+        w_np, bc, gamma, bg_np, (gx, gy) = state if state is not None else make_state(name)
+        bg = None if bg_np is None else torch.from_numpy(bg_np).cuda(device)
+        has_bg = bg_np is not None
+        params = dict(hd_on=1 if hd else 0, gx=gx, gy=gy)
+        sim = (pkg.SmaugGroup(decomp[0], decomp[1], nx, ny, gamma, bc, bg=bg, **params) if decomp
+               else pkg.Smaug(nx, ny, gamma, bc, bg=bg, device=torch.device("cuda", device), **params))
+        cells = float(nx) * ny
+        sim.set_state(w_np if torch.is_tensor(w_np) else torch.from_numpy(w_np))
+    del w_np
+
+    def timed(k):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        sim.step(k, 0.3)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    k0 = 200 if cells < 1e4 else (20 if cells < 2e6 else 4)
+    timed(k0)                                                   # warm-up (graph capture, smem attributes)
+    per = timed(k0) / k0
+    K = int(min(max(8, math.ceil(min_ms / per)), 200000))
+    ms = timed(K)
+    row = {"workload": name, "hd": hd, "steps": K, "ms_per_step": ms / K, "value": cells * K / (ms * 1e-3), "unit": UNIT,
+           "launch_path": "as smaug_step runs it (CUDA-graph replay where the library uses it)"}
+    peak, _ = peaks()
+    if decomp:
+        row["decomposition"] = f"{decomp[0]}x{decomp[1]} members on one device (smaug_group_*)"
+        row["kernel"] = "smaug::split_kernel per member + group_pull_kernel"
+        row["roofline"] = {"frac": cells * BYTES_PER_CELL_UPDATE / (ms / K * 1e-3) / 1e9 / peak,
+                           "basis": "whole step: 576 B per cell-update / ms_per_step (exchange and barriers included)"}
+    elif three_d:
+        row["kernel"] = "smaug3 RK stage (ghost3, kappa3, stage3)"
+        row["roofline"] = {"frac": cells * 768.0 / (ms / K * 1e-3) / 1e9 / peak,
+                           "basis": "whole step: 768 B per cell-update of a fully fused stage / ms_per_step"}
+    else:
+        row["kernel"] = "smaug::" + sim.kernel_name()
+        bpcu = bytes_per_cell_update(has_bg, 4)
+        if sim.kernel_name().startswith("line_step_kernel"):
+            row["roofline"] = {"frac": None, "basis": "whole steps in one persistent cluster launch, state in distributed "
+                                                      "shared memory: no HBM traffic per step to set against a roofline"}
+        else:
+            sim.set_kernel_timing(True)
+            k2 = max(8, K // 4)
+            ms2 = timed(k2)
+            stage_ms, stage_n = sim.kernel_timing()
+            sim.set_kernel_timing(False)
+            avg = stage_ms / max(stage_n, 1)
+            ach = bpcu / 4 * cells / (avg * 1e-3) / 1e9
+            row["roofline"] = {"frac": ach / peak, "achieved": ach, "unit": "GB/s", "avg_launch_ms": avg, "launches_timed": stage_n,
+                               "bytes_per_launch": bpcu / 4 * cells, "ms_per_step_with_events": ms2 / k2,
+                               "basis": "fused stage kernel alone: algorithmic bytes per launch / CUDA-event duration"}
+            if cells * 48 * 4 < 4e8:
+                row["roofline"]["l2"] = "working set comparable to L2 (126 MB): DRAM traffic is below algorithmic"
+    t_sim, dt_last = sim.time()
+    row["sim"] = {"t": t_sim, "last_dt": dt_last}
+    row["clocks"] = sampler.stop()
+    sim.close()
+    return row
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric/unit/config keys (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -322,7 +410,18 @@ def run_ours(args):
             "sim": {"t": t_sim, "last_dt": dt_last, "finite": finite},
         }
         if line["fp64_pipe"]:
-            line["fp64_pipe"]["frac"] = line["fp64_pipe"]["achieved"] / line["fp64_pipe"]["peak"]
+            fp = line["fp64_pipe"]
+            fp["frac"] = fp["achieved"] / fp["peak"]
+            # the two floors of one launch: the kernel can be no faster than the higher one
+            rf = line["roofline"]
+            rf["hbm_floor_ms"] = per_launch_bytes / (peak * 1e9) * 1e3
+            rf["fp64_floor_ms"] = fp64_per_cell * cells / (fp["peak"] * 1e12) * 1e3
+            if rf["fp64_floor_ms"] > rf["hbm_floor_ms"]:
+                rf["bound"] = "alu"
+                rf["bound_note"] = ("the fp64 pipe sets the higher floor of this kernel (fp64_floor_ms > hbm_floor_ms), so it "
+                                    "is ALU-bound in principle; achieved / peak / frac stay the HBM figures north_star asks "
+                                    "for, the ALU figures are in `fp64_pipe`; frac can reach at most hbm_floor_ms / fp64_floor_ms")
+                rf["max_hbm_frac_at_full_fp64_pipe"] = rf["hbm_floor_ms"] / rf["fp64_floor_ms"]
         if not args.no_cpu_baseline and world == 1:
             n_s, steps_s = 1000, 6
             kind = WORKLOADS[name][2] if has_bg else "ot"
@@ -332,6 +431,16 @@ def run_ours(args):
                 "sample": f"{ {'strat': 'stratified atmosphere', 'otbg': 'Orszag-Tang on a uniform background'}.get(kind, 'Orszag-Tang')} {n_s}x{n_s} (same IC and "
                           f"parameters), {steps_s} steps, {el:.1f} s, "
                           f"1 of {os.cpu_count()} host cores"}
+        if args.rows and world == 1:
+            sim.close()
+            rows = []
+            for wl, hd, decomp in ROWS:
+                try:
+                    st = (w_host, bc, gamma, None, (0.0, 0.0)) if wl == name and not has_bg else None
+                    rows.append(compact_row(pkg, wl, hd=hd, decomp=decomp, device=local, state=st))
+                except Exception as e:  # noqa: BLE001
+                    rows.append({"workload": wl, "hd": hd, "error": repr(e)})
+            line["rows"] = rows
         print(json.dumps(line), flush=True)
     sim.close()
     if world > 1:
@@ -493,9 +602,15 @@ def main():
     ap.add_argument("--decomp", default=None, metavar="PXxPY",
                     help="extra row (SURVEY 8(f) NEXT-1): run the workload as a PX x PY decomposition group on ONE device "
                          "(halo pull through peer pointers, shared reduction, lockstep stages) and report its rate")
+    ap.add_argument("--no-rows", action="store_true",
+                    help="leave out the `rows` list (the other BASELINE configs, HD off, background, 3-D and 2x2-group "
+                         "rows, each timed for >= 0.5 s) that the default single-GPU invocation adds to its line")
     ap.add_argument("--no-hd", action="store_true",
                     help="hyperdiffusion off (the 'Without HD' column of the paper's Table 1); extra row, not the default")
     args = ap.parse_args()
+    # the extra rows ride on the default headline invocation only (one GPU, default workload and scheme)
+    args.rows = (not args.no_rows and args.impl == "ours" and args.gpus == 1 and args.workload == "orszag_tang_8000"
+                 and not args.no_hd and args.rk_order == 4 and not args.decomp and not args.no_kernel_timing)
     if args.impl == "reference":
         run_reference(args)
     elif WORKLOADS[args.workload][2] == "ot3d":
