@@ -13,7 +13,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
-LIB_PATH = os.environ.get("SMAUG_LIB") or os.path.join(_HERE, "libsmaug.so")   # SMAUG_LIB: a variant build (tuning)
+LIB_PATH = os.path.join(_HERE, "libsmaug.so")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 BC_PERIODIC, BC_OPEN, BC_FIXED = 0, 1, 2
@@ -35,8 +35,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in _sources() + [os.path.join(INCLUDE, "smaug.h"), os.path.join(INCLUDE, "smaug3d.h")])
     if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        extra = os.environ.get("SMAUG_NVCC_EXTRA", "").split()     # e.g. -DSMAUG_TW=24 for tuning sweeps
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", LIB_PATH, os.path.join(_CSRC, "smaug.cu"), os.path.join(_CSRC, "smaug3d.cu"),
                os.path.join(_CSRC, "smaug_static.cu")]
         subprocess.run(cmd, check=True)
@@ -48,9 +47,7 @@ def lib() -> C.CDLL:
     global _lib
     if _lib is None:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        if os.environ.get("SMAUG_LIB"):
-            pass                            # an explicitly chosen variant build is loaded as it is
-        elif os.path.exists(nvcc):
+        if os.path.exists(nvcc):
             try:
                 build()                     # no-op unless the library is missing or older than csrc/ or smaug.h
             except Exception as e:  # noqa: BLE001
