@@ -569,6 +569,13 @@ def run_decomp(args):
     ms_grp = timed(grp)
     t_grp = grp.time()
     n_stage, n_exch = grp.launch_count()
+    # the paper's three terms and tau, from CUDA events on the members' streams over K more steps
+    grp.set_timing(True)
+    t0 = time.perf_counter()
+    grp.step(K, 0.3)
+    ms_tau = (time.perf_counter() - t0) * 1e3
+    tau = grp.tau()
+    grp.set_timing(False)
     grp.close()
     cells = float(nx) * ny
     line = {
@@ -582,6 +589,14 @@ def run_decomp(args):
         "decomposition_cost": ms_grp / ms_one - 1.0,
         "bit_identical_time": list(t_grp) == list(t_one),
         "gpu_launches": n_stage + n_exch, "exchange_launches": n_exch,
+        "tau": {"T_comp_ms_per_step": tau["t_comp"] / K, "T_comm_ms_per_step": tau["t_comm"] / K,
+                "T_idle_ms_per_step": tau["t_idle"] / K, "tau": tau["tau"], "ms_per_step_while_timed": ms_tau / K,
+                "definition": "PAPER.md:138-144: T = T_comp + T_comm + T_idle, tau = ln(T_comp / (T_comm + T_idle)); mean over "
+                              "the members; T_comm = halo-pull kernels, T_comp = stage kernels, T_idle = a member's wait "
+                              "in the inter-member barriers after its own work",
+                "caveat": "all members share ONE device here: a member's intervals include the time its kernels wait for "
+                          "or share the SMs with the other members' kernels, so tau describes the lockstep schedule on "
+                          "one GPU, not a link; across GPUs the same call measures the paper's quantity"},
     }
     print(json.dumps(line), flush=True)
 

@@ -223,6 +223,16 @@ int smaug_group_get_time(smaug_group* grp, double* t, double* last_dt);
 int smaug_group_get_wavespeeds(smaug_group* grp, double out[4]);
 /* kernels launched so far: stage / dt / reduction kernels of all members, and exchange (halo) kernels */
 int smaug_group_get_launch_count(smaug_group* grp, long long* stage_and_aux, long long* exchange);
+/* The paper's load-balance measure: T = T_comp + T_comm + T_idle and tau = ln(T_comp / (T_comm + T_idle)).
+ * smaug_group_set_timing(grp, 1) starts recording CUDA events on every member's stream (and clears what was recorded);
+ * smaug_group_get_tau returns out = { T_comp, T_comm, T_idle, tau }, times in milliseconds, mean over the members, of all
+ * steps since then:  T_comm = the halo-pull kernels (the whole of the paper's exchange_halo),  T_comp = the stage kernels
+ * (and the leader's dt kernel),  T_idle = what a member's stream spends in the inter-member barriers after its own work
+ * is done.  With all members on ONE device they share its SMs, so a member's intervals contain the time its kernels
+ * wait for, or share the device with, the other members' kernels: the three terms then sum to the wall time of the
+ * steps, and tau describes the lockstep schedule, not a communication link.  Both calls synchronise.  0 = timing off. */
+int smaug_group_set_timing(smaug_group* grp, int on);
+int smaug_group_get_tau(smaug_group* grp, double out[4]);
 void smaug_group_destroy(smaug_group* grp); /* destroys the members too; NULL is a no-op */
 /* Host-only view of the decomposition logic (needs no GPU; used by the CPU tests): for ghost cell (i, j) -- local
  * indices outside [0, nx_m) x [0, ny_m) -- of member `member`, out = { x0, y0, nx_m, ny_m of the member,  source member

@@ -93,6 +93,8 @@ def lib() -> C.CDLL:
         L.smaug_group_get_time.argtypes = [vp, dp, dp]
         L.smaug_group_get_wavespeeds.argtypes = [vp, dp]
         L.smaug_group_get_launch_count.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+        L.smaug_group_set_timing.argtypes = [vp, C.c_int]
+        L.smaug_group_get_tau.argtypes = [vp, dp]
         L.smaug_group_destroy.argtypes = [vp]
         L.smaug_group_destroy.restype = None
         L.smaug_group_map_cell.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, ip, C.c_int, C.c_int, C.c_int, C.c_int, ip]
@@ -329,6 +331,17 @@ class SmaugGroup:
         a, b = C.c_longlong(), C.c_longlong()
         _check(lib().smaug_group_get_launch_count(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def set_timing(self, on=True):
+        """smaug_group_set_timing: start (and clear) the event record behind tau()."""
+        _check(lib().smaug_group_set_timing(self._h, int(on)))
+
+    def tau(self):
+        """smaug_group_get_tau: dict(t_comp, t_comm, t_idle in ms -- mean over the members, all steps since
+        set_timing(True) -- and tau = ln(t_comp / (t_comm + t_idle)), PAPER.md:138-144)."""
+        o = (C.c_double * 4)()
+        _check(lib().smaug_group_get_tau(self._h, o))
+        return dict(t_comp=o[0], t_comm=o[1], t_idle=o[2], tau=o[3])
 
     def close(self):
         if getattr(self, "_h", None):

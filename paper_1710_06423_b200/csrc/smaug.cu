@@ -170,6 +170,13 @@ struct smaug_group {
   int state_set = 0;
   long long exchange_launches = 0;
   bool pending_status = false;
+  // tau measurement (smaug_group_set_timing): per member a list of timestamps on its stream, each
+  // tagged with what has just finished there -- 0: the member's own work (it now enters a barrier), 1: the barrier's
+  // waits, 2: the halo pull.  The gaps 0->1, 1->2, 2->0 are T_idle, T_comm, T_comp of that member.
+  bool tau_on = false, tau_broken = false;
+  std::vector<std::vector<cudaEvent_t>> tev;
+  std::vector<std::vector<unsigned char>> tkind;
+  std::vector<size_t> tused;
 };
 
 namespace {
@@ -1060,18 +1067,42 @@ int group_check(smaug_group* g) {
   return SMAUG_OK;
 }
 
+// A timestamp on member k's stream for the tau measurement (the member's device is current).  Never throws and never
+// fails the step: if the pool cannot grow or the event cannot be recorded the measurement is abandoned and
+// smaug_group_get_tau says so.
+void tau_mark(smaug_group* g, int k, unsigned char kind) {
+  if (!g->tau_on) return;
+  auto give_up = [&]() { cudaGetLastError(); g->tau_on = false; g->tau_broken = true; };
+  if (g->tused[k] == g->tev[k].size()) {
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) return give_up();
+    try {
+      g->tkind[k].push_back(kind);
+      g->tev[k].push_back(e);
+    } catch (...) {
+      cudaEventDestroy(e);
+      return give_up();
+    }
+  }
+  g->tkind[k][g->tused[k]] = kind;
+  if (cudaEventRecord(g->tev[k][g->tused[k]], g->m[k]->stream) != cudaSuccess) return give_up();
+  ++g->tused[k];
+}
+
 // Every member's stream waits for everything enqueued so far on every other member's stream.
 int group_barrier(smaug_group* g) {
   if (g->one_stream) return SMAUG_OK;
   const int n = (int)g->m.size();
   for (int k = 0; k < n; ++k) {
     DeviceGuard dg(g->m[k]->device);
+    tau_mark(g, k, 0);
     CU(cudaEventRecord(g->ev[k], g->m[k]->stream));
   }
   for (int k = 0; k < n; ++k) {
     DeviceGuard dg(g->m[k]->device);
     for (int o = 0; o < n; ++o)
       if (o != k) CU(cudaStreamWaitEvent(g->m[k]->stream, g->ev[o], 0));
+    tau_mark(g, k, 1);
   }
   return SMAUG_OK;
 }
@@ -1095,6 +1126,7 @@ int group_exchange(smaug_group* g, int buf, int nplanes, int freeze) {
     c->launches++;
     g->exchange_launches++;
     CU(cudaGetLastError());
+    tau_mark(g, (int)k, 2);
   }
   return SMAUG_OK;
 }
@@ -1178,6 +1210,8 @@ void smaug_group_destroy(smaug_group* g) {
     cudaStreamSynchronize(st);
     if (k < g->table.size() && g->table[k]) cudaFree(g->table[k]);
     if (k < g->ev.size() && g->ev[k]) cudaEventDestroy(g->ev[k]);
+    if (k < g->tev.size())
+      for (cudaEvent_t e : g->tev[k]) cudaEventDestroy(e);
     g->m[k]->group = nullptr;
     smaug_destroy(g->m[k]);
     if (st) cudaStreamDestroy(st);
@@ -1355,7 +1389,53 @@ int smaug_group_step(smaug_group* g, int n_steps, double cfl) {
   for (int s = 0; s < n_steps; ++s)
     if (int rc = group_enqueue_step(g, cfl)) return rc;
   if (n_steps > 0) g->pending_status = true;
+  if (g->tau_on)                                  // closes the last stage's compute interval of every member
+    for (size_t k = 0; k < g->m.size(); ++k) {
+      DeviceGuard dg(g->m[k]->device);
+      tau_mark(g, (int)k, 0);
+    }
   return group_status(g);
+}
+
+int smaug_group_set_timing(smaug_group* g, int on) {
+  if (int rc = group_check(g)) return rc;
+  if (int rc = group_sync(g)) return rc;          // recorded events may still be pending
+  const size_t n = g->m.size();
+  try {
+    g->tev.resize(n);
+    g->tkind.resize(n);
+    g->tused.assign(n, 0);
+  } catch (...) {
+    return fail(SMAUG_ENOMEM, "host allocation failed");
+  }
+  g->tau_on = on != 0;
+  g->tau_broken = false;
+  return SMAUG_OK;
+}
+
+int smaug_group_get_tau(smaug_group* g, double out[4]) {
+  if (int rc = group_check(g)) return rc;
+  if (!out) return fail(SMAUG_EINVAL, "out is NULL");
+  if (int rc = group_sync(g)) return rc;
+  if (g->tau_broken) return fail(SMAUG_ECUDA, "the tau measurement was abandoned: a CUDA event could not be created or recorded");
+  if (g->tused.size() != g->m.size()) return fail(SMAUG_EINVAL, "timing was never switched on (smaug_group_set_timing)");
+  double sum[3] = {0.0, 0.0, 0.0};                // idle, comm, comp, summed over members
+  for (size_t k = 0; k < g->m.size(); ++k) {
+    DeviceGuard dg(g->m[k]->device);
+    for (size_t e = 0; e + 1 < g->tused[k]; ++e) {
+      const int a = g->tkind[k][e], b = g->tkind[k][e + 1];
+      if (a == 0 && b == 0) continue;             // end of one call -> first barrier of the next: host time, not the step's
+      float t = 0.f;
+      CU(cudaEventElapsedTime(&t, g->tev[k][e], g->tev[k][e + 1]));
+      sum[a == 0 ? 0 : (b == 2 ? 1 : 2)] += t;    // 0->1 idle; 1->2 comm; 2->0 and 1->0 (dt kernel / nothing) comp
+    }
+  }
+  const double n = (double)g->m.size();
+  out[0] = sum[2] / n;
+  out[1] = sum[1] / n;
+  out[2] = sum[0] / n;
+  out[3] = std::log(out[0] / (out[1] + out[2]));
+  return SMAUG_OK;
 }
 
 int smaug_group_get_state(smaug_group* g, double* w) {

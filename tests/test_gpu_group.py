@@ -135,6 +135,34 @@ def test_member_cannot_be_stepped_alone_and_devices_are_validated(gpu):
     assert L.smaug_group_create(2, 1, 64, 64, 1.4, bc, None, (C.c_int * 2)(0, 99), C.byref(h)) == gpu.EINVAL
 
 
+def test_tau_terms_add_up_to_the_step_time(gpu):
+    """smaug_group_get_tau: with timing on, the three terms of every member cover its stream's time
+    gap-free, so their sum is the device time of the steps (checked against CUDA events around the call, loosely: the
+    marks sit inside the call), each term is positive, tau is their log ratio, and the state is unchanged by timing."""
+    import math
+    import torch
+    w, bc, gamma = si.orszag_tang(600, 400)
+    g = gpu.SmaugGroup(2, 2, 600, 400, gamma, bc)
+    g.set_state(torch.from_numpy(w))
+    g.step(4, 0.3)
+    g.set_timing(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    g.step(10, 0.3)
+    e1.record()
+    torch.cuda.synchronize()
+    tau = g.tau()
+    timed = g.get_state(torch.empty((6, 400, 600), dtype=torch.float64)).numpy(), g.time()
+    g.close()
+    total = tau["t_comp"] + tau["t_comm"] + tau["t_idle"]
+    assert tau["t_comp"] > 0 and tau["t_comm"] > 0 and tau["t_idle"] >= 0
+    assert 0.5 * e0.elapsed_time(e1) < total < 1.05 * e0.elapsed_time(e1), (tau, e0.elapsed_time(e1))
+    assert math.isclose(tau["tau"], math.log(tau["t_comp"] / (tau["t_comm"] + tau["t_idle"])), rel_tol=1e-12)
+    plain, _ = split(gpu, 2, 2, w, bc, gamma, 14)
+    assert np.array_equal(timed[0], plain[0]) and tuple(timed[1]) == tuple(plain[1])
+
+
 def _visible_gpus():
     try:
         import torch
