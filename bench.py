@@ -565,7 +565,10 @@ def run_decomp(args):
     ms_one = timed(one)
     t_one = one.time()
     one.close()
-    grp = pkg.SmaugGroup(px, py, nx, ny, gamma, bc, bg=bg, **params)
+    devices = [int(v) for v in args.devices.split(",")] if args.devices else None
+    if devices is not None and len(devices) != px * py:
+        raise SystemExit(f"bench.py: --devices needs {px * py} entries (member b * px + a runs on devices[b * px + a])")
+    grp = pkg.SmaugGroup(px, py, nx, ny, gamma, bc, bg=bg, devices=devices, **params)
     ms_grp = timed(grp)
     t_grp = grp.time()
     n_stage, n_exch = grp.launch_count()
@@ -583,7 +586,9 @@ def run_decomp(args):
         "ms_per_step": ms_grp / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": name, "nx": nx, "ny": ny, "cfl": 0.3, "hd": not args.no_hd, "rk_order": args.rk_order,
-                   "decomposition": f"{px}x{py} members on one device (smaug_group_*)",
+                   "decomposition": f"{px}x{py} members on " + ("one device" if devices is None or len(set(devices)) == 1
+                                                                 else f"devices {devices} (one process, peer access; EXPERIMENTAL path)")
+                                    + " (smaug_group_*)",
                    "timing": "host wall clock around the synchronising step call, after a device synchronise"},
         "unsplit": {"value": cells * K / (ms_one * 1e-3), "ms_per_step": ms_one / K},
         "decomposition_cost": ms_grp / ms_one - 1.0,
@@ -617,6 +622,10 @@ def main():
     ap.add_argument("--decomp", default=None, metavar="PXxPY",
                     help="extra row (SURVEY 8(f) NEXT-1): run the workload as a PX x PY decomposition group on ONE device "
                          "(halo pull through peer pointers, shared reduction, lockstep stages) and report its rate")
+    ap.add_argument("--devices", default=None, metavar="D0,D1,...",
+                    help="with --decomp: run ONE group across these visible devices in this single process (member "
+                         "b * PX + a on the (b * PX + a)-th entry; the devices need peer access).  Default: all members on "
+                         "the current device.  The several-GPU path is experimental: it has not run on hardware yet")
     ap.add_argument("--no-rows", action="store_true",
                     help="leave out the `rows` list (the other BASELINE configs, HD off, background, 3-D and 2x2-group "
                          "rows, each timed for >= 0.5 s) that the default single-GPU invocation adds to its line")
