@@ -248,8 +248,13 @@ def compact_row(pkg, name, hd=True, decomp=None, min_ms=500.0, device=0, state=N
                            "basis": "whole step: 576 B per cell-update / ms_per_step (exchange and barriers included)"}
     elif three_d:
         row["kernel"] = "smaug3 RK stage (ghost3, kappa3, stage3)"
+        cap = ncu_capture(name)
         row["roofline"] = {"frac": cells * 768.0 / (ms / K * 1e-3) / 1e9 / peak,
-                           "basis": "whole step: 768 B per cell-update of a fully fused stage / ms_per_step"}
+                           "basis": "whole step: 768 B per cell-update of a fully fused stage / ms_per_step; the kernels as "
+                                    "built move more than that (kappa / Phi volumes go through HBM): see traffic",
+                           "algorithmic_bytes_per_stage": 192.0 * cells, "traffic": cap.get("dram_bytes"),
+                           "traffic_over_algorithmic": (cap["dram_bytes"] / (192.0 * cells)) if cap.get("dram_bytes") else None,
+                           "traffic_source": cap.get("capture")}
     else:
         row["kernel"] = "smaug::" + sim.kernel_name()
         bpcu = bytes_per_cell_update(has_bg, 4)
@@ -511,6 +516,9 @@ def run_3d(args):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "frac_of_nominal_8TBs": achieved / 8000.0, "traffic": cap.get("dram_bytes"),
                      "traffic_source": cap.get("capture"), "peak_source": peak_src,
+                     "traffic_over_algorithmic": (cap["dram_bytes"] / (bpcu / stages * cells)) if cap.get("dram_bytes") else None,
+                     "achieved_note": "`achieved` divides the bytes a fully fused stage must move by the measured time; the "
+                                      "kernels as built move `traffic` (ncu, per stage), several times more",
                      "kernel": "smaug3 RK stage (ghost3, kappa3, stage3); "
                                f"largest share: {top}",
                      "bytes_per_launch": bpcu / stages * cells, "avg_launch_ms": stage_ms,
